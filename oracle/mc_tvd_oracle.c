@@ -1,0 +1,497 @@
+/*
+ * oracle/mc_tvd_oracle.c -- CPU ORACLE. TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+ * See mc_tvd_oracle.h for scope, layout and the list of parity pins.
+ *
+ * Every function cites the passage of /root/reference/PAPER.md it restates
+ * (arXiv 2411.10372) or the DESIGN.md reading (R1..R18) it takes where the
+ * paper is silent.  Plain C99, fp64, single thread, whole-array passes in the
+ * paper's order; build with -O2 -ffp-contract=off (no FMA contraction).
+ *
+ * Internally a 2-D problem is the 3-D one with ny = 1 and rho*u_y = 0: every
+ * y-difference is then an exact zero, so the 4-field result is bit-identical
+ * to carrying five fields (tests/test_oracle_pins.py::test_2d_is_3d_with_ny1).
+ */
+#include "mc_tvd_oracle.h"
+
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+
+enum { Q_RHO = 0, Q_MX = 1, Q_MY = 2, Q_MZ = 3, Q_E = 4 };   /* X of Eq. 27 */
+enum { W_UX = 0, W_UY = 1, W_UZ = 2, W_T = 3, W_P = 4 };     /* primitive variables */
+
+typedef struct {
+    int ndim, nx, ny, nz, nf;
+    size_t N;
+    double d[3];                 /* dx, dy, dz */
+    double gamma, R, cv, icv, g, mu, K, lam;
+    double Tw[2];                /* T at the bottom (k = 0) and top (k = nz-1) plates */
+    int walls;                   /* 1: no-slip isothermal plates at k = 0, nz-1; 0: periodic in z */
+    int tvd_form, tvd_off, dir_mode;
+    double cfl, fixed_dt;
+} ctx;
+
+/* Coefficients from the paper's dimensionless numbers (DESIGN.md table "Parameters -> coefficients"):
+ * p = R rho T with R = (gamma-1)/(gamma eps D)            Eq. 16
+ * internal energy rho c_v T with c_v = 1/(gamma eps D)    Eq. 17
+ * gravity g = 1/eps                                        Eq. 14
+ * mu = sqrt(Pr/Ra)                                         Eq. 18
+ * K = 1/(eps D sqrt(Ra Pr))                                Eq. 15
+ * Grid (R17): x_i = i lx/nx, y_j = j ly/ny periodic; z_k = k lz/(nz-1) with nodes on the plates
+ * (z_k = k lz/nz when z is periodic). */
+static int ctx_init(ctx *c, const orc_grid *g, const orc_params *p)
+{
+    if (!g || !p) return -1;
+    if (g->ndim != 2 && g->ndim != 3) return -1;
+    if (g->nx < 1 || g->ny < 1 || g->nz < 1) return -1;
+    if (g->ndim == 2 && g->ny != 1) return -1;
+    c->ndim = g->ndim; c->nx = g->nx; c->ny = g->ny; c->nz = g->nz;
+    c->nf = (g->ndim == 2) ? 4 : 5;
+    c->N = (size_t)g->nx * (size_t)g->ny * (size_t)g->nz;
+    c->walls = (p->bc_z == 0);
+    c->d[0] = g->lx / g->nx;
+    c->d[1] = (g->ndim == 3) ? g->ly / g->ny : 1.0;
+    c->d[2] = c->walls ? g->lz / (g->nz - 1) : g->lz / g->nz;
+    c->gamma = p->gamma;
+    c->icv = p->gamma * p->eps * p->D;               /* gamma eps D: T = icv*(E/rho - u^2/2 - z/eps), Eq. 17 */
+    c->cv = 1.0 / c->icv;
+    c->R = (p->gamma - 1.0) / c->icv;
+    c->g = (p->g_override >= 0.0) ? p->g_override : 1.0 / p->eps;
+    c->mu = (p->mu_override >= 0.0) ? p->mu_override : sqrt(p->Pr / p->Ra);
+    c->K = (p->K_override >= 0.0) ? p->K_override : 1.0 / (p->eps * p->D * sqrt(p->Ra * p->Pr));
+    c->lam = p->lambda_coef;
+    c->Tw[0] = p->T_bot; c->Tw[1] = p->T_top;
+    c->tvd_form = p->tvd_form; c->tvd_off = p->tvd_off; c->dir_mode = p->dir_mode;
+    c->cfl = p->cfl; c->fixed_dt = p->fixed_dt;
+    return 0;
+}
+
+static size_t at(const ctx *c, int i, int j, int k)
+{
+    return ((size_t)k * (size_t)c->ny + (size_t)j) * (size_t)c->nx + (size_t)i;
+}
+
+/* Node reached from (i,j,k) by `off` steps along `axis`: periodic wrap in x and y ("periodic
+ * boundary condition for the vertical sideways walls") and in z when z is periodic;
+ * -1 if the step leaves the box through a plate. */
+static long nb(const ctx *c, int i, int j, int k, int axis, int off)
+{
+    if (axis == 0) { i = ((i + off) % c->nx + c->nx) % c->nx; }
+    else if (axis == 1) { j = ((j + off) % c->ny + c->ny) % c->ny; }
+    else {
+        k += off;
+        if (c->walls) { if (k < 0 || k >= c->nz) return -1; }
+        else k = (k % c->nz + c->nz) % c->nz;
+    }
+    return (long)at(c, i, j, k);
+}
+
+static double z_of(const ctx *c, int k) { return (double)k * c->d[2]; }
+
+/* Primitive variables from X (Eqs. 16-17):
+ * u = (rho u)/rho;  T = gamma eps D (E/rho - u^2/2 - z/eps);  p = (gamma-1)/(gamma eps D) rho T. */
+static void primitives(const ctx *c, double *const q[5], double *w[5])
+{
+    for (int k = 0; k < c->nz; ++k)
+        for (int j = 0; j < c->ny; ++j)
+            for (int i = 0; i < c->nx; ++i) {
+                size_t n = at(c, i, j, k);
+                double inv = 1.0 / q[Q_RHO][n];
+                double ux = q[Q_MX][n] * inv, uy = q[Q_MY][n] * inv, uz = q[Q_MZ][n] * inv;
+                double ke = 0.5 * (ux * ux + uy * uy + uz * uz);
+                double T = (q[Q_E][n] * inv - ke - c->g * z_of(c, k)) * c->icv;
+                w[W_UX][n] = ux; w[W_UY][n] = uy; w[W_UZ][n] = uz;
+                w[W_T][n] = T;
+                w[W_P][n] = c->R * q[Q_RHO][n] * T;
+            }
+}
+
+/* Finite difference of a node array along `axis`: mode 0 = 2nd-order central, +1 = forward,
+ * -1 = backward one-sided (first order).  NaN when a needed neighbour lies outside a plate
+ * (such values are never used; a NaN that leaks into a result fails every test). */
+static double deriv(const ctx *c, const double *f, int i, int j, int k, int axis, int mode)
+{
+    long n0 = (long)at(c, i, j, k);
+    long np = nb(c, i, j, k, axis, +1), nm = nb(c, i, j, k, axis, -1);
+    if (mode == 0) { if (np < 0 || nm < 0) return NAN; return (f[np] - f[nm]) / (2.0 * c->d[axis]); }
+    if (mode > 0)  { if (np < 0) return NAN; return (f[np] - f[n0]) / c->d[axis]; }
+    if (nm < 0) return NAN;
+    return (f[n0] - f[nm]) / c->d[axis];
+}
+
+/* Flux F_alpha at one node (Eq. 28, with the pressure in the rho*u_alpha row as
+ * Eq. 14 has it, R2) and the stress tensor of Eq. 18:
+ *   tau_{i alpha} = mu (d_alpha u_i + d_i u_alpha + lambda delta_{i alpha} d_m u_m).
+ * Inner derivatives (R7): along alpha the one-sided difference of sign s (the caller passes the
+ * sign opposite to the stage's outer difference); across alpha the central difference. */
+static void flux_node(const ctx *c, int a, int s, double *const q[5], double *const w[5],
+                      int i, int j, int k, double F[5])
+{
+    double G[3][3];                               /* G[ax][b] = d u_b / d x_ax */
+    for (int ax = 0; ax < 3; ++ax)
+        for (int b = 0; b < 3; ++b)
+            G[ax][b] = deriv(c, w[b], i, j, k, ax, ax == a ? s : 0);
+    double dT = deriv(c, w[W_T], i, j, k, a, s);
+    double div = G[0][0] + G[1][1] + G[2][2];
+    double tau[3];
+    for (int b = 0; b < 3; ++b)
+        tau[b] = c->mu * (G[a][b] + G[b][a] + (b == a ? c->lam * div : 0.0));
+    size_t n = at(c, i, j, k);
+    double ua = w[a][n], p = w[W_P][n];
+    F[Q_RHO] = q[Q_MX + a][n];
+    for (int b = 0; b < 3; ++b)
+        F[Q_MX + b] = q[Q_MX + b][n] * ua + (b == a ? p : 0.0) - tau[b];
+    F[Q_E] = ua * (q[Q_E][n] + p) - c->K * dT
+             - (w[W_UX][n] * tau[0] + w[W_UY][n] * tau[1] + w[W_UZ][n] * tau[2]);
+}
+
+static int is_wall_row(const ctx *c, int k) { return c->walls && (k == 0 || k == c->nz - 1); }
+
+/* Flux at every node where the sweep uses it.  x- and y-sweeps leave plate rows untouched (R10),
+ * so no flux is formed there.  In a z-sweep a plate node whose one-sided neighbour is missing
+ * keeps only its mass flux rho*u_z (all the wall closure needs); the other rows are NaN. */
+static void flux_field(const ctx *c, int a, int s, double *const q[5], double *const w[5], double *F[5])
+{
+    for (int k = 0; k < c->nz; ++k)
+        for (int j = 0; j < c->ny; ++j)
+            for (int i = 0; i < c->nx; ++i) {
+                size_t n = at(c, i, j, k);
+                double Fn[5];
+                if (a != 2 && is_wall_row(c, k)) {
+                    for (int f = 0; f < 5; ++f) Fn[f] = NAN;
+                } else {
+                    flux_node(c, a, s, q, w, i, j, k, Fn);
+                    if (a == 2 && c->walls && nb(c, i, j, k, 2, s) < 0) {
+                        Fn[Q_RHO] = q[Q_MZ][n];
+                        for (int f = 1; f < 5; ++f) Fn[f] = NAN;
+                    }
+                }
+                for (int f = 0; f < 5; ++f) F[f][n] = Fn[f];
+            }
+}
+
+/* Plate node (i,j,kw) in a z-sweep: no-slip (rho u = 0) and isothermal (T = T_w) conditions
+ * fix every unknown except rho, which follows the conservative
+ * half-cell closure (R10): the plate node owns a cell of height dz/2 whose outer face carries the
+ * plate's own mass flux.  `o` is the stage's outer difference (-1 backward, +1 forward). */
+static void wall_node(const ctx *c, double *const X[5], double *const Fl[5], double *Xs[5],
+                      int i, int j, int kw, int o, double tau)
+{
+    size_t n = at(c, i, j, kw);
+    double rho = X[Q_RHO][n];
+    if (kw == 0 && o > 0) {
+        size_t n1 = at(c, i, j, 1);
+        rho = rho - (2.0 * tau / c->d[2]) * (Fl[Q_RHO][n1] - Fl[Q_RHO][n]);
+    } else if (kw == c->nz - 1 && o < 0) {
+        size_t n1 = at(c, i, j, c->nz - 2);
+        rho = rho - (2.0 * tau / c->d[2]) * (Fl[Q_RHO][n] - Fl[Q_RHO][n1]);
+    }
+    double Tw = c->Tw[kw == 0 ? 0 : 1];
+    Xs[Q_RHO][n] = rho;
+    Xs[Q_MX][n] = 0.0; Xs[Q_MY][n] = 0.0; Xs[Q_MZ][n] = 0.0;
+    Xs[Q_E][n] = rho * (c->cv * Tw + c->g * z_of(c, kw));     /* Eq. 17 with u = 0, T = T_w */
+}
+
+/* One MacCormack stage (Eq. 31 when o = -1, Eq. 32 when o = +1; R1: the
+ * corrector differences the flux of the predicted state at both nodes):
+ *   Xs_k = X_k - (tau/dx_alpha)(Fl_k - Fl_{k-1}) + tau S_k        (o = -1, backward)
+ *   Xs_k = X_k - (tau/dx_alpha)(Fl_{k+1} - Fl_k) + tau S_k        (o = +1, forward)
+ * S = (0,0,0,-g rho,0) in the z-sweep only (f_3 = -rho g), evaluated on `Ssrc`. */
+static void stage(const ctx *c, int a, int o, double tau, double *const X[5], double *const Fl[5],
+                  double *const Ssrc[5], double *Xs[5])
+{
+    double cdt = tau / c->d[a];
+    for (int k = 0; k < c->nz; ++k)
+        for (int j = 0; j < c->ny; ++j)
+            for (int i = 0; i < c->nx; ++i) {
+                size_t n = at(c, i, j, k);
+                if (is_wall_row(c, k)) {
+                    if (a == 2) wall_node(c, X, Fl, Xs, i, j, k, o, tau);
+                    else for (int f = 0; f < 5; ++f) Xs[f][n] = X[f][n];
+                    continue;
+                }
+                long hi = (o > 0) ? nb(c, i, j, k, a, +1) : (long)n;
+                long lo = (o > 0) ? (long)n : nb(c, i, j, k, a, -1);
+                for (int f = 0; f < 5; ++f)
+                    Xs[f][n] = X[f][n] - cdt * (Fl[f][hi] - Fl[f][lo]);
+                if (a == 2) Xs[Q_MZ][n] = Xs[Q_MZ][n] + tau * (-c->g * Ssrc[Q_RHO][n]);
+            }
+}
+
+static double phi_minmod(double x) { return fmax(0.0, fmin(2.0 * x, 1.0)); }
+
+/* TVD term (Eqs. 34-39), all from the sweep input X, along alpha:
+ *   dX_{k+1/2} = X_{k+1} - X_k                                        Eqs. 35-36
+ *   r+_k = (dX_{k-1/2}, dX_{k+1/2}) / (dX_{k+1/2}, dX_{k+1/2}),
+ *   r-_k = (dX_{k-1/2}, dX_{k+1/2}) / (dX_{k-1/2}, dX_{k-1/2})        Eq. 37 (dot product over the fields)
+ *   G(x) = 0.5 C (1 - phi(x)), phi(x) = max(0, min(2x, 1))            Eq. 38
+ *   C = Co(1-Co) if Co <= 0.5 else 0.25                               Eq. 39
+ *   T_k = Dh_{k+1/2} - Dh_{k-1/2}                                     Eq. 34
+ * with Dh_{k+1/2} = G(r+_k + r-_{k+1}) dX_{k+1/2} (tvd_form 0, as printed; C = mean of the two
+ * nodes' C, R6) or [G_k(r+_k) + G_{k+1}(r-_{k+1})] dX_{k+1/2} (tvd_form 1, Davis/Yee, R4).
+ * Co_k = (|u_alpha| + c_s)_k tau/dx_alpha (R5); r := 1 when its denominator is 0 (R15);
+ * Dh := 0 on the two plate-adjacent interfaces of a z-sweep (R11).  Dh_{k+1/2} is stored at node k. */
+static void tvd_interface_flux(const ctx *c, int a, double tau, double *const X[5], double *const w[5],
+                               double *Dh[5])
+{
+    double *Cn = (double *)malloc(c->N * sizeof(double));
+    for (int k = 0; k < c->nz; ++k)
+        for (int j = 0; j < c->ny; ++j)
+            for (int i = 0; i < c->nx; ++i) {
+                size_t n = at(c, i, j, k);
+                double cs = sqrt(c->gamma * c->R * w[W_T][n]);
+                double Co = (fabs(w[a][n]) + cs) * tau / c->d[a];
+                Cn[n] = (Co <= 0.5) ? Co * (1.0 - Co) : 0.25;
+            }
+    for (int k = 0; k < c->nz; ++k)
+        for (int j = 0; j < c->ny; ++j)
+            for (int i = 0; i < c->nx; ++i) {
+                size_t n = at(c, i, j, k);
+                long nm = nb(c, i, j, k, a, -1), np = nb(c, i, j, k, a, +1), npp = nb(c, i, j, k, a, +2);
+                int zero = (a != 2 && is_wall_row(c, k)) || nm < 0 || np < 0 || npp < 0;
+                if (zero) { for (int f = 0; f < 5; ++f) Dh[f][n] = 0.0; continue; }
+                double dm[5], d0[5], dp[5], b0 = 0.0, ak = 0.0, akp = 0.0;
+                for (int f = 0; f < 5; ++f) {
+                    dm[f] = X[f][n] - X[f][nm];
+                    d0[f] = X[f][np] - X[f][n];
+                    dp[f] = X[f][npp] - X[f][np];
+                }
+                for (int f = 0; f < 5; ++f) { b0 += d0[f] * d0[f]; ak += dm[f] * d0[f]; akp += d0[f] * dp[f]; }
+                double rplus_k = (b0 == 0.0) ? 1.0 : ak / b0;      /* r+ at node k   */
+                double rminus_kp = (b0 == 0.0) ? 1.0 : akp / b0;   /* r- at node k+1 */
+                double coef;
+                if (c->tvd_form == 0)
+                    coef = 0.5 * (0.5 * (Cn[n] + Cn[np])) * (1.0 - phi_minmod(rplus_k + rminus_kp));
+                else
+                    coef = 0.5 * Cn[n] * (1.0 - phi_minmod(rplus_k))
+                         + 0.5 * Cn[np] * (1.0 - phi_minmod(rminus_kp));
+                for (int f = 0; f < 5; ++f) Dh[f][n] = coef * d0[f];
+            }
+    free(Cn);
+}
+
+static double *arr(size_t n) { return (double *)calloc(n, sizeof(double)); }
+
+/* L_alpha(tau) on five internal fields: predictor, boundary values, corrector, TVD term, average
+ * (Eqs. 31-39 in the order of PAPER.md:273-309; dir = -1 swaps the two one-sided differences, R9). */
+static void sweep5(const ctx *c, int a, double tau, int dir, double *const X[5], double *Xo[5])
+{
+    double *w[5], *F[5], *XP[5], *XC[5], *Dh[5];
+    for (int f = 0; f < 5; ++f) {
+        w[f] = arr(c->N); F[f] = arr(c->N); XP[f] = arr(c->N); XC[f] = arr(c->N); Dh[f] = arr(c->N);
+    }
+    /* predictor, Eq. 31: outer difference backward (dir=+1), inner derivatives forward */
+    primitives(c, X, w);
+    flux_field(c, a, +dir, X, w, F);
+    stage(c, a, -dir, tau, X, F, X, XP);
+    /* TVD term from X^n while its primitives are at hand */
+    if (!c->tvd_off) tvd_interface_flux(c, a, tau, X, w, Dh);
+    /* corrector, Eq. 32: flux and source of the predicted state, opposite differences */
+    primitives(c, XP, w);
+    flux_field(c, a, -dir, XP, w, F);
+    stage(c, a, +dir, tau, X, F, XP, XC);
+    /* Eq. 33: X = (X^P + X^C)/2 + T, then the plate values again */
+    for (int k = 0; k < c->nz; ++k)
+        for (int j = 0; j < c->ny; ++j)
+            for (int i = 0; i < c->nx; ++i) {
+                size_t n = at(c, i, j, k);
+                if (is_wall_row(c, k)) {
+                    if (a != 2) { for (int f = 0; f < 5; ++f) Xo[f][n] = X[f][n]; continue; }
+                    double rho = 0.5 * (XP[Q_RHO][n] + XC[Q_RHO][n]);
+                    double Tw = c->Tw[k == 0 ? 0 : 1];
+                    Xo[Q_RHO][n] = rho;
+                    Xo[Q_MX][n] = 0.0; Xo[Q_MY][n] = 0.0; Xo[Q_MZ][n] = 0.0;
+                    Xo[Q_E][n] = rho * (c->cv * Tw + c->g * z_of(c, k));
+                    continue;
+                }
+                long nm = nb(c, i, j, k, a, -1);
+                for (int f = 0; f < 5; ++f) {
+                    double T = Dh[f][n] - Dh[f][nm];               /* Eq. 34 */
+                    Xo[f][n] = 0.5 * (XP[f][n] + XC[f][n]) + T;    /* Eq. 33 */
+                }
+            }
+    for (int f = 0; f < 5; ++f) { free(w[f]); free(F[f]); free(XP[f]); free(XC[f]); free(Dh[f]); }
+}
+
+/* Map the caller's nf-field SoA block onto five internal field pointers (2-D: rho u_y = zeros). */
+static void map_fields(const ctx *c, double *X, double *zeros, double *q[5])
+{
+    if (c->ndim == 3) { for (int f = 0; f < 5; ++f) q[f] = X + (size_t)f * c->N; }
+    else { q[Q_RHO] = X; q[Q_MX] = X + c->N; q[Q_MY] = zeros; q[Q_MZ] = X + 2 * c->N; q[Q_E] = X + 3 * c->N; }
+}
+
+int orc_sweep(const orc_grid *g, const orc_params *p, const double *X_in, double *X_out,
+              int alpha, double tau, int dir)
+{
+    ctx c;
+    if (ctx_init(&c, g, p) || alpha < 0 || alpha > 2 || (dir != 1 && dir != -1)) return -1;
+    if (c.ndim == 2 && alpha == 1) return -1;
+    if (c.walls && c.nz < 5) return -1;
+    double *zin = arr(c.N), *zout = arr(c.N), *qi[5], *qo[5];
+    map_fields(&c, (double *)X_in, zin, qi);
+    map_fields(&c, X_out, zout, qo);
+    sweep5(&c, alpha, tau, dir, qi, qo);
+    free(zin); free(zout);
+    return 0;
+}
+
+/* R12: s = max over nodes and directions of (|u_alpha| + c_s)/dx_alpha, c_s = sqrt(gamma R T). */
+double orc_max_speed(const orc_grid *g, const orc_params *p, const double *X)
+{
+    ctx c;
+    if (ctx_init(&c, g, p)) return NAN;
+    double *zeros = arr(c.N), *q[5];
+    map_fields(&c, (double *)X, zeros, q);
+    double s = 0.0;
+    int bad = 0;
+    for (int k = 0; k < c.nz; ++k)
+        for (int j = 0; j < c.ny; ++j)
+            for (int i = 0; i < c.nx; ++i) {
+                size_t n = at(&c, i, j, k);
+                double rho = q[Q_RHO][n];
+                double inv = 1.0 / rho;
+                double u[3] = { q[Q_MX][n] * inv, q[Q_MY][n] * inv, q[Q_MZ][n] * inv };
+                double ke = 0.5 * (u[0] * u[0] + u[1] * u[1] + u[2] * u[2]);
+                double T = (q[Q_E][n] * inv - ke - c.g * z_of(&c, k)) * c.icv;
+                if (!(rho > 0.0) || !(T > 0.0) || !isfinite(rho) || !isfinite(T)) { bad = 1; continue; }
+                double cs = sqrt(c.gamma * c.R * T);
+                for (int a = 0; a < 3; ++a) {
+                    if (c.ndim == 2 && a == 1) continue;
+                    double v = (fabs(u[a]) + cs) / c.d[a];
+                    if (!isfinite(v)) bad = 1;
+                    if (v > s) s = v;
+                }
+            }
+    free(zeros);
+    return bad ? NAN : s;
+}
+
+double orc_dt(const orc_grid *g, const orc_params *p, const double *X)
+{
+    if (p->fixed_dt > 0.0) return p->fixed_dt;
+    return p->cfl / orc_max_speed(g, p, X);
+}
+
+/* Eq. 30: X^(n+1) = Lx Ly Lz Lx Ly Lz X^(n), each with dt/2, operators acting
+ * right to left; the y operator is absent in 2-D.  dir_mode 1 (R9): dir = +1 in the first triple,
+ * -1 in the second. */
+int orc_step(const orc_grid *g, const orc_params *p, double *X, int n_steps,
+             const double *dt_in, double *dt_out, double *time)
+{
+    ctx c;
+    if (ctx_init(&c, g, p) || n_steps < 0) return -1;
+    if (c.walls && c.nz < 5) return -1;
+    double *za = arr(c.N), *zb = arr(c.N), *Y = arr((size_t)c.nf * c.N), *qa[5], *qb[5];
+    map_fields(&c, X, za, qa);
+    map_fields(&c, Y, zb, qb);
+    for (int s = 0; s < n_steps; ++s) {
+        double dt = dt_in ? dt_in[s] : orc_dt(g, p, X);
+        if (!(dt > 0.0) || !isfinite(dt)) { free(za); free(zb); free(Y); return -4; }
+        double tau = 0.5 * dt;
+        double **src = qa, **dst = qb;
+        for (int half = 0; half < 2; ++half) {
+            int dir = (half == 1 && c.dir_mode == 1) ? -1 : +1;
+            for (int a = 2; a >= 0; --a) {            /* L_z, then L_y, then L_x */
+                if (c.ndim == 2 && a == 1) continue;
+                sweep5(&c, a, tau, dir, src, dst);
+                double **t = src; src = dst; dst = t;
+            }
+        }
+        /* 4 (2-D) or 6 (3-D) sweeps: an even count, so the result is back in X */
+        if (dt_out) dt_out[s] = dt;
+        if (time) *time += dt;
+    }
+    free(za); free(zb); free(Y);
+    return 0;
+}
+
+/* Diagnostics, instantaneous (the paper also averages in time):
+ *   <f>_A(k): plane mean; <f>_V: trapezoid in z (R16);  T_A = 1 - D z (Eq. 19); T_sa = T - T_A
+ *   Nu_conv = sqrt(Ra Pr)/eps <rho u_z T_sa>_V,  Nu_K = D sqrt(Ra Pr)/2 <rho u_z u^2>_V,
+ *   Nu_bulk = 1 + Nu_conv + Nu_K                                       Eq. 22
+ *   Nu_{z=0,1} = -(1/eps) d<T_sa>_A/dz with 2nd-order one-sided differences at the plates
+ *                                                                      Eq. 23
+ *   Nu_bar = (Nu_0 + Nu_1)/2                                           Eq. 24
+ *   Re = sqrt(Ra/Pr) sqrt(<u^2>_V)                                     Eq. 26
+ * Sums: serial along each row, rows into planes, planes into the trapezoid rule. */
+int orc_diagnostics(const orc_grid *g, const orc_params *p, const double *X, orc_diag *out,
+                    double *T_prof, double *rho_prof, double *p_prof)
+{
+    ctx c;
+    if (ctx_init(&c, g, p) || !out) return -1;
+    double *zeros = arr(c.N), *q[5];
+    map_fields(&c, (double *)X, zeros, q);
+    memset(out, 0, sizeof(*out));
+    int nz = c.nz;
+    double *sT = arr(nz), *sTsa = arr(nz);
+    double vol_w = 0.0, v_conv = 0.0, v_K = 0.0, v_u2 = 0.0;
+    double tot[5] = { 0, 0, 0, 0, 0 };
+    double max_mach = 0.0, min_rho = INFINITY, min_T = INFINITY;
+    double nplane = (double)c.nx * (double)c.ny;
+    for (int k = 0; k < nz; ++k) {
+        double z = z_of(&c, k), TA = 1.0 - p->D * z;
+        double pT = 0, prho = 0, pp = 0, pconv = 0, pK = 0, pu2 = 0, pq[5] = { 0, 0, 0, 0, 0 };
+        for (int j = 0; j < c.ny; ++j) {
+            double rT = 0, rrho = 0, rp = 0, rconv = 0, rK = 0, ru2 = 0, rq[5] = { 0, 0, 0, 0, 0 };
+            for (int i = 0; i < c.nx; ++i) {
+                size_t n = at(&c, i, j, k);
+                double rho = q[Q_RHO][n], inv = 1.0 / rho;
+                double ux = q[Q_MX][n] * inv, uy = q[Q_MY][n] * inv, uz = q[Q_MZ][n] * inv;
+                double u2 = ux * ux + uy * uy + uz * uz;
+                double T = (q[Q_E][n] * inv - 0.5 * u2 - c.g * z) * c.icv;
+                double pr = c.R * rho * T;
+                rT += T; rrho += rho; rp += pr;
+                rconv += rho * uz * (T - TA);
+                rK += rho * uz * u2;
+                ru2 += u2;
+                for (int f = 0; f < 5; ++f) rq[f] += q[f][n];
+                double mach = sqrt(u2) / sqrt(c.gamma * c.R * T);
+                if (mach > max_mach) max_mach = mach;
+                if (rho < min_rho) min_rho = rho;
+                if (T < min_T) min_T = T;
+            }
+            pT += rT; prho += rrho; pp += rp; pconv += rconv; pK += rK; pu2 += ru2;
+            for (int f = 0; f < 5; ++f) pq[f] += rq[f];
+        }
+        double wk = c.d[2] * ((c.walls && (k == 0 || k == nz - 1)) ? 0.5 : 1.0);
+        sT[k] = pT / nplane;
+        sTsa[k] = sT[k] - TA;
+        if (T_prof) T_prof[k] = sT[k];
+        if (rho_prof) rho_prof[k] = prho / nplane;
+        if (p_prof) p_prof[k] = pp / nplane;
+        vol_w += wk;
+        v_conv += wk * (pconv / nplane);
+        v_K += wk * (pK / nplane);
+        v_u2 += wk * (pu2 / nplane);
+        for (int f = 0; f < 5; ++f) tot[f] += wk * c.d[0] * c.d[1] * pq[f];
+    }
+    double sRaPr = sqrt(p->Ra * p->Pr);
+    out->nu_conv = sRaPr / p->eps * (v_conv / vol_w);
+    out->nu_K = p->D * sRaPr / 2.0 * (v_K / vol_w);
+    out->nu_bulk = 1.0 + out->nu_conv + out->nu_K;
+    out->u_rms = sqrt(v_u2 / vol_w);
+    out->re = sqrt(p->Ra / p->Pr) * out->u_rms;
+    if (nz >= 3) {
+        double dz = c.d[2];
+        double g0 = (-3.0 * sTsa[0] + 4.0 * sTsa[1] - sTsa[2]) / (2.0 * dz);
+        double g1 = (3.0 * sTsa[nz - 1] - 4.0 * sTsa[nz - 2] + sTsa[nz - 3]) / (2.0 * dz);
+        out->nu_bottom = -g0 / p->eps;
+        out->nu_top = -g1 / p->eps;
+        out->nu_bar = 0.5 * (out->nu_bottom + out->nu_top);
+    }
+    out->mass = tot[Q_RHO]; out->mom_x = tot[Q_MX]; out->mom_y = tot[Q_MY]; out->mom_z = tot[Q_MZ];
+    out->energy = tot[Q_E];
+    out->max_mach = max_mach; out->min_rho = min_rho; out->min_T = min_T;
+    out->dt = orc_dt(g, p, X);
+    free(sT); free(sTsa); free(zeros);
+    return 0;
+}
+
+int orc_coefficients(const orc_grid *g, const orc_params *p, double *o)
+{
+    ctx c;
+    if (ctx_init(&c, g, p) || !o) return -1;
+    o[0] = c.R; o[1] = c.cv; o[2] = c.g; o[3] = c.mu; o[4] = c.K; o[5] = c.lam;
+    o[6] = c.d[0]; o[7] = c.d[1]; o[8] = c.d[2];
+    return 0;
+}

@@ -1,0 +1,488 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix (no GPU needed).
+
+BASELINE.json's five checks (uniform state, conservation, Sod tube vs the exact Riemann solution,
+second-order convergence, mirror symmetry) plus closed forms that pin every term of Eq. 28:
+viscous shear decay (inner and cross derivative halves of tau_ij), acoustic attenuation (the
+dilatation coefficient), thermal diffusion (K), viscous heating pattern (the u_j tau_ij work term),
+hydrostatic balance (gravity source and the potential energy inside E), and axis-permutation
+identities that carry each pin from one sweep direction to the other two.
+"""
+import numpy as np
+import pytest
+
+from paper_2411_10372_b200 import inputs
+from tests.helpers import (advance_to, ideal_gas_params, primitives_of, rel_err, riemann_exact,
+                           state_from_primitives)
+
+
+def periodic_grid(ndim, nx, nz, ny=1, lx=1.0, ly=1.0, lz=1.0):
+    return inputs.make_grid(ndim, nx, nz, ny, lx=lx, ly=ly, lz=lz)
+
+
+# ----------------------------------------------------------------------------- coefficients
+def test_coefficients_from_paper_numbers(orc):
+    """tests/golden/coefficients.txt: values that Eqs. 14-18 and PAPER.md:204 give for the configs."""
+    import os
+    gold = {}
+    with open(os.path.join(os.path.dirname(__file__), "golden", "coefficients.txt")) as fh:
+        for line in fh:
+            if line.strip() and not line.startswith("#"):
+                k, v = line.split()[:2]
+                gold[k] = float(v)
+    g, p, _ = inputs.config("C1")
+    c = orc.coefficients(orc.Problem(g, p))
+    for k in ("R", "cv", "g", "mu", "K"):
+        assert c[k] == pytest.approx(gold[k], rel=1e-14), k
+    assert p["T_top"] == pytest.approx(gold["T_top"], rel=1e-15)
+    assert c["dx"] == 4.0 / 256 and c["dz"] == 1.0 / 63
+
+
+# ----------------------------------------------------------------------------- check 1: uniform
+@pytest.mark.parametrize("ndim", [2, 3])
+def test_uniform_state_stays_uniform_bitwise(orc, ndim):
+    """Every flux difference and dX of a uniform state is exactly 0 (BASELINE check 1)."""
+    g = periodic_grid(ndim, 12, 10, 6 if ndim == 3 else 1)
+    p = ideal_gas_params(mu_override=0.01, K_override=0.02)
+    X = state_from_primitives(g, p, 1.3, 0.4, -0.2 if ndim == 3 else 0.0, 0.3, 2.0)
+    Y, dts, _ = orc.step(orc.Problem(g, p), X, 20)
+    assert np.array_equal(X, Y)
+    # plates: u = 0, both plates at the gas temperature, no gravity
+    p = ideal_gas_params(bc_z=0, mu_override=0.01, K_override=0.02)
+    X = state_from_primitives(g, p, 1.3, 0.0, 0.0, 0.0, 1.3 * (p["gamma"] - 1.0))   # T = 1 = T_w
+    Y, _, _ = orc.step(orc.Problem(g, p), X, 20)
+    assert np.array_equal(X, Y)
+
+
+# ----------------------------------------------------------------------------- check 2: conservation
+@pytest.mark.parametrize("ndim,tvd_form", [(2, 0), (2, 1), (3, 1)])
+def test_conservation_periodic(orc, ndim, tvd_form):
+    """All-periodic box, g = 0, viscous and conducting: sums of rho, rho*u, E stay constant to
+    round-off because flux differences and the TVD term telescope (BASELINE check 2a)."""
+    g = periodic_grid(ndim, 24, 20, 16 if ndim == 3 else 1)
+    p = ideal_gas_params(mu_override=5e-3, K_override=7e-3, tvd_form=tvd_form)
+    X = inputs.smooth_random_state(g, p, seed=7)
+    Y, _, _ = orc.step(orc.Problem(g, p), X, 10)
+    s0, s1 = X.sum(axis=1), Y.sum(axis=1)
+    scale = np.abs(X).sum(axis=1)
+    assert np.all(np.abs(s1 - s0) <= 2e-14 * scale), (s1 - s0) / scale
+    assert not np.array_equal(X, Y)
+
+
+def test_mass_conserved_between_plates(orc):
+    """Config C1 (plates): trapezoid mass constant to round-off under the conservative half-cell
+    closure; horizontal momentum is reported only (the plates exert drag) (BASELINE check 2b)."""
+    g, p, _ = inputs.config("C1")
+    X = inputs.conduction_state(g, p)
+    prob = orc.Problem(g, p)
+    d0 = orc.diagnostics(prob, X)[0]
+    Y, _, _ = orc.step(prob, X, 25)
+    d1 = orc.diagnostics(prob, Y)[0]
+    assert abs(d1["mass"] - d0["mass"]) <= 1e-14 * d0["mass"]
+    assert d0["mass"] == pytest.approx(3.0, rel=1e-12)     # 4 * integral of the linear rho = 4*(1+0.5)/2
+    assert abs(d1["mom_x"]) < 1e-6
+
+
+# ----------------------------------------------------------------------------- check 3: Sod
+def _sod(orc, n, axis, tvd_form, ndim=2, t_end=0.2):
+    """Classical two-state tube (8:1 density, 10:1 pressure, at rest, gamma 1.4), doubled so the
+    periodic box holds two mirrored tubes; returns (x, rho(x), u(x), p(x)) along `axis`."""
+    gam = 1.4
+    x = np.arange(n) * 2.0 / n
+    left = (x >= 0.5) & (x < 1.5)
+    rho1, p1 = np.where(left, 1.0, 0.125), np.where(left, 1.0, 0.1)
+    m = 4
+    if axis == 0:
+        g = periodic_grid(ndim, n, m, m if ndim == 3 else 1, lx=2.0, ly=m * 2.0 / n, lz=m * 2.0 / n)
+        shape = (1, 1, n)
+    elif axis == 2:
+        g = periodic_grid(ndim, m, n, m if ndim == 3 else 1, lx=m * 2.0 / n, ly=m * 2.0 / n, lz=2.0)
+        shape = (n, 1, 1)
+    else:
+        g = periodic_grid(3, m, m, n, lx=m * 2.0 / n, ly=2.0, lz=m * 2.0 / n)
+        shape = (1, n, 1)
+    p = ideal_gas_params(gamma=gam, tvd_form=tvd_form)
+    X = state_from_primitives(g, p, rho1.reshape(shape), 0.0, 0.0, 0.0, p1.reshape(shape))
+    X, _ = advance_to(orc, orc.Problem(g, p), X, t_end)
+    prim = primitives_of(g, p, X)
+    line = {0: np.s_[1, 0, :], 1: np.s_[1, :, 1], 2: np.s_[:, 0, 1]}[axis]
+    return x, prim[0][line], prim[1 + axis][line], prim[5][line]
+
+
+def test_sod_star_state_golden():
+    """The test's own Riemann solver reproduces the star values quoted in tests/golden/sod.txt."""
+    _, _, _, ps, us = riemann_exact(1.0, 0.0, 1.0, 0.125, 0.0, 0.1, 1.4, np.array([0.0]))
+    assert ps == pytest.approx(0.30313, abs(1e-5)) and us == pytest.approx(0.92745, abs=1e-5)
+
+
+@pytest.mark.parametrize("axis,ndim", [(0, 2), (2, 2), (1, 3)])
+def test_sod_tube_vs_exact_riemann(orc, axis, ndim):
+    """L1(rho) error falls about first order with N and the solution stays oscillation-free
+    (BASELINE check 3) along every sweep direction."""
+    errs = []
+    for n in (100, 200, 400) if axis == 0 else (100, 200):
+        x, rho, u, pr = _sod(orc, n, axis, tvd_form=1, ndim=ndim)
+        sel = x >= 1.0
+        re, ue, pe, _, _ = riemann_exact(1.0, 0.0, 1.0, 0.125, 0.0, 0.1, 1.4, (x[sel] - 1.5) / 0.2)
+        errs.append(np.abs(rho[sel] - re).mean())
+        tv = np.abs(np.diff(np.r_[rho, rho[0]])).sum()
+        assert rho.max() <= 1.0 * (1 + 1e-3) and rho.min() >= 0.125 * (1 - 1e-3)
+        assert tv <= 1.01 * (2 * 0.875)
+        # mirrored tube: the initial data are symmetric under i -> n-1-i, the solution nearly so
+        assert np.abs(rho - rho[::-1]).mean() < 2e-3
+        assert np.abs(u[sel] - ue).mean() < 4 * errs[-1] + 1e-3 and np.abs(pr[sel] - pe).mean() < 2 * errs[-1]
+    for a, b in zip(errs, errs[1:]):
+        assert 1.6 < a / b < 2.6, errs
+    assert errs[0] < 0.02
+
+
+def test_tvd_form_decision(orc):
+    """DESIGN.md R4: Eq. 34 as printed (G of the sum r+ + r-) lets the total variation of the Sod
+    density grow by ~75 %, the Davis/Yee form (sum of two G's) keeps it non-increasing; this is why
+    tvd_form = 1 is the default."""
+    tv0 = 2 * 0.875
+    _, rho0, _, _ = _sod(orc, 200, 0, tvd_form=0)
+    _, rho1, _, _ = _sod(orc, 200, 0, tvd_form=1)
+    tv = lambda r: np.abs(np.diff(np.r_[r, r[0]])).sum()
+    assert tv(rho1) <= 1.001 * tv0
+    assert tv(rho0) > 1.3 * tv0
+    assert inputs.make_params()["tvd_form"] == 1
+
+
+# ----------------------------------------------------------------------------- check 4: convergence
+def _density_wave_error(orc, n, ndim, oblique, tvd_off, t_end=0.4, corrector_literal=False):
+    gam = 1.4
+    ny = n if (ndim == 3) else 1
+    nz = n if oblique else 4
+    g = periodic_grid(ndim, n, nz, ny, lx=1.0, ly=1.0, lz=1.0 if oblique else 4.0 / n)
+    p = ideal_gas_params(gamma=gam, tvd_off=tvd_off, cfl=0.4)
+    x = (np.arange(n) / n)[None, None, :]
+    y = (np.arange(ny) / ny)[None, :, None]
+    z = (np.arange(nz) / nz)[:, None, None]
+    u = (1.0, 0.5 if ndim == 3 else 0.0, 0.75 if oblique else 0.0)
+    kz, ky = (1 if oblique else 0), (1 if ndim == 3 else 0)
+    phase = lambda t: 2 * np.pi * ((x - u[0] * t) + ky * (y - u[1] * t) + kz * (z - u[2] * t))
+    rho0 = 1.0 + 0.2 * np.sin(phase(0.0))
+    X = state_from_primitives(g, p, rho0, u[0], u[1], u[2], 1.0)
+    X, _ = advance_to(orc, orc.Problem(g, p), X, t_end)
+    rho = X[0].reshape(nz, ny, n)
+    exact = 1.0 + 0.2 * np.sin(phase(t_end)) + 0 * rho
+    return np.abs(rho - exact).mean()
+
+
+@pytest.mark.parametrize("ndim,oblique", [(2, False), (2, True), (3, True)])
+def test_second_order_convergence_density_wave(orc, ndim, oblique):
+    """Smooth advected density wave, dt ~ dx: L1 error ratio per doubling ~4 without the TVD term
+    and >= 3.6 with it (the limiter clips extrema) (BASELINE check 4).  The oblique
+    cases exercise the operator splitting of Eq. 30."""
+    sizes = (16, 32) if ndim == 3 else (32, 64)
+    e_off = [_density_wave_error(orc, n, ndim, oblique, tvd_off=1) for n in sizes]
+    assert 3.7 < e_off[0] / e_off[1] < 4.4, e_off
+    if ndim == 2:
+        sizes = (64, 128)
+        e_on = [_density_wave_error(orc, n, ndim, oblique, tvd_off=0) for n in sizes]
+        assert e_on[0] / e_on[1] > 3.0, e_on
+        assert e_on[1] < 2e-3
+
+
+# ----------------------------------------------------------------------------- check 5: mirror
+def _mirror(X, grid, axis):
+    nf = X.shape[0]
+    F = X.reshape(nf, grid["nz"], grid["ny"], grid["nx"]).copy()
+    ax = {0: 3, 1: 2, 2: 1}[axis]
+    F = np.roll(np.flip(F, axis=ax), 1, axis=ax)          # i -> (n - i) mod n
+    mom = {0: 1, 1: 2, 2: nf - 2}[axis]
+    F[mom] = -F[mom]
+    return F.reshape(nf, -1)
+
+
+@pytest.mark.parametrize("ndim", [2, 3])
+def test_mirror_identity(orc, ndim):
+    """mirror(L_alpha^{dir}(X)) == L_alpha^{-dir}(mirror X) and, across the sweep,
+    mirror_beta(L_alpha^{dir}(X)) == L_alpha^{dir}(mirror_beta X): the forward/backward pair is the
+    exact mirror image of the backward/forward pair (BASELINE check 5a, R9)."""
+    g = periodic_grid(ndim, 16, 12, 10 if ndim == 3 else 1)
+    p = ideal_gas_params(mu_override=4e-3, K_override=6e-3)
+    X = inputs.smooth_random_state(g, p, seed=11)
+    prob = orc.Problem(g, p)
+    axes = (0, 2) if ndim == 2 else (0, 1, 2)
+    for a in axes:
+        for m in axes:
+            for d in (+1, -1):
+                lhs = _mirror(orc.sweep(prob, X, a, 0.01, d), g, m)
+                rhs = orc.sweep(prob, _mirror(X, g, m), a, 0.01, -d if m == a else d)
+                assert np.max(rel_err(lhs, rhs)) < 5e-16, (a, m, d)
+
+
+def test_symmetric_state_asymmetry_shrinks(orc):
+    """A left-right symmetric state stays symmetric up to truncation error, which falls at second
+    order (BASELINE check 5b)."""
+    asym = []
+    for n in (32, 64):
+        g = periodic_grid(2, n, n)
+        p = ideal_gas_params(tvd_off=1, cfl=0.4)
+        x = (np.arange(n) / n)[None, None, :]
+        z = (np.arange(n) / n)[:, None, None]
+        rho = 1.0 + 0.2 * np.cos(2 * np.pi * x) * (1 + 0.5 * np.sin(2 * np.pi * z))
+        ux = 0.3 * np.sin(2 * np.pi * x)
+        uz = 0.2 * np.cos(2 * np.pi * x) * np.sin(2 * np.pi * z)
+        X = state_from_primitives(g, p, rho, ux, 0.0, uz, 1.0 + 0 * rho)
+        assert np.allclose(_mirror(X, g, 0), X, rtol=0, atol=1e-15)
+        X = 0.5 * (X + _mirror(X, g, 0))                       # exactly symmetric
+        Y, _ = advance_to(orc, orc.Problem(g, inputs.make_params(**{**p, "dir_mode": 0})), X, 0.1)
+        asym.append(np.abs(_mirror(Y, g, 0) - Y)[0].max())
+    assert asym[0] / asym[1] > 3.0 and asym[1] < 1e-3, asym
+
+
+# ----------------------------------------------------------------------------- viscous terms
+def _shear_decay(orc, n, plane, tvd_off=1, drop=None, t_end=0.4, nu=0.01):
+    """Oblique, divergence-free shear wave u = A t sin(k.x) (t perpendicular to k) in a uniform
+    low-Mach gas: the amplitude decays as exp(-nu |k|^2 t) exactly when tau_ij carries both
+    d_j u_i and d_i u_j.  `plane` picks the two axes spanning k."""
+    a1, a2 = plane
+    ndim = 2 if 1 not in plane else 3
+    dims = {0: n, 1: n, 2: n}
+    for a in (0, 1, 2):
+        if a not in plane:
+            dims[a] = 4 if ndim == 3 else 1
+    if ndim == 2:
+        dims[1] = 1
+    g = periodic_grid(ndim, dims[0], dims[2], dims[1], lx=1.0 if 0 in plane else 4.0 / n,
+                      ly=1.0 if 1 in plane else 4.0 / n, lz=1.0 if 2 in plane else 4.0 / n)
+    gam = 1.4
+    p = ideal_gas_params(gamma=gam, mu_override=nu, tvd_off=tvd_off, cfl=0.5)
+    coords = [(np.arange(dims[0]) / dims[0])[None, None, :], (np.arange(dims[1]) / dims[1])[None, :, None],
+              (np.arange(dims[2]) / dims[2])[:, None, None]]
+    theta = 2 * np.pi * (coords[a1] + coords[a2])
+    A = 0.02
+    u = [0.0, 0.0, 0.0]
+    u[a1] = A / np.sqrt(2) * np.sin(theta)
+    u[a2] = -A / np.sqrt(2) * np.sin(theta)
+    X = state_from_primitives(g, p, 1.0, u[0], u[1], u[2], 1.0 / gam)      # c_s = 1
+    X, _ = advance_to(orc, orc.Problem(g, p), X, t_end)
+    prim = primitives_of(g, p, X)
+    amp = 2 * np.mean((prim[1 + a1] - prim[1 + a2]) / np.sqrt(2) * np.sin(theta + 0 * prim[0]))
+    return amp / A, np.exp(-nu * 8 * np.pi**2 * t_end)
+
+
+@pytest.mark.parametrize("plane", [(0, 2), (0, 1), (1, 2)])
+def test_oblique_shear_wave_decay_rate(orc, plane):
+    """Pins mu = sqrt(Pr/Ra)'s role and both halves of tau_ij = mu(d_j u_i + d_i u_j) (Eq. 18):
+    without the cross-derivative half the wave would decay 1.5x faster, with the wrong sign 2x."""
+    got, want = _shear_decay(orc, 48, plane)
+    assert got == pytest.approx(want, rel=6e-3), (got, want)
+    assert abs(np.log(got) / np.log(want) - 1.0) < 0.02
+    got_tvd, _ = _shear_decay(orc, 48, plane, tvd_off=0)
+    assert got_tvd == pytest.approx(want, rel=0.05)
+
+
+@pytest.mark.parametrize("lam", [-2.0 / 3.0, 2.0 / 3.0])
+def test_acoustic_attenuation_pins_dilatation_coefficient(orc, lam):
+    """A standing sound wave in a viscous, non-conducting gas loses acoustic energy as
+    exp(-(2 + lambda) nu k^2 t) (classical absorption, tau_xx = mu (2 + lambda) d_x u_x)."""
+    n, nu, gam, A = 64, 0.005, 1.4, 1e-3
+    g = periodic_grid(2, n, 4, lz=4.0 / n)
+    p = ideal_gas_params(gamma=gam, mu_override=nu, lambda_coef=lam, tvd_off=1)
+    x = (np.arange(n) / n)[None, None, :]
+    X = state_from_primitives(g, p, 1.0, A * np.sin(2 * np.pi * x), 0.0, 0.0, 1.0 / gam)
+
+    def energy(Y):
+        rho, ux, _, _, _, pr = primitives_of(g, p, Y)
+        return np.mean(0.5 * rho * ux**2 + (pr - 1.0 / gam) ** 2 / 2.0)     # rho0 c^2 = 1
+
+    t_end = 2.0
+    Y, _ = advance_to(orc, orc.Problem(g, p), X, t_end)
+    rate = np.log(energy(X) / energy(Y)) / t_end
+    assert rate == pytest.approx((2.0 + lam) * nu * (2 * np.pi) ** 2, rel=0.03)
+
+
+def test_thermal_diffusion_rate_pins_K(orc):
+    """Isobaric temperature ripple in a gas at rest decays at K k^2/(rho c_p), c_p = gamma c_v:
+    pins the -K dT/dx term of the energy flux (Eq. 15) and c_v of Eq. 17."""
+    n, K, gam, a = 64, 0.02, 1.4, 1e-3
+    g = periodic_grid(2, n, 4, lz=4.0 / n)
+    p = ideal_gas_params(gamma=gam, K_override=K, tvd_off=1)
+    x = (np.arange(n) / n)[None, None, :]
+    T0 = 1.0 / (gam * (gam - 1.0))                                          # c_s = 1 with R = gam-1
+    T = T0 * (1 + a * np.sin(2 * np.pi * x))
+    pr = 1.0 / gam
+    X = state_from_primitives(g, p, pr / ((gam - 1.0) * T), 0.0, 0.0, 0.0, pr)
+    t_end = 1.0
+    Y, _ = advance_to(orc, orc.Problem(g, p), X, t_end)
+    Tn = primitives_of(g, p, Y)[4]
+    amp = 2 * np.mean((Tn / T0 - 1) * np.sin(2 * np.pi * x + 0 * Tn)) / a
+    kappa = K / (1.0 * gam * 1.0)                                           # rho0 = 1, c_v = 1
+    assert amp == pytest.approx(np.exp(-kappa * (2 * np.pi) ** 2 * t_end), rel=0.02)
+
+
+def test_viscous_heating_pattern_pins_work_term(orc):
+    """Shear u_x = A sin(kz) heats the gas where the shear is largest: the early temperature rise
+    is mu A^2 k^2 cos^2(kz) t/(rho c_v), i.e. a positive cos(2kz) coefficient.  Without the
+    u_j tau_ij term of the energy flux (Eq. 15) that coefficient would be negative."""
+    n, nu, gam, A = 64, 0.02, 1.4, 0.05
+    g = periodic_grid(2, 4, n, lx=4.0 / n)
+    p = ideal_gas_params(gamma=gam, mu_override=nu, tvd_off=1)
+    z = (np.arange(n) / n)[:, None, None]
+    k = 2 * np.pi
+    X = state_from_primitives(g, p, 1.0, A * np.sin(k * z), 0.0, 0.0, 1.0 / gam)
+    T0 = primitives_of(g, p, X)[4]
+    t_end = 0.03                                                           # << acoustic time 0.5
+    Y, _ = advance_to(orc, orc.Problem(g, p), X, t_end)
+    dT = primitives_of(g, p, Y)[4] - T0
+    c2 = 2 * np.mean(dT * np.cos(2 * k * z + 0 * dT))
+    want = nu * A**2 * k**2 * t_end / 2.0                                   # rho = c_v = 1
+    assert 0.7 * want < c2 < 1.1 * want, (c2, want)
+
+
+# ----------------------------------------------------------------------------- gravity, plates
+def test_hydrostatic_conduction_state_drift_is_second_order(orc):
+    """The noise-free conduction state is a steady solution of Eqs. 13-15 (linear T: constant heat
+    flux; hydrostatic p).  The discrete drift is truncation error only: small and ~4x smaller per
+    grid doubling.  Pins the -rho/eps source (Eq. 14), the z/eps term of E (Eq. 17) and the plate
+    treatment."""
+    drift = []
+    for nz in (33, 65, 129):
+        g = inputs.make_grid(2, 8, nz, lx=8.0 / (nz - 1))
+        p = inputs.make_params(Ra=1e4)
+        X = inputs.conduction_state(g, p, amplitude=0.0)
+        Y, _ = advance_to(orc, orc.Problem(g, p), X, 0.05)
+        drift.append(np.abs(primitives_of(g, p, Y)[3]).max())
+    assert drift[0] < 2e-4
+    assert drift[0] / drift[1] > 3.3 and drift[1] / drift[2] > 3.3, drift
+
+
+def test_discrete_hydrostatic_density_is_polytrope():
+    """Input recipe: the hydrostatic polytrope of a linear T is rho = T^m with
+    m = gamma D/((gamma-1)(eps+D)) - 1 (from Eqs. 14, 16).  For the configs (gamma = 5/3, eps = 0.1,
+    D = 0.4) m = 1 and the trapezoid recursion is exact; for gamma = 1.4 (m = 1.8) it converges at
+    second order."""
+    for gam, m in ((5.0 / 3.0, 1.0), (1.4, 1.8)):
+        err = []
+        for nz in (33, 65):
+            g = inputs.make_grid(2, 4, nz)
+            p = inputs.make_params(gamma=gam)
+            X = inputs.conduction_state(g, p, amplitude=0.0)
+            rho = X[0].reshape(nz, 4)[:, 0]
+            err.append(np.abs(rho - (1 - 0.5 * inputs.z_nodes(g, p)) ** m).max())
+        if m == 1.0:
+            assert max(err) < 1e-14
+        else:
+            assert err[1] < 1e-4 and 3.5 < err[0] / err[1] < 4.5, err
+
+
+def test_plate_values_hold(orc):
+    """No-slip, isothermal plates: after any number of steps the plate nodes
+    carry zero momentum and exactly the plate temperatures."""
+    g = inputs.make_grid(2, 32, 17)
+    p = inputs.make_params(Ra=1e5)
+    X = inputs.smooth_random_state(g, p, seed=3)
+    Y, _, _ = orc.step(orc.Problem(g, p), X, 8)
+    rho, ux, _, uz, T, _ = primitives_of(g, p, Y)
+    for k, Tw in ((0, p["T_bot"]), (-1, p["T_top"])):
+        assert np.all(ux[k] == 0) and np.all(uz[k] == 0)
+        assert np.allclose(T[k], Tw, rtol=1e-13, atol=0)
+    assert rho.min() > 0
+
+
+# ----------------------------------------------------------------------------- diagnostics
+def test_diagnostics_closed_forms(orc):
+    """Conduction state: T_sa = -eps z so Nu_0 = Nu_1 = Nu_bulk = 1 and Re = 0 (Eqs. 22-26)."""
+    g, p, _ = inputs.config("C1")
+    prob = orc.Problem(g, p)
+    X = inputs.conduction_state(g, p, amplitude=0.0)
+    d, Tp, rp, pp = orc.diagnostics(prob, X)
+    for k in ("nu_bottom", "nu_top", "nu_bar", "nu_bulk"):
+        assert d[k] == pytest.approx(1.0, abs=1e-11), k
+    assert d["re"] == 0.0 and d["u_rms"] == 0.0 and d["nu_conv"] == 0.0 and d["nu_K"] == 0.0
+    z = inputs.z_nodes(g, p)
+    assert np.allclose(Tp, 1 - 0.5 * z, rtol=1e-13)
+    assert np.allclose(pp, 10.0 * rp * Tp, rtol=1e-13)
+    assert d["min_T"] == pytest.approx(0.5, rel=1e-13) and d["max_mach"] == 0.0
+
+
+def test_diagnostics_synthetic_flow(orc):
+    """Uniform rho, constant u_z = a, T = T_A + b + c z^2: every mean of Eqs. 22-26 has a closed
+    form, and the 2nd-order one-sided plate gradients are exact for a quadratic."""
+    g = inputs.make_grid(3, 6, 21, 5)
+    p = inputs.make_params(Ra=1e4, Pr=0.7)
+    a, b, c = 0.03, 0.05, -0.2
+    z = inputs.z_nodes(g, p)[:, None, None]
+    T = (1 - p["D"] * z) + b + c * z**2 + np.zeros((21, 5, 6))
+    X = inputs.pack(g, np.full_like(T, 1.25), 0 * T, 0 * T, a + 0 * T, T, p)
+    d, Tp, rp, pp = orc.diagnostics(orc.Problem(g, p), X)
+    sRaPr = np.sqrt(p["Ra"] * p["Pr"])
+    zz = z.ravel()
+    w = np.full(21, zz[1]); w[0] = w[-1] = zz[1] / 2
+    mean_tsa = np.sum(w * (b + c * zz**2)) / np.sum(w)
+    assert d["nu_conv"] == pytest.approx(sRaPr / p["eps"] * 1.25 * a * mean_tsa, rel=1e-12)
+    assert d["nu_K"] == pytest.approx(p["D"] * sRaPr / 2 * 1.25 * a**3, rel=1e-12)
+    assert d["nu_bulk"] == pytest.approx(1 + d["nu_conv"] + d["nu_K"], rel=1e-15)
+    assert d["re"] == pytest.approx(np.sqrt(p["Ra"] / p["Pr"]) * a, rel=1e-12)
+    assert d["nu_bottom"] == pytest.approx(0.0, abs=1e-11)
+    assert d["nu_top"] == pytest.approx(-2 * c / p["eps"], rel=1e-10)
+    assert d["nu_bar"] == pytest.approx(0.5 * (d["nu_bottom"] + d["nu_top"]), rel=1e-15)
+    assert d["mass"] == pytest.approx(1.25 * 16.0, rel=1e-13)
+    assert d["mom_z"] == pytest.approx(1.25 * a * 16.0, rel=1e-13)
+    assert np.allclose(rp, 1.25) and np.allclose(Tp, T[:, 0, 0], rtol=1e-14)
+
+
+def test_dt_rule(orc):
+    """R12: dt = cfl / max((|u_a| + c_s)/dx_a); closed form on a uniform state; NaN on bad data."""
+    g = periodic_grid(3, 8, 6, 4, lx=2.0, ly=1.0, lz=3.0)
+    p = ideal_gas_params(gamma=1.4, cfl=0.5)
+    X = state_from_primitives(g, p, 2.0, 0.3, -0.7, 0.1, 2.0 / 1.4)      # c_s = 1
+    prob = orc.Problem(g, p)
+    want = 0.5 / max(1.3 / (2.0 / 8), 1.7 / (1.0 / 4), 1.1 / (3.0 / 6))
+    assert orc.dt(prob, X) == pytest.approx(want, rel=1e-14)
+    p2 = ideal_gas_params(gamma=1.4, fixed_dt=1e-3)
+    assert orc.dt(orc.Problem(g, p2), X) == 1e-3
+    X[0, 5] = -1.0
+    assert np.isnan(orc.max_speed(prob, X))
+
+
+# ----------------------------------------------------------------------------- axis permutations
+def test_2d_is_3d_with_ny1_and_y_invariance(orc):
+    """A 3-D run of a y-invariant state equals the 2-D run copied along y, bit for bit: every
+    y-difference is an exact zero, so L_y is the identity there."""
+    g2 = inputs.make_grid(2, 16, 13)
+    p = inputs.make_params(Ra=1e4)
+    X2 = inputs.smooth_random_state(g2, p, seed=5)
+    g3 = inputs.make_grid(3, 16, 13, 4, ly=4 * 4.0 / 16)
+    F2 = X2.reshape(4, 13, 1, 16)
+    X3 = np.stack([np.repeat(F2[0], 4, 1), np.repeat(F2[1], 4, 1), np.zeros((13, 4, 16)),
+                   np.repeat(F2[2], 4, 1), np.repeat(F2[3], 4, 1)]).reshape(5, -1)
+    dts = [2e-3] * 3
+    Y2, _, _ = orc.step(orc.Problem(g2, p), X2, 3, dt_in=dts)
+    Y3, _, _ = orc.step(orc.Problem(g3, p), X3, 3, dt_in=dts)
+    G3 = Y3.reshape(5, 13, 4, 16)
+    for j in range(4):
+        assert np.array_equal(G3[[0, 1, 3, 4], :, j, :].reshape(4, -1), Y2)
+    assert np.all(G3[2] == 0)
+
+
+def _swap_axes(X, grid, a, b):
+    """Relabel axes a <-> b of a 3-D state (fields reshaped (nz, ny, nx)); returns (X', grid')."""
+    ax = {0: 3, 1: 2, 2: 1}
+    F = X.reshape(5, grid["nz"], grid["ny"], grid["nx"]).swapaxes(ax[a], ax[b]).copy()
+    F[[1 + a, 1 + b]] = F[[1 + b, 1 + a]]
+    n = ["nx", "ny", "nz"]; l = ["lx", "ly", "lz"]
+    g = dict(grid)
+    g[n[a]], g[n[b]] = grid[n[b]], grid[n[a]]
+    g[l[a]], g[l[b]] = grid[l[b]], grid[l[a]]
+    return F.reshape(5, -1), g
+
+
+@pytest.mark.parametrize("a,b", [(0, 1), (0, 2), (1, 2)])
+def test_sweeps_are_one_operator_under_axis_relabelling(orc, a, b):
+    """L_a on the relabelled state equals the relabelled L_b (all-periodic box, g = 0): the three
+    sweeps implement one 1-D operator, so every pin above holds for each of them.  Sums over
+    fields and axes change order under the relabelling, hence a few-ulp tolerance."""
+    g = periodic_grid(3, 12, 8, 10, lx=1.0, ly=0.9, lz=0.7)
+    p = ideal_gas_params(mu_override=4e-3, K_override=6e-3)
+    X = inputs.smooth_random_state(g, p, seed=13)
+    Xs, gs = _swap_axes(X, g, a, b)
+    for d in (+1, -1):
+        for sweep_axis in (0, 1, 2):
+            mapped = {a: b, b: a}.get(sweep_axis, sweep_axis)
+            lhs, _ = _swap_axes(orc.sweep(orc.Problem(g, p), X, sweep_axis, 0.004, d), g, a, b)
+            rhs = orc.sweep(orc.Problem(gs, p), Xs, mapped, 0.004, d)
+            assert np.max(rel_err(lhs, rhs)) < 1e-14, (sweep_axis, d)
