@@ -1,0 +1,123 @@
+/*
+ * include/mc_tvd.h -- C ABI of libmc_tvd.so, the B200 (sm_100a) MacCormack-TVD step of
+ * arXiv 2411.10372 ("Compressible turbulent convection at very high Rayleigh numbers").
+ *
+ * The library advances the conserved state X = (rho, rho u_x, [rho u_y,] rho u_z, E) of the fully
+ * compressible Navier-Stokes + energy equations with gravity (Eqs. 13-18; vector
+ * form PAPER.md:255-263, Eqs. 27-28) by the operator-split MacCormack predictor-corrector scheme with
+ * a TVD correction (Eqs. 29-39), chooses the time step by an acoustic CFL rule
+ * (reading R12; the paper is silent) and evaluates the Nusselt / Reynolds diagnostics
+ * (Eqs. 22-26).  Every step of that path runs in CUDA kernels; there is no CPU
+ * fallback.  All arithmetic is fp64.
+ *
+ * Conventions
+ *   - Plain C: POD structs, raw pointers, sizes.  No torch / C++ types.  "d_" = DEVICE pointer,
+ *     "h_" / unmarked = HOST pointer.
+ *   - Field layout (device): nf = 4 (2-D: rho, rho u_x, rho u_z, E) or 5 (3-D: rho, rho u_x,
+ *     rho u_y, rho u_z, E) arrays of N = nx*ny*nz doubles, one after the other (SoA); node (i,j,k)
+ *     at (k*ny + j)*nx + i; x fastest.  x_i = i lx/nx and y_j = j ly/ny are periodic; z_k = k lz/(nz-1)
+ *     with k = 0 and k = nz-1 ON the plates (z_k = k lz/nz when bc_z = 1).
+ *   - Ownership: the caller owns every device buffer (d_fields, d_workspace) and the stream; the
+ *     library owns only the host-side handle.  d_fields and d_workspace must stay valid and must
+ *     not be touched by the caller between a call and the next stream synchronisation.
+ *   - Errors: every int-returning call returns MC_TVD_OK (0) or a negative mc_tvd_status; it never
+ *     throws, aborts or prints.  mc_tvd_last_error() returns a thread-local message.
+ *   - Threading: a handle is not thread-safe; distinct handles are independent.
+ */
+#ifndef MC_TVD_H
+#define MC_TVD_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    MC_TVD_OK = 0,
+    MC_TVD_EINVAL = -1,       /* bad argument (NULL, size, unsupported switch value) */
+    MC_TVD_ECUDA = -2,        /* a CUDA runtime call or kernel launch failed */
+    MC_TVD_ENOMEM = -3,       /* workspace too small / host allocation failed */
+    MC_TVD_ENONFINITE = -4,   /* state holds a non-finite value or non-positive rho or T */
+    MC_TVD_EUNSUPPORTED = -5  /* valid request this build does not implement (e.g. z_nodes != NULL) */
+} mc_tvd_status;
+
+/* The box (Sec. 2; aspect ratio 4). */
+typedef struct {
+    int ndim;                 /* 2 or 3 */
+    int nx, ny, nz;           /* ny = 1 in 2-D; nx, ny = distinct periodic nodes; nz counts both plate nodes */
+    double lx, ly, lz;        /* box size: 4, 4, 1 for the paper's runs */
+    const double *z_nodes;    /* NULL = uniform z.  Non-NULL (tanh grid) -> MC_TVD_EUNSUPPORTED */
+} mc_tvd_grid;
+
+/* The paper's dimensionless numbers and the switches of DESIGN.md's readings. */
+typedef struct {
+    double gamma, Pr, Ra, eps, D;   /* PAPER.md:153-167 Eqs. 9-12; closures PAPER.md:189-193 Eqs. 16-18 */
+    double cfl, fixed_dt;           /* dt = cfl / max (|u_a| + c_s)/dx_a (R12); fixed_dt > 0 overrides */
+    double T_bot, T_top;            /* plate temperatures; paper: 1 and 1 - eps - D */
+    double lambda_coef;             /* dilatation coefficient in tau_ij: -2/3 (Stokes) or +2/3 (Eq. 18 as printed) */
+    double g_override, mu_override, K_override; /* < 0: derive from the paper's numbers; >= 0: use as is */
+    int bc_z;                       /* 0 = no-slip isothermal plates (paper); 1 = periodic z (test problems) */
+    int tvd_form;                   /* 0 = Eq. 34 as printed; 1 = Davis/Yee sum of two G's (R4) */
+    int dir_mode;                   /* 0 = backward predictor always (paper); 1 = alternate per half step (R9) */
+    int tvd_off;                    /* 1 = drop the TVD term (tests) */
+} mc_tvd_params;
+
+/* Result of mc_tvd_diagnostics (host POD).  Instantaneous values; Eqs. 22-26. */
+typedef struct {
+    double time, dt; long long step;       /* simulated time, dt the NEXT step will use, steps taken */
+    double nu_bottom, nu_top, nu_bar;      /* Eqs. 23-24: -(1/eps) d<T_sa>_A/dz at the plates, and their mean */
+    double nu_bulk, nu_conv, nu_K;         /* Eq. 22 */
+    double re, u_rms;                      /* Eq. 26 */
+    double mass, mom_x, mom_y, mom_z, energy; /* trapezoid-weighted volume totals of X */
+    double max_mach, min_rho, min_T;
+} mc_tvd_diag;
+
+typedef struct mc_tvd_state mc_tvd_state;  /* opaque host-side handle */
+
+/* Bytes of device workspace mc_tvd_init needs for this problem: the second (ping-pong) state
+ * buffer, reduction partials and device scalars.  0 on invalid arguments. */
+size_t mc_tvd_workspace_bytes(const mc_tvd_grid *grid, const mc_tvd_params *params);
+
+/* Create a handle.  d_fields (DEVICE, nf*N doubles, 16-byte aligned) holds the initial state and
+ * receives every later state; d_workspace (DEVICE, >= mc_tvd_workspace_bytes, 256-byte aligned) is
+ * scratch; cuda_stream is a cudaStream_t (NULL = the legacy default stream) on which ALL work of
+ * this handle is enqueued.  Enqueues the max-speed reduction of the initial state so that dt is
+ * defined (R12).  Does not synchronise. */
+int mc_tvd_init(const mc_tvd_grid *grid, const mc_tvd_params *params, double *d_fields,
+                void *d_workspace, size_t workspace_bytes, void *cuda_stream, mc_tvd_state **out);
+
+/* Advance n_steps steps of Eq. 30: X <- Lx Ly Lz Lx Ly Lz X, each operator with
+ * dt/2 (operators act right to left; no Ly in 2-D); dt from the CFL rule on the step's input state,
+ * kept on the device.  Asynchronous on the handle's stream; never synchronises.  The result is
+ * always back in d_fields. */
+int mc_tvd_step(mc_tvd_state *s, int n_steps);
+
+/* One operator L_alpha(tau) (Eqs. 31-39) applied to d_fields in place (through the workspace):
+ * alpha = 0,1,2 for x,y,z; dir = +1 backward predictor / forward corrector,
+ * -1 the mirrored pair.  Exposed for per-operator parity tests; does not advance time or dt. */
+int mc_tvd_sweep(mc_tvd_state *s, int alpha, int dir, double tau);
+
+/* dt the next step will use (host double).  Synchronises the stream.  MC_TVD_ENONFINITE if the
+ * state holds a non-finite value or a non-positive rho or T. */
+int mc_tvd_dt(mc_tvd_state *s, double *dt_host);
+
+/* Diagnostics of the current state (Eqs. 22-26) into a HOST struct, and the
+ * horizontal means <T>_A, <rho>_A, <p>_A into HOST arrays of nz doubles (each may be NULL).
+ * Synchronises the stream. */
+int mc_tvd_diagnostics(mc_tvd_state *s, mc_tvd_diag *out, double *T_prof, double *rho_prof,
+                       double *p_prof);
+
+/* Number of kernel launches this handle has enqueued so far (for bench.py's gpu_launches). */
+long long mc_tvd_launch_count(const mc_tvd_state *s);
+
+/* Free the handle (host memory only).  Synchronises the stream first. */
+int mc_tvd_destroy(mc_tvd_state *s);
+
+/* Thread-local message of the last failing call on this thread ("" if none). */
+const char *mc_tvd_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MC_TVD_H */

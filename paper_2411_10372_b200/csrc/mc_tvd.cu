@@ -1,0 +1,389 @@
+// mc_tvd.cu -- the C ABI of libmc_tvd.so (include/mc_tvd.h): host-side validation, derived
+// coefficients, launch geometry and the per-step launch list.  All arithmetic of the path runs in the
+// kernels of sweep_march.cuh, sweep_lane.cuh and reduce_kernels.cuh; this file only enqueues them.
+#include "../../include/mc_tvd.h"
+
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+#include <new>
+
+#include "mc_common.cuh"
+#include "reduce_kernels.cuh"
+#include "sweep_lane.cuh"
+#include "sweep_march.cuh"
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+int fail(int code, const char *fmt, const char *detail = "")
+{
+    snprintf(g_err, sizeof(g_err), fmt, detail);
+    return code;
+}
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+constexpr int MARCH_WX_2D = 128;       // k_march, 2-D: 124 outputs per block row
+constexpr int TILE_WB_3D = 16;         // 3-D tiles: 32 x 16 threads, 28 x 12 outputs
+constexpr int LANE_WARPS_2D = 4;       // k_lane, 2-D: independent warps per block
+constexpr int DIAG_MAX_BLOCKS = 64;    // blocks per plane in the diagnostics pass
+
+struct Layout {                        // byte offsets inside the workspace
+    size_t Y, scalars, partial, ext, plane_sums, diag_out, total;
+    int diag_blocks;
+};
+
+}  // namespace
+
+struct mc_tvd_state {
+    mc_tvd_grid grid;
+    mc_tvd_params par;
+    int nd, nf;
+    long long N, plane;
+    double d[3];                       // dx, dy, dz
+    double R, cv, icv, g, mu, K;
+    bool walls;
+    double *X, *Y;
+    mc::Scalars *S;
+    double *partial, *ext, *plane_sums, *diag_out;
+    int diag_blocks;
+    cudaStream_t stream;
+    long long launches;
+    int chunk_override;
+};
+
+namespace {
+
+bool valid_problem(const mc_tvd_grid *g, const mc_tvd_params *p, int *code)
+{
+    *code = MC_TVD_EINVAL;
+    if (!g || !p) return fail(0, "grid or params is NULL"), false;
+    if (g->ndim != 2 && g->ndim != 3) return fail(0, "ndim must be 2 or 3"), false;
+    if (g->nx < 4 || g->nz < 5 || g->ny < 1) return fail(0, "need nx >= 4, nz >= 5, ny >= 1"), false;
+    if (g->ndim == 2 && g->ny != 1) return fail(0, "ny must be 1 in 2-D"), false;
+    if (g->ndim == 3 && g->ny < 4) return fail(0, "need ny >= 4 in 3-D"), false;
+    if (!(g->lx > 0) || !(g->lz > 0) || (g->ndim == 3 && !(g->ly > 0))) return fail(0, "box size must be > 0"), false;
+    if (g->z_nodes) { *code = MC_TVD_EUNSUPPORTED; return fail(0, "non-uniform z grid is not built (SURVEY 8f)"), false; }
+    if (!(p->gamma > 1) || !(p->eps > 0) || !(p->D > 0) || !(p->Pr > 0) || !(p->Ra > 0))
+        return fail(0, "need gamma > 1 and eps, D, Pr, Ra > 0"), false;
+    if (!(p->fixed_dt > 0) && !(p->cfl > 0)) return fail(0, "need cfl > 0 or fixed_dt > 0"), false;
+    if ((p->bc_z | 1) != 1 || (p->tvd_form | 1) != 1 || (p->dir_mode | 1) != 1 || (p->tvd_off | 1) != 1)
+        return fail(0, "bc_z, tvd_form, dir_mode, tvd_off must be 0 or 1"), false;
+    return true;
+}
+
+Layout make_layout(const mc_tvd_grid *g)
+{
+    Layout L;
+    const size_t nf = (g->ndim == 2) ? 4 : 5;
+    const size_t N = (size_t)g->nx * g->ny * g->nz, plane = (size_t)g->nx * g->ny;
+    int nb = (int)((plane + (size_t)mc::DIAG_THREADS * 8 - 1) / ((size_t)mc::DIAG_THREADS * 8));
+    if (nb < 1) nb = 1;
+    if (nb > DIAG_MAX_BLOCKS) nb = DIAG_MAX_BLOCKS;
+    L.diag_blocks = nb;
+    size_t o = 0;
+    L.Y = o;          o = align_up(o + nf * N * sizeof(double), 256);
+    L.scalars = o;    o = align_up(o + sizeof(mc::Scalars), 256);
+    L.partial = o;    o = align_up(o + (size_t)g->nz * nb * 2 * mc::DQ_MAXQ * sizeof(double), 256);
+    L.ext = o;        o = align_up(o + (size_t)g->nz * nb * 3 * sizeof(double), 256);
+    L.plane_sums = o; o = align_up(o + (size_t)g->nz * mc::DQ_MAXQ * sizeof(double), 256);
+    L.diag_out = o;   o = align_up(o + (19 + 3 * (size_t)g->nz) * sizeof(double), 256);
+    L.total = o;
+    return L;
+}
+
+int cuda_check(cudaError_t e, const char *what)
+{
+    if (e == cudaSuccess) return MC_TVD_OK;
+    snprintf(g_err, sizeof(g_err), "%s: %s", what, cudaGetErrorString(e));
+    return MC_TVD_ECUDA;
+}
+
+// velocity-component index of physical axis a (0 x, 1 y, 2 z): 2-D carries (x, z)
+int comp_of_axis(int nd, int a) { return (nd == 2) ? (a == 0 ? 0 : 1) : a; }
+
+void fill_common(const mc_tvd_state *s, mc::SweepArgs &A, const double *in, double *out, int alpha, int dir,
+                 double tau, bool use_dt, bool reduce)
+{
+    memset(&A, 0, sizeof(A));
+    A.in = in; A.out = out;
+    A.dt_ptr = use_dt ? &s->S->dt : nullptr;
+    A.tau_fixed = tau;
+    A.smax_bits = &s->S->smax_bits;
+    A.N = s->N; A.nx = s->grid.nx;
+    A.dir = dir;
+    A.src = (alpha == 2);
+    A.tvd_form = s->par.tvd_form; A.tvd_off = s->par.tvd_off;
+    A.reduce = reduce ? 1 : 0;
+    A.d_a = s->d[alpha];
+    A.inv2d_x = 1.0 / (2.0 * s->d[0]);
+    for (int a = 0; a < 3; ++a) {
+        if (s->nd == 2 && a == 1) continue;
+        A.inv_d[comp_of_axis(s->nd, a)] = 1.0 / s->d[a];
+    }
+    A.dz = s->d[2];
+    A.R = s->R; A.cv = s->cv; A.icv = s->icv; A.g = s->g; A.mu = s->mu; A.K = s->K;
+    A.lam = s->par.lambda_coef; A.gamma = s->par.gamma;
+    A.Tw0 = s->par.T_bot; A.Tw1 = s->par.T_top;
+    A.nz = s->grid.nz;
+}
+
+int pick_chunk(const mc_tvd_state *s, int n_m, long long tiles)
+{
+    if (s->chunk_override > 0) return s->chunk_override < n_m ? s->chunk_override : n_m;
+    // enough blocks for a few waves over 148 SMs, but chunks long enough to amortise the 4-level warm-up
+    int chunk = n_m;
+    while (chunk > 64 && tiles * ((n_m + chunk - 1) / chunk) < 148 * 8) chunk = (chunk + 1) / 2;
+    return chunk;
+}
+
+// Enqueue one operator L_alpha(tau): in -> out.
+int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int dir, double tau, bool use_dt,
+                 bool reduce)
+{
+    mc::SweepArgs A;
+    fill_common(s, A, in, out, alpha, dir, tau, use_dt, reduce);
+    const int nx = s->grid.nx, ny = s->grid.ny, nz = s->grid.nz;
+    const int wl = s->walls ? 1 : 0;
+    dim3 block, grid;
+    size_t smem = 0;
+    if (s->nd == 2) {
+        if (alpha == 2) {            // z-sweep: march z, tile x
+            A.n_b = 1; A.s_b = 0; A.n_m = nz; A.s_m = nx; A.wall_m = wl; A.wall_b = 0;
+            block = dim3(MARCH_WX_2D, 1, 1);
+            long long tiles = (nx + MARCH_WX_2D - 5) / (MARCH_WX_2D - 4);
+            A.chunk = pick_chunk(s, nz, tiles);
+            grid = dim3((unsigned)tiles, 1, (unsigned)((nz + A.chunk - 1) / A.chunk));
+            smem = (size_t)4 * 2 * MARCH_WX_2D * sizeof(double);
+            mc::k_march<2, 1, -1><<<grid, block, smem, s->stream>>>(A);
+        } else if (alpha == 0) {     // x-sweep: lanes x, march z
+            A.n_b = 1; A.s_b = 0; A.n_m = nz; A.s_m = nx; A.wall_m = wl; A.wall_b = 0;
+            A.inv2d_m = 1.0 / (2.0 * s->d[2]);
+            block = dim3(32, LANE_WARPS_2D, 1);
+            long long xt = (nx + mc::LANE_OUT - 1) / mc::LANE_OUT;
+            long long tiles = (xt + LANE_WARPS_2D - 1) / LANE_WARPS_2D;
+            A.chunk = pick_chunk(s, nz, tiles);
+            grid = dim3((unsigned)tiles, 1, (unsigned)((nz + A.chunk - 1) / A.chunk));
+            mc::k_lane<2, -1, 1><<<grid, block, 0, s->stream>>>(A);
+        } else {
+            return fail(MC_TVD_EINVAL, "a 2-D problem has no y-sweep");
+        }
+    } else {
+        const int WB = TILE_WB_3D, OB = WB - 4;
+        block = dim3(32, WB, 1);
+        long long xt = (nx + mc::LANE_OUT - 1) / mc::LANE_OUT;
+        if (alpha == 2) {            // z-sweep: march z, tile (x, y)
+            A.n_b = ny; A.s_b = nx; A.wall_b = 0; A.inv2d_b = 1.0 / (2.0 * s->d[1]);
+            A.n_m = nz; A.s_m = (long long)nx * ny; A.wall_m = wl;
+            long long bt = (ny + OB - 1) / OB;
+            A.chunk = pick_chunk(s, nz, xt * bt);
+            grid = dim3((unsigned)xt, (unsigned)bt, (unsigned)((nz + A.chunk - 1) / A.chunk));
+            smem = (size_t)4 * 3 * 32 * WB * sizeof(double);
+            mc::k_march<3, 2, 1><<<grid, block, smem, s->stream>>>(A);
+        } else if (alpha == 1) {     // y-sweep: march y, tile (x, z)
+            A.n_b = nz; A.s_b = (long long)nx * ny; A.wall_b = wl; A.inv2d_b = 1.0 / (2.0 * s->d[2]);
+            A.n_m = ny; A.s_m = nx; A.wall_m = 0;
+            long long bt = (nz + OB - 1) / OB;
+            A.chunk = pick_chunk(s, ny, xt * bt);
+            grid = dim3((unsigned)xt, (unsigned)bt, (unsigned)((ny + A.chunk - 1) / A.chunk));
+            smem = (size_t)4 * 3 * 32 * WB * sizeof(double);
+            mc::k_march<3, 1, 2><<<grid, block, smem, s->stream>>>(A);
+        } else {                     // x-sweep: lanes x, tile (x, y), march z
+            A.n_b = ny; A.s_b = nx; A.wall_b = 0; A.inv2d_b = 1.0 / (2.0 * s->d[1]);
+            A.n_m = nz; A.s_m = (long long)nx * ny; A.wall_m = wl; A.inv2d_m = 1.0 / (2.0 * s->d[2]);
+            long long bt = (ny + OB - 1) / OB;
+            A.chunk = pick_chunk(s, nz, xt * bt);
+            grid = dim3((unsigned)xt, (unsigned)bt, (unsigned)((nz + A.chunk - 1) / A.chunk));
+            smem = (size_t)4 * 2 * 32 * WB * sizeof(double);
+            mc::k_lane<3, 1, 2><<<grid, block, smem, s->stream>>>(A);
+        }
+    }
+    s->launches += 1;
+    return cuda_check(cudaGetLastError(), "sweep launch");
+}
+
+mc::PointArgs point_args(const mc_tvd_state *s)
+{
+    mc::PointArgs P;
+    memset(&P, 0, sizeof(P));
+    P.X = s->X; P.N = s->N; P.plane = s->plane; P.nz = s->grid.nz;
+    P.dz = s->d[2]; P.g = s->g; P.icv = s->icv; P.R = s->R; P.gamma = s->par.gamma; P.D = s->par.D;
+    for (int a = 0; a < 3; ++a) {
+        if (s->nd == 2 && a == 1) continue;
+        P.inv_d[comp_of_axis(s->nd, a)] = 1.0 / s->d[a];
+    }
+    return P;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *mc_tvd_last_error(void) { return g_err; }
+
+size_t mc_tvd_workspace_bytes(const mc_tvd_grid *grid, const mc_tvd_params *params)
+{
+    int code;
+    if (!valid_problem(grid, params, &code)) return 0;
+    return make_layout(grid).total;
+}
+
+int mc_tvd_init(const mc_tvd_grid *grid, const mc_tvd_params *params, double *d_fields, void *d_workspace,
+                size_t workspace_bytes, void *cuda_stream, mc_tvd_state **out)
+{
+    int code;
+    if (!out) return fail(MC_TVD_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (!valid_problem(grid, params, &code)) return code;
+    if (!d_fields || !d_workspace) return fail(MC_TVD_EINVAL, "d_fields or d_workspace is NULL");
+    if (((uintptr_t)d_fields & 15) || ((uintptr_t)d_workspace & 255))
+        return fail(MC_TVD_EINVAL, "d_fields must be 16-byte and d_workspace 256-byte aligned");
+    Layout L = make_layout(grid);
+    if (workspace_bytes < L.total) return fail(MC_TVD_ENOMEM, "workspace smaller than mc_tvd_workspace_bytes");
+    mc_tvd_state *s = new (std::nothrow) mc_tvd_state;
+    if (!s) return fail(MC_TVD_ENOMEM, "host allocation failed");
+    memset(s, 0, sizeof(*s));
+    s->grid = *grid; s->par = *params;
+    s->nd = grid->ndim; s->nf = (grid->ndim == 2) ? 4 : 5;
+    s->plane = (long long)grid->nx * grid->ny;
+    s->N = s->plane * grid->nz;
+    s->walls = (params->bc_z == 0);
+    // grid spacings (R17) and coefficients from the paper's numbers (Eqs. 14-18)
+    s->d[0] = grid->lx / grid->nx;
+    s->d[1] = (grid->ndim == 3) ? grid->ly / grid->ny : 1.0;
+    s->d[2] = s->walls ? grid->lz / (grid->nz - 1) : grid->lz / grid->nz;
+    s->icv = params->gamma * params->eps * params->D;
+    s->cv = 1.0 / s->icv;
+    s->R = (params->gamma - 1.0) / s->icv;
+    s->g = (params->g_override >= 0.0) ? params->g_override : 1.0 / params->eps;
+    s->mu = (params->mu_override >= 0.0) ? params->mu_override : sqrt(params->Pr / params->Ra);
+    s->K = (params->K_override >= 0.0) ? params->K_override
+                                       : 1.0 / (params->eps * params->D * sqrt(params->Ra * params->Pr));
+    char *w = (char *)d_workspace;
+    s->X = d_fields;
+    s->Y = (double *)(w + L.Y);
+    s->S = (mc::Scalars *)(w + L.scalars);
+    s->partial = (double *)(w + L.partial);
+    s->ext = (double *)(w + L.ext);
+    s->plane_sums = (double *)(w + L.plane_sums);
+    s->diag_out = (double *)(w + L.diag_out);
+    s->diag_blocks = L.diag_blocks;
+    s->stream = (cudaStream_t)cuda_stream;
+    const char *ce = getenv("MC_TVD_CHUNK");
+    s->chunk_override = ce ? atoi(ce) : 0;
+
+    mc::Scalars h;
+    memset(&h, 0, sizeof(h));
+    h.cfl = params->cfl; h.fixed_dt = params->fixed_dt;
+    int rc = cuda_check(cudaMemcpyAsync(s->S, &h, sizeof(h), cudaMemcpyHostToDevice, s->stream), "scalar upload");
+    if (rc == MC_TVD_OK) rc = cuda_check(cudaStreamSynchronize(s->stream), "scalar upload sync");   // h is on the stack
+    if (rc == MC_TVD_OK) {
+        mc::PointArgs P = point_args(s);
+        int blocks = (int)((s->N + 255) / 256);
+        if (blocks > 148 * 16) blocks = 148 * 16;
+        if (s->nd == 2) mc::k_max_speed<2><<<blocks, 256, 0, s->stream>>>(P, &s->S->smax_bits);
+        else mc::k_max_speed<3><<<blocks, 256, 0, s->stream>>>(P, &s->S->smax_bits);
+        mc::k_dt_update<<<1, 32, 0, s->stream>>>(s->S, 0);
+        s->launches += 2;
+        rc = cuda_check(cudaGetLastError(), "init launch");
+    }
+    if (rc != MC_TVD_OK) { delete s; return rc; }
+    *out = s;
+    return MC_TVD_OK;
+}
+
+int mc_tvd_step(mc_tvd_state *s, int n_steps)
+{
+    if (!s || n_steps < 0) return fail(MC_TVD_EINVAL, "bad handle or n_steps");
+    for (int it = 0; it < n_steps; ++it) {
+        const double *src = s->X;
+        double *dst = s->Y;
+        for (int half = 0; half < 2; ++half) {
+            int dir = (half == 1 && s->par.dir_mode == 1) ? -1 : +1;
+            for (int a = 2; a >= 0; --a) {                       // L_z, then L_y, then L_x (Eq. 30)
+                if (s->nd == 2 && a == 1) continue;
+                bool last = (half == 1 && a == 0);
+                int rc = launch_sweep(s, src, dst, a, dir, 0.0, true, last);
+                if (rc != MC_TVD_OK) return rc;
+                const double *t = src; src = dst; dst = (double *)t;
+            }
+        }
+        mc::k_dt_update<<<1, 32, 0, s->stream>>>(s->S, 1);
+        s->launches += 1;
+        int rc = cuda_check(cudaGetLastError(), "dt launch");
+        if (rc != MC_TVD_OK) return rc;
+    }
+    return MC_TVD_OK;
+}
+
+int mc_tvd_sweep(mc_tvd_state *s, int alpha, int dir, double tau)
+{
+    if (!s || alpha < 0 || alpha > 2 || (dir != 1 && dir != -1) || !(tau > 0))
+        return fail(MC_TVD_EINVAL, "bad handle, alpha, dir or tau");
+    int rc = launch_sweep(s, s->X, s->Y, alpha, dir, tau, false, false);
+    if (rc != MC_TVD_OK) return rc;
+    return cuda_check(cudaMemcpyAsync(s->X, s->Y, (size_t)s->nf * s->N * sizeof(double), cudaMemcpyDeviceToDevice,
+                                      s->stream), "sweep copy-back");
+}
+
+int mc_tvd_dt(mc_tvd_state *s, double *dt_host)
+{
+    if (!s || !dt_host) return fail(MC_TVD_EINVAL, "bad handle or dt_host");
+    int rc = cuda_check(cudaMemcpyAsync(dt_host, &s->S->dt, sizeof(double), cudaMemcpyDeviceToHost, s->stream), "dt copy");
+    if (rc == MC_TVD_OK) rc = cuda_check(cudaStreamSynchronize(s->stream), "dt sync");
+    if (rc != MC_TVD_OK) return rc;
+    if (!(*dt_host > 0.0) || !isfinite(*dt_host))
+        return fail(MC_TVD_ENONFINITE, "state holds a non-finite value or a non-positive rho or T");
+    return MC_TVD_OK;
+}
+
+int mc_tvd_diagnostics(mc_tvd_state *s, mc_tvd_diag *out, double *T_prof, double *rho_prof, double *p_prof)
+{
+    if (!s || !out) return fail(MC_TVD_EINVAL, "bad handle or out");
+    static_assert(sizeof(mc_tvd_diag) == 19 * sizeof(double), "mc_tvd_diag layout");
+    mc::PointArgs P = point_args(s);
+    dim3 grid((unsigned)s->diag_blocks, (unsigned)s->grid.nz, 1);
+    if (s->nd == 2) mc::k_plane_partials<2><<<grid, mc::DIAG_THREADS, 0, s->stream>>>(P, s->partial, s->ext);
+    else mc::k_plane_partials<3><<<grid, mc::DIAG_THREADS, 0, s->stream>>>(P, s->partial, s->ext);
+    mc::DiagArgs G;
+    memset(&G, 0, sizeof(G));
+    G.partial = s->partial; G.ext = s->ext; G.plane_sums = s->plane_sums; G.out = s->diag_out; G.S = s->S;
+    G.nz = s->grid.nz; G.nblk = s->diag_blocks; G.nq = 6 + s->nf; G.walls = s->walls ? 1 : 0;
+    G.nplane = (double)s->grid.nx * (double)s->grid.ny;
+    G.dz = s->d[2]; G.dxdy = s->d[0] * s->d[1];
+    G.eps = s->par.eps; G.D = s->par.D; G.Ra = s->par.Ra; G.Pr = s->par.Pr;
+    mc::k_diag_finish<<<1, mc::DIAG_THREADS, 0, s->stream>>>(G);
+    s->launches += 2;
+    int rc = cuda_check(cudaGetLastError(), "diagnostics launch");
+    if (rc != MC_TVD_OK) return rc;
+    const size_t nz = (size_t)s->grid.nz;
+    double *h = (double *)malloc((19 + 3 * nz) * sizeof(double));
+    if (!h) return fail(MC_TVD_ENOMEM, "host allocation failed");
+    rc = cuda_check(cudaMemcpyAsync(h, s->diag_out, (19 + 3 * nz) * sizeof(double), cudaMemcpyDeviceToHost, s->stream),
+                    "diagnostics copy");
+    if (rc == MC_TVD_OK) rc = cuda_check(cudaStreamSynchronize(s->stream), "diagnostics sync");
+    if (rc == MC_TVD_OK) {
+        memcpy(out, h, sizeof(*out));
+        if (T_prof) memcpy(T_prof, h + 19, nz * sizeof(double));
+        if (rho_prof) memcpy(rho_prof, h + 19 + nz, nz * sizeof(double));
+        if (p_prof) memcpy(p_prof, h + 19 + 2 * nz, nz * sizeof(double));
+    }
+    free(h);
+    return rc;
+}
+
+long long mc_tvd_launch_count(const mc_tvd_state *s) { return s ? s->launches : 0; }
+
+int mc_tvd_destroy(mc_tvd_state *s)
+{
+    if (!s) return MC_TVD_OK;
+    cudaError_t e = cudaStreamSynchronize(s->stream);
+    delete s;
+    return cuda_check(e, "destroy sync");
+}
+
+}  // extern "C"
