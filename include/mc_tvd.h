@@ -98,6 +98,13 @@ int mc_tvd_step(mc_tvd_state *s, int n_steps);
  * -1 the mirrored pair.  Exposed for per-operator parity tests; does not advance time or dt. */
 int mc_tvd_sweep(mc_tvd_state *s, int alpha, int dir, double tau);
 
+/* The end-to-end call for callers whose state lives in HOST memory (pinned memory makes the copies
+ * asynchronous, pageable memory works too): copies h_in (HOST, nf*N doubles, same layout) into
+ * d_fields, recomputes dt from it (as mc_tvd_init does) and resets time and step count to zero, runs
+ * n_steps steps, copies the result into h_out (HOST, nf*N doubles; may alias h_in) and synchronises
+ * the stream.  Every arithmetic step still runs in the kernels; this call only adds the two copies. */
+int mc_tvd_step_host(mc_tvd_state *s, const double *h_in, double *h_out, int n_steps);
+
 /* dt the next step will use (host double).  Synchronises the stream.  MC_TVD_ENONFINITE if the
  * state holds a non-finite value or a non-positive rho or T. */
 int mc_tvd_dt(mc_tvd_state *s, double *dt_host);

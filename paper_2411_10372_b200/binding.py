@@ -1,0 +1,209 @@
+"""Thin ctypes binding over the C-ABI library libmc_tvd.so (include/mc_tvd.h).
+
+Argument marshalling only: every step of the path (Eqs. 27-39, the CFL reduction,
+the diagnostics of Eqs. 22-26) runs in the CUDA kernels behind the C ABI.  PyTorch supplies device
+memory and the stream, nothing else.  There is no CPU fallback: if the library cannot be loaded the
+import of this module's users fails with the reason.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from .build import LIB_PATH, build_library
+
+_DP = C.POINTER(C.c_double)
+
+
+class Grid(C.Structure):            # mc_tvd_grid
+    _fields_ = [("ndim", C.c_int), ("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int),
+                ("lx", C.c_double), ("ly", C.c_double), ("lz", C.c_double), ("z_nodes", _DP)]
+
+
+class Params(C.Structure):          # mc_tvd_params
+    _fields_ = [("gamma", C.c_double), ("Pr", C.c_double), ("Ra", C.c_double), ("eps", C.c_double),
+                ("D", C.c_double), ("cfl", C.c_double), ("fixed_dt", C.c_double),
+                ("T_bot", C.c_double), ("T_top", C.c_double), ("lambda_coef", C.c_double),
+                ("g_override", C.c_double), ("mu_override", C.c_double), ("K_override", C.c_double),
+                ("bc_z", C.c_int), ("tvd_form", C.c_int), ("dir_mode", C.c_int), ("tvd_off", C.c_int)]
+
+
+class Diag(C.Structure):            # mc_tvd_diag
+    _fields_ = [("time", C.c_double), ("dt", C.c_double), ("step", C.c_longlong),
+                ("nu_bottom", C.c_double), ("nu_top", C.c_double), ("nu_bar", C.c_double),
+                ("nu_bulk", C.c_double), ("nu_conv", C.c_double), ("nu_K", C.c_double),
+                ("re", C.c_double), ("u_rms", C.c_double),
+                ("mass", C.c_double), ("mom_x", C.c_double), ("mom_y", C.c_double),
+                ("mom_z", C.c_double), ("energy", C.c_double),
+                ("max_mach", C.c_double), ("min_rho", C.c_double), ("min_T", C.c_double)]
+
+
+# every symbol include/mc_tvd.h declares: name -> (restype, argtypes)
+SYMBOLS = {
+    "mc_tvd_workspace_bytes": (C.c_size_t, [C.POINTER(Grid), C.POINTER(Params)]),
+    "mc_tvd_init": (C.c_int, [C.POINTER(Grid), C.POINTER(Params), C.c_void_p, C.c_void_p, C.c_size_t,
+                              C.c_void_p, C.POINTER(C.c_void_p)]),
+    "mc_tvd_step": (C.c_int, [C.c_void_p, C.c_int]),
+    "mc_tvd_sweep": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_double]),
+    "mc_tvd_step_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]),
+    "mc_tvd_dt": (C.c_int, [C.c_void_p, _DP]),
+    "mc_tvd_diagnostics": (C.c_int, [C.c_void_p, C.POINTER(Diag), _DP, _DP, _DP]),
+    "mc_tvd_launch_count": (C.c_longlong, [C.c_void_p]),
+    "mc_tvd_destroy": (C.c_int, [C.c_void_p]),
+    "mc_tvd_last_error": (C.c_char_p, []),
+}
+
+STATUS = {0: "MC_TVD_OK", -1: "MC_TVD_EINVAL", -2: "MC_TVD_ECUDA", -3: "MC_TVD_ENOMEM",
+          -4: "MC_TVD_ENONFINITE", -5: "MC_TVD_EUNSUPPORTED"}
+
+
+class MCTVDError(RuntimeError):
+    def __init__(self, code: int, message: str):
+        super().__init__(f"{STATUS.get(code, code)}: {message}")
+        self.code = code
+
+
+_lib = None
+
+
+def declare(lib: C.CDLL) -> C.CDLL:
+    """Attach the prototypes of include/mc_tvd.h to a loaded library."""
+    for name, (res, args) in SYMBOLS.items():
+        fn = getattr(lib, name)          # AttributeError if the symbol is missing
+        fn.restype = res
+        fn.argtypes = args
+    return lib
+
+
+def load_library(path: str | None = None) -> C.CDLL:
+    """Load libmc_tvd.so, building it with nvcc first if it is missing or stale.  Raises (never
+    falls back) when neither works."""
+    global _lib
+    if _lib is not None and path is None:
+        return _lib
+    if path is None:
+        if os.environ.get("MC_TVD_NO_BUILD") != "1":
+            build_library()
+        path = LIB_PATH
+    if not os.path.exists(path):
+        raise ImportError(f"{path} is missing: run `python -m paper_2411_10372_b200.build` (needs nvcc)")
+    lib = declare(C.CDLL(path))
+    if path == LIB_PATH:
+        _lib = lib
+    return lib
+
+
+def make_grid(grid: dict) -> Grid:
+    return Grid(int(grid["ndim"]), int(grid["nx"]), int(grid.get("ny", 1)), int(grid["nz"]),
+                float(grid["lx"]), float(grid.get("ly", 1.0)), float(grid["lz"]), None)
+
+
+def make_params(p: dict) -> Params:
+    return Params(p["gamma"], p["Pr"], p["Ra"], p["eps"], p["D"], p["cfl"], p["fixed_dt"],
+                  p["T_bot"], p["T_top"], p["lambda_coef"], p["g_override"], p["mu_override"],
+                  p["K_override"], int(p["bc_z"]), int(p["tvd_form"]), int(p["dir_mode"]),
+                  int(p["tvd_off"]))
+
+
+class MCTVD:
+    """One solver handle: owns the torch device buffers and the C handle.
+
+    X0: initial conserved state, numpy (nf, N) / flat, or a CUDA float64 torch tensor (copied).
+    """
+
+    def __init__(self, grid: dict, params: dict, X0, device="cuda:0", stream=None):
+        import torch
+
+        self._torch = torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("mc_tvd needs a CUDA device (sm_100a); there is no CPU fallback")
+        self.lib = load_library()
+        self.grid, self.params = dict(grid), dict(params)
+        self.nf = 4 if int(grid["ndim"]) == 2 else 5
+        self.N = int(grid["nx"]) * int(grid.get("ny", 1)) * int(grid["nz"])
+        self.nz = int(grid["nz"])
+        self.device = torch.device(device)
+        self._g, self._p = make_grid(grid), make_params(params)
+        wb = self.lib.mc_tvd_workspace_bytes(C.byref(self._g), C.byref(self._p))
+        if wb == 0:
+            raise MCTVDError(-1, self.lib.mc_tvd_last_error().decode())
+        with torch.cuda.device(self.device):
+            self.stream = stream if stream is not None else torch.cuda.current_stream()
+            self.fields = torch.empty(self.nf * self.N, dtype=torch.float64, device=self.device)
+            self.workspace = torch.empty((wb + 7) // 8, dtype=torch.float64, device=self.device)
+            self.set_state(X0)
+            h = C.c_void_p()
+            rc = self.lib.mc_tvd_init(C.byref(self._g), C.byref(self._p), self.fields.data_ptr(),
+                                      self.workspace.data_ptr(), self.workspace.numel() * 8,
+                                      self.stream.cuda_stream, C.byref(h))
+        self._h = h
+        self._check(rc)
+
+    # -- helpers ------------------------------------------------------------------------------
+    def _check(self, rc: int):
+        if rc != 0:
+            raise MCTVDError(rc, self.lib.mc_tvd_last_error().decode())
+
+    def set_state(self, X0):
+        """Copy a state into the device fields (does NOT recompute dt; init does that)."""
+        torch = self._torch
+        if isinstance(X0, torch.Tensor):
+            src = X0.to(dtype=torch.float64).reshape(-1)
+        else:
+            src = torch.from_numpy(np.ascontiguousarray(X0, dtype=np.float64).reshape(-1))
+        assert src.numel() == self.nf * self.N, (src.numel(), self.nf, self.N)
+        with torch.cuda.stream(self.stream):
+            self.fields.copy_(src, non_blocking=False)
+
+    # -- the C ABI, one method per call ---------------------------------------------------------
+    def step(self, n_steps: int = 1):
+        self._check(self.lib.mc_tvd_step(self._h, int(n_steps)))
+
+    def sweep(self, alpha: int, direction: int, tau: float):
+        self._check(self.lib.mc_tvd_sweep(self._h, int(alpha), int(direction), float(tau)))
+
+    def step_host(self, h_in, h_out, n_steps: int):
+        """h_in / h_out: CPU float64 torch tensors (pinned for async copies) or numpy arrays."""
+        self._check(self.lib.mc_tvd_step_host(self._h, _host_ptr(h_in), _host_ptr(h_out), int(n_steps)))
+
+    def dt(self) -> float:
+        v = C.c_double()
+        self._check(self.lib.mc_tvd_dt(self._h, C.byref(v)))
+        return v.value
+
+    def diagnostics(self):
+        """Returns (dict of scalars, T_prof, rho_prof, p_prof) -- same shape as the oracle's."""
+        d = Diag()
+        Tp, rp, pp = np.zeros(self.nz), np.zeros(self.nz), np.zeros(self.nz)
+        self._check(self.lib.mc_tvd_diagnostics(self._h, C.byref(d), Tp.ctypes.data_as(_DP),
+                                                rp.ctypes.data_as(_DP), pp.ctypes.data_as(_DP)))
+        return {n: getattr(d, n) for n, _ in Diag._fields_}, Tp, rp, pp
+
+    def launch_count(self) -> int:
+        return int(self.lib.mc_tvd_launch_count(self._h))
+
+    def state(self) -> np.ndarray:
+        """Download the current state as numpy (nf, N).  Synchronises."""
+        self.stream.synchronize()
+        return self.fields.cpu().numpy().reshape(self.nf, self.N)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self.lib.mc_tvd_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def _host_ptr(a) -> int:
+    if isinstance(a, np.ndarray):
+        assert a.dtype == np.float64 and a.flags["C_CONTIGUOUS"]
+        return a.ctypes.data
+    assert a.device.type == "cpu" and a.is_contiguous()
+    return a.data_ptr()

@@ -28,7 +28,7 @@ int fail(int code, const char *fmt, const char *detail = "")
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 constexpr int MARCH_WX_2D = 128;       // k_march, 2-D: 124 outputs per block row
-constexpr int TILE_WB_3D = 16;         // 3-D tiles: 32 x 16 threads, 28 x 12 outputs
+constexpr int TILE_WB_3D = 12;         // 3-D tiles: 32 x 12 threads, 28 x 8 outputs (register-limited)
 constexpr int LANE_WARPS_2D = 4;       // k_lane, 2-D: independent warps per block
 constexpr int DIAG_MAX_BLOCKS = 64;    // blocks per plane in the diagnostics pass
 
@@ -159,7 +159,7 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
             A.chunk = pick_chunk(s, nz, tiles);
             grid = dim3((unsigned)tiles, 1, (unsigned)((nz + A.chunk - 1) / A.chunk));
             smem = (size_t)4 * 2 * MARCH_WX_2D * sizeof(double);
-            mc::k_march<2, 1, -1><<<grid, block, smem, s->stream>>>(A);
+            { auto kfn = mc::k_march<2, 1, -1>; MC_LAUNCH(kfn, grid, block, smem, s->stream, A); }
         } else if (alpha == 0) {     // x-sweep: lanes x, march z
             A.n_b = 1; A.s_b = 0; A.n_m = nz; A.s_m = nx; A.wall_m = wl; A.wall_b = 0;
             A.inv2d_m = 1.0 / (2.0 * s->d[2]);
@@ -168,7 +168,7 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
             long long tiles = (xt + LANE_WARPS_2D - 1) / LANE_WARPS_2D;
             A.chunk = pick_chunk(s, nz, tiles);
             grid = dim3((unsigned)tiles, 1, (unsigned)((nz + A.chunk - 1) / A.chunk));
-            mc::k_lane<2, -1, 1><<<grid, block, 0, s->stream>>>(A);
+            { auto kfn = mc::k_lane<2, -1, 1>; MC_LAUNCH(kfn, grid, block, 0, s->stream, A); }
         } else {
             return fail(MC_TVD_EINVAL, "a 2-D problem has no y-sweep");
         }
@@ -183,7 +183,7 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
             A.chunk = pick_chunk(s, nz, xt * bt);
             grid = dim3((unsigned)xt, (unsigned)bt, (unsigned)((nz + A.chunk - 1) / A.chunk));
             smem = (size_t)4 * 3 * 32 * WB * sizeof(double);
-            mc::k_march<3, 2, 1><<<grid, block, smem, s->stream>>>(A);
+            { auto kfn = mc::k_march<3, 2, 1>; MC_LAUNCH(kfn, grid, block, smem, s->stream, A); }
         } else if (alpha == 1) {     // y-sweep: march y, tile (x, z)
             A.n_b = nz; A.s_b = (long long)nx * ny; A.wall_b = wl; A.inv2d_b = 1.0 / (2.0 * s->d[2]);
             A.n_m = ny; A.s_m = nx; A.wall_m = 0;
@@ -191,7 +191,7 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
             A.chunk = pick_chunk(s, ny, xt * bt);
             grid = dim3((unsigned)xt, (unsigned)bt, (unsigned)((ny + A.chunk - 1) / A.chunk));
             smem = (size_t)4 * 3 * 32 * WB * sizeof(double);
-            mc::k_march<3, 1, 2><<<grid, block, smem, s->stream>>>(A);
+            { auto kfn = mc::k_march<3, 1, 2>; MC_LAUNCH(kfn, grid, block, smem, s->stream, A); }
         } else {                     // x-sweep: lanes x, tile (x, y), march z
             A.n_b = ny; A.s_b = nx; A.wall_b = 0; A.inv2d_b = 1.0 / (2.0 * s->d[1]);
             A.n_m = nz; A.s_m = (long long)nx * ny; A.wall_m = wl; A.inv2d_m = 1.0 / (2.0 * s->d[2]);
@@ -199,7 +199,7 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
             A.chunk = pick_chunk(s, nz, xt * bt);
             grid = dim3((unsigned)xt, (unsigned)bt, (unsigned)((nz + A.chunk - 1) / A.chunk));
             smem = (size_t)4 * 2 * 32 * WB * sizeof(double);
-            mc::k_lane<3, 1, 2><<<grid, block, smem, s->stream>>>(A);
+            { auto kfn = mc::k_lane<3, 1, 2>; MC_LAUNCH(kfn, grid, block, smem, s->stream, A); }
         }
     }
     s->launches += 1;
@@ -217,6 +217,19 @@ mc::PointArgs point_args(const mc_tvd_state *s)
         P.inv_d[comp_of_axis(s->nd, a)] = 1.0 / s->d[a];
     }
     return P;
+}
+
+// Enqueue the max-speed reduction of the state in s->X and the dt it implies (R12).
+int enqueue_initial_dt(mc_tvd_state *s)
+{
+    mc::PointArgs P = point_args(s);
+    int blocks = (int)((s->N + 255) / 256);
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    if (s->nd == 2) { auto kfn = mc::k_max_speed<2>; MC_LAUNCH(kfn, blocks, 256, 0, s->stream, P, &s->S->smax_bits); }
+    else { auto kfn = mc::k_max_speed<3>; MC_LAUNCH(kfn, blocks, 256, 0, s->stream, P, &s->S->smax_bits); }
+    { auto kfn = mc::k_dt_update; MC_LAUNCH(kfn, 1, 32, 0, s->stream, s->S, 0); }
+    s->launches += 2;
+    return cuda_check(cudaGetLastError(), "initial dt launch");
 }
 
 }  // namespace
@@ -281,16 +294,7 @@ int mc_tvd_init(const mc_tvd_grid *grid, const mc_tvd_params *params, double *d_
     h.cfl = params->cfl; h.fixed_dt = params->fixed_dt;
     int rc = cuda_check(cudaMemcpyAsync(s->S, &h, sizeof(h), cudaMemcpyHostToDevice, s->stream), "scalar upload");
     if (rc == MC_TVD_OK) rc = cuda_check(cudaStreamSynchronize(s->stream), "scalar upload sync");   // h is on the stack
-    if (rc == MC_TVD_OK) {
-        mc::PointArgs P = point_args(s);
-        int blocks = (int)((s->N + 255) / 256);
-        if (blocks > 148 * 16) blocks = 148 * 16;
-        if (s->nd == 2) mc::k_max_speed<2><<<blocks, 256, 0, s->stream>>>(P, &s->S->smax_bits);
-        else mc::k_max_speed<3><<<blocks, 256, 0, s->stream>>>(P, &s->S->smax_bits);
-        mc::k_dt_update<<<1, 32, 0, s->stream>>>(s->S, 0);
-        s->launches += 2;
-        rc = cuda_check(cudaGetLastError(), "init launch");
-    }
+    if (rc == MC_TVD_OK) rc = enqueue_initial_dt(s);
     if (rc != MC_TVD_OK) { delete s; return rc; }
     *out = s;
     return MC_TVD_OK;
@@ -312,7 +316,7 @@ int mc_tvd_step(mc_tvd_state *s, int n_steps)
                 const double *t = src; src = dst; dst = (double *)t;
             }
         }
-        mc::k_dt_update<<<1, 32, 0, s->stream>>>(s->S, 1);
+        { auto kfn = mc::k_dt_update; MC_LAUNCH(kfn, 1, 32, 0, s->stream, s->S, 1); }
         s->launches += 1;
         int rc = cuda_check(cudaGetLastError(), "dt launch");
         if (rc != MC_TVD_OK) return rc;
@@ -328,6 +332,24 @@ int mc_tvd_sweep(mc_tvd_state *s, int alpha, int dir, double tau)
     if (rc != MC_TVD_OK) return rc;
     return cuda_check(cudaMemcpyAsync(s->X, s->Y, (size_t)s->nf * s->N * sizeof(double), cudaMemcpyDeviceToDevice,
                                       s->stream), "sweep copy-back");
+}
+
+int mc_tvd_step_host(mc_tvd_state *s, const double *h_in, double *h_out, int n_steps)
+{
+    if (!s || !h_in || !h_out || n_steps < 0) return fail(MC_TVD_EINVAL, "bad handle, host pointer or n_steps");
+    const size_t bytes = (size_t)s->nf * s->N * sizeof(double);
+    int rc = cuda_check(cudaMemcpyAsync(s->X, h_in, bytes, cudaMemcpyHostToDevice, s->stream), "state upload");
+    if (rc != MC_TVD_OK) return rc;
+    mc::Scalars h;
+    memset(&h, 0, sizeof(h));
+    h.cfl = s->par.cfl; h.fixed_dt = s->par.fixed_dt;
+    rc = cuda_check(cudaMemcpyAsync(s->S, &h, sizeof(h), cudaMemcpyHostToDevice, s->stream), "scalar upload");
+    if (rc == MC_TVD_OK) rc = cuda_check(cudaStreamSynchronize(s->stream), "upload sync");      // h is on the stack
+    if (rc == MC_TVD_OK) rc = enqueue_initial_dt(s);
+    if (rc == MC_TVD_OK) rc = mc_tvd_step(s, n_steps);
+    if (rc == MC_TVD_OK) rc = cuda_check(cudaMemcpyAsync(h_out, s->X, bytes, cudaMemcpyDeviceToHost, s->stream), "state download");
+    if (rc == MC_TVD_OK) rc = cuda_check(cudaStreamSynchronize(s->stream), "download sync");
+    return rc;
 }
 
 int mc_tvd_dt(mc_tvd_state *s, double *dt_host)
@@ -347,8 +369,8 @@ int mc_tvd_diagnostics(mc_tvd_state *s, mc_tvd_diag *out, double *T_prof, double
     static_assert(sizeof(mc_tvd_diag) == 19 * sizeof(double), "mc_tvd_diag layout");
     mc::PointArgs P = point_args(s);
     dim3 grid((unsigned)s->diag_blocks, (unsigned)s->grid.nz, 1);
-    if (s->nd == 2) mc::k_plane_partials<2><<<grid, mc::DIAG_THREADS, 0, s->stream>>>(P, s->partial, s->ext);
-    else mc::k_plane_partials<3><<<grid, mc::DIAG_THREADS, 0, s->stream>>>(P, s->partial, s->ext);
+    if (s->nd == 2) { auto kfn = mc::k_plane_partials<2>; MC_LAUNCH(kfn, grid, mc::DIAG_THREADS, 0, s->stream, P, s->partial, s->ext); }
+    else { auto kfn = mc::k_plane_partials<3>; MC_LAUNCH(kfn, grid, mc::DIAG_THREADS, 0, s->stream, P, s->partial, s->ext); }
     mc::DiagArgs G;
     memset(&G, 0, sizeof(G));
     G.partial = s->partial; G.ext = s->ext; G.plane_sums = s->plane_sums; G.out = s->diag_out; G.S = s->S;
@@ -356,7 +378,7 @@ int mc_tvd_diagnostics(mc_tvd_state *s, mc_tvd_diag *out, double *T_prof, double
     G.nplane = (double)s->grid.nx * (double)s->grid.ny;
     G.dz = s->d[2]; G.dxdy = s->d[0] * s->d[1];
     G.eps = s->par.eps; G.D = s->par.D; G.Ra = s->par.Ra; G.Pr = s->par.Pr;
-    mc::k_diag_finish<<<1, mc::DIAG_THREADS, 0, s->stream>>>(G);
+    { auto kfn = mc::k_diag_finish; MC_LAUNCH(kfn, 1, mc::DIAG_THREADS, 0, s->stream, G); }
     s->launches += 2;
     int rc = cuda_check(cudaGetLastError(), "diagnostics launch");
     if (rc != MC_TVD_OK) return rc;

@@ -36,22 +36,24 @@ MC_KERNEL void k_march(SweepArgs A)
     const int gx = (int)blockIdx.x * (Wx - 4) + tx - 2;
     const int ix = wrap(gx, A.nx);
     const int rx = min(tx, Wx - 1 - tx);
-    int gb = 0, rb = 99;
+    int gb = 0, rb = 99, gb_raw = 0;
     bool row_exists = true, wallrow = false;
     long long col = ix;
     if (HAS_B) {
         gb = (int)blockIdx.y * (Wb - 4) + ty - 2;
+        gb_raw = gb;
         rb = min(ty, Wb - 1 - ty);
         if (A.wall_b) {
             row_exists = (gb >= 0 && gb < A.n_b);
             wallrow = (gb == 0 || gb == A.n_b - 1);
             col += (long long)(row_exists ? gb : 0) * A.s_b;
         } else {
-            col += (long long)wrap(gb, A.n_b) * A.s_b;
+            gb = wrap(gb, A.n_b);                     // periodic b: the node's own index (z_k of Eq. 17)
+            col += (long long)gb * A.s_b;
         }
     }
     const bool needP = row_exists && !wallrow && rx >= 1 && rb >= 1 && (rx >= 2 || rb >= 2);
-    const bool owner = row_exists && rx >= 2 && rb >= 2 && gx < A.nx && (!HAS_B || gb < A.n_b);
+    const bool owner = row_exists && rx >= 2 && rb >= 2 && gx < A.nx && (!HAS_B || gb_raw < A.n_b);
 
     // ---- sweep constants ------------------------------------------------------------------
     const double tau = A.dt_ptr ? 0.5 * (*A.dt_ptr) : A.tau_fixed;

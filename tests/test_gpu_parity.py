@@ -1,0 +1,234 @@
+"""GPU parity: the CUDA path (through the C ABI, include/mc_tvd.h) against the CPU oracle, element by
+element on the same seeded inputs.  Tolerances (BASELINE.json north_star):
+field-max-normalised error <= 1e-12 after 1 step, <= 1e-9 after 100 steps, Nu within 1e-10 relative.
+"""
+from __future__ import annotations
+
+import numpy as np
+import pytest
+
+from paper_2411_10372_b200 import inputs
+from tests.helpers import rel_err
+
+pytestmark = pytest.mark.gpu
+
+TOL_SWEEP = 2e-13      # one operator L_alpha: a handful of roundings on O(1) fields
+TOL_1STEP = 1e-12
+TOL_100STEP = 1e-9
+TOL_NU = 1e-10
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    assert torch.cuda.is_available(), "these tests need a CUDA device"
+    from paper_2411_10372_b200 import binding
+    binding.load_library()
+    return binding
+
+
+def _solver(gpu, grid, params, X0):
+    return gpu.MCTVD(grid, params, X0)
+
+
+# ---- one operator L_alpha(tau) (Eqs. 31-39), every axis, both directions, both z boundaries ------
+SWEEP_GRIDS = [
+    (2, 300, 1, 70),      # 2-D: 3 march tiles (124 outputs) / 11 lane warps (28 outputs), ragged tails
+    (2, 29, 1, 5),        # smallest plate problem, one ragged tile
+    (3, 60, 21, 19),      # 3-D: 3 x-tiles, 3 b-tiles (8 outputs) with ragged tails, walls in b for Ly
+    (3, 30, 9, 33),       # ragged the other way
+]
+
+
+@pytest.mark.parametrize("ndim,nx,ny,nz", SWEEP_GRIDS)
+@pytest.mark.parametrize("bc_z", [0, 1])
+@pytest.mark.parametrize("tvd_form", [0, 1])
+def test_sweep_parity(gpu, orc, ndim, nx, ny, nz, bc_z, tvd_form):
+    grid = inputs.make_grid(ndim, nx, nz, ny)
+    params = inputs.make_params(Ra=1e4, bc_z=bc_z, tvd_form=tvd_form)
+    X0 = inputs.smooth_random_state(grid, params, seed=11 + nx + bc_z)
+    prob = orc.Problem(grid, params)
+    tau = 0.25 * orc.dt(prob, X0)
+    for alpha in ((0, 2) if ndim == 2 else (0, 1, 2)):
+        for direction in (1, -1):
+            ref = orc.sweep(prob, X0, alpha, tau, direction)
+            s = _solver(gpu, grid, params, X0)
+            s.sweep(alpha, direction, tau)
+            err = rel_err(s.state(), ref).max()
+            s.close()
+            assert err <= TOL_SWEEP, (alpha, direction, err)
+
+
+@pytest.mark.parametrize("ndim,nx,ny,nz", [(2, 300, 1, 70), (3, 60, 21, 19)])
+@pytest.mark.parametrize("chunk", [7, 16])
+def test_sweep_parity_chunked(gpu, orc, monkeypatch, ndim, nx, ny, nz, chunk):
+    """Blocks that start in the middle of the marching direction (4-level warm-up)."""
+    monkeypatch.setenv("MC_TVD_CHUNK", str(chunk))
+    grid = inputs.make_grid(ndim, nx, nz, ny)
+    params = inputs.make_params(Ra=1e4)
+    X0 = inputs.smooth_random_state(grid, params, seed=5)
+    prob = orc.Problem(grid, params)
+    tau = 0.25 * orc.dt(prob, X0)
+    for alpha in ((0, 2) if ndim == 2 else (0, 1, 2)):
+        for direction in (1, -1):
+            ref = orc.sweep(prob, X0, alpha, tau, direction)
+            s = _solver(gpu, grid, params, X0)
+            s.sweep(alpha, direction, tau)
+            err = rel_err(s.state(), ref).max()
+            s.close()
+            assert err <= TOL_SWEEP, (alpha, direction, err)
+
+
+def test_tvd_off_and_paper_direction(gpu, orc):
+    grid = inputs.make_grid(3, 40, 13, 12)
+    for over in (dict(tvd_off=1), dict(dir_mode=0), dict(lambda_coef=2.0 / 3.0)):
+        params = inputs.make_params(Ra=1e3, **over)
+        X0 = inputs.smooth_random_state(grid, params, seed=3)
+        prob = orc.Problem(grid, params)
+        ref, dts, _ = orc.step(prob, X0, 1)
+        s = _solver(gpu, grid, params, X0)
+        s.step(1)
+        assert rel_err(s.state(), ref).max() <= TOL_1STEP, over
+        s.close()
+
+
+# ---- config C1 (BASELINE.json configs[0]): 1 step, 100 steps, dt, Nu ------------------------------
+@pytest.fixture(scope="module")
+def c1(orc):
+    grid, params, steps = inputs.config("C1")
+    X0 = inputs.conduction_state(grid, params)
+    prob = orc.Problem(grid, params)
+    ref1, dts1, _ = orc.step(prob, X0, 1)
+    ref100, dts100, t100 = orc.step(prob, X0, steps)
+    return dict(grid=grid, params=params, steps=steps, X0=X0, prob=prob, ref1=ref1, ref100=ref100,
+                dts=dts100, t100=t100)
+
+
+def test_c1_one_step(gpu, orc, c1):
+    s = _solver(gpu, c1["grid"], c1["params"], c1["X0"])
+    dt0 = s.dt()
+    assert abs(dt0 - c1["dts"][0]) <= 4e-16 * dt0
+    s.step(1)
+    assert rel_err(s.state(), c1["ref1"]).max() <= TOL_1STEP
+    s.close()
+
+
+def test_c1_100_steps_and_diagnostics(gpu, orc, c1):
+    s = _solver(gpu, c1["grid"], c1["params"], c1["X0"])
+    s.step(c1["steps"])
+    X = s.state()
+    assert rel_err(X, c1["ref100"]).max() <= TOL_100STEP
+    d, Tp, rp, pp = s.diagnostics()
+    assert d["step"] == c1["steps"]
+    assert abs(d["time"] - c1["t100"]) <= 1e-9 * c1["t100"]
+    # Nu on an IDENTICAL state (the downloaded GPU state): tolerance 1e-10 relative
+    do, To, ro, po = orc.diagnostics(c1["prob"], X)
+    for k in ("nu_bottom", "nu_top", "nu_bar", "nu_bulk"):
+        assert abs(d[k] - do[k]) <= TOL_NU * abs(do[k]), (k, d[k], do[k])
+    for k in ("re", "u_rms", "mass", "energy", "max_mach", "min_rho", "min_T"):
+        assert abs(d[k] - do[k]) <= 1e-12 * max(abs(do[k]), 1e-30), (k, d[k], do[k])
+    for k in ("nu_conv", "nu_K", "mom_x", "mom_z"):          # sums that cancel: absolute on their scale
+        scale = {"nu_conv": 1.0, "nu_K": 1.0, "mom_x": do["mass"], "mom_z": do["mass"]}[k]
+        assert abs(d[k] - do[k]) <= 1e-10 * scale, (k, d[k], do[k])
+    np.testing.assert_allclose(Tp, To, rtol=1e-13)
+    np.testing.assert_allclose(rp, ro, rtol=1e-13)
+    np.testing.assert_allclose(pp, po, rtol=1e-13)
+    assert abs(d["dt"] - orc.dt(c1["prob"], X)) <= 4e-16 * d["dt"]
+    # end to end: Nu of the GPU run against Nu of the oracle run
+    dref, *_ = orc.diagnostics(c1["prob"], c1["ref100"])
+    assert abs(d["nu_bar"] - dref["nu_bar"]) <= 1e-7 * abs(dref["nu_bar"])
+    s.close()
+
+
+def test_step_host_matches_step(gpu, orc, c1):
+    import torch
+    s = _solver(gpu, c1["grid"], c1["params"], c1["X0"])
+    s.step(3)
+    a = s.state().copy()
+    hin = torch.from_numpy(c1["X0"].reshape(-1).copy()).pin_memory()
+    hout = torch.empty_like(hin).pin_memory()
+    s.step_host(hin, hout, 3)
+    assert np.array_equal(hout.numpy().reshape(a.shape), a)      # same kernels, same order: bit-equal
+    s.close()
+
+
+def test_3d_steps(gpu, orc):
+    """A 3-D box with plates, 3 full steps of Eq. 30 (18 sweeps), CFL dt from the fused reduction."""
+    grid = inputs.make_grid(3, 64, 20, 24)
+    params = inputs.make_params(Ra=1e5)
+    X0 = inputs.conduction_state(grid, params, amplitude=1e-2)
+    prob = orc.Problem(grid, params)
+    ref, dts, t = orc.step(prob, X0, 3)
+    s = _solver(gpu, grid, params, X0)
+    s.step(1)
+    ref1, _, _ = orc.step(prob, X0, 1)
+    assert rel_err(s.state(), ref1).max() <= TOL_1STEP
+    s.step(2)
+    assert rel_err(s.state(), ref).max() <= 3 * TOL_1STEP
+    d, *_ = s.diagnostics()
+    assert abs(d["time"] - t) <= 1e-12 * t
+    do, *_ = orc.diagnostics(prob, s.state())
+    assert abs(d["nu_bar"] - do["nu_bar"]) <= TOL_NU * abs(do["nu_bar"])
+    s.close()
+
+
+# ---- properties that hold at any size --------------------------------------------------------------
+def test_uniform_state_is_a_fixed_point(gpu):
+    """Every flux difference and dX is exactly zero: the state must not change in a single bit."""
+    from tests.helpers import ideal_gas_params, state_from_primitives
+    for ndim, nx, ny, nz in [(2, 130, 1, 40), (3, 60, 12, 10)]:
+        grid = inputs.make_grid(ndim, nx, nz, ny)
+        params = ideal_gas_params(mu_override=1e-2, K_override=1e-2)
+        X0 = state_from_primitives(grid, params, 1.3, 0.4, 0.0 if ndim == 2 else -0.2, 0.1, 0.9)
+        s = _solver(gpu, grid, params, X0)
+        s.step(5)
+        assert np.array_equal(s.state(), X0)
+        s.close()
+
+
+def test_mass_conserved_with_plates(gpu):
+    grid, params, _ = inputs.config("C1")
+    X0 = inputs.conduction_state(grid, params, amplitude=1e-2)
+    s = _solver(gpu, grid, params, X0)
+    m0 = s.diagnostics()[0]["mass"]
+    s.step(50)
+    m1 = s.diagnostics()[0]["mass"]
+    assert abs(m1 - m0) <= 1e-12 * abs(m0)
+    s.close()
+
+
+# ---- error behaviour of the C ABI -------------------------------------------------------------------
+def test_nonfinite_state_is_reported(gpu):
+    grid = inputs.make_grid(2, 64, 16)
+    params = inputs.make_params()
+    X0 = inputs.conduction_state(grid, params)
+    bad = X0.copy()
+    bad[0, 37] = -1.0                      # non-positive rho
+    s = _solver(gpu, grid, params, bad)
+    with pytest.raises(gpu.MCTVDError) as e:
+        s.dt()
+    assert e.value.code == -4
+    s.close()
+    bad = X0.copy()
+    bad[3, 100] = np.nan
+    s = _solver(gpu, grid, params, bad)
+    with pytest.raises(gpu.MCTVDError) as e:
+        s.dt()
+    assert e.value.code == -4
+    s.close()
+
+
+def test_workspace_too_small(gpu):
+    import ctypes as C
+    import torch
+    lib = gpu.load_library()
+    grid = inputs.make_grid(2, 64, 16)
+    g, p = gpu.make_grid(grid), gpu.make_params(inputs.make_params())
+    wb = lib.mc_tvd_workspace_bytes(C.byref(g), C.byref(p))
+    f = torch.zeros(4 * 64 * 16, dtype=torch.float64, device="cuda")
+    w = torch.zeros(wb // 8, dtype=torch.float64, device="cuda")
+    h = C.c_void_p()
+    rc = lib.mc_tvd_init(C.byref(g), C.byref(p), f.data_ptr(), w.data_ptr(), wb - 8, None, C.byref(h))
+    assert rc == -3 and not h.value
+    rc = lib.mc_tvd_init(C.byref(g), C.byref(p), f.data_ptr() + 8, w.data_ptr(), wb, None, C.byref(h))
+    assert rc == -1 and not h.value
