@@ -1,0 +1,336 @@
+"""bench.py -- throughput of the MacCormack-TVD step (Eqs. 30-39) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C5|C3|C4|C2|C1] [--impl ours|reference]
+
+One "step" is one pass of the whole hot path over the whole grid: the CFL time step (fused max-reduction
++ dt kernel) and the 4 (2-D) or 6 (3-D) operators L_z L_y L_x L_z L_y L_x, each predictor + boundary
+values + corrector + TVD term + average in one kernel.  Metric (BASELINE.json): cell-updates/s, with the
+achieved HBM bandwidth of the dominant kernel as a fraction of the measured copy bandwidth.
+
+Default workload: BASELINE config C5 (3-D 1024x1024x256, 268M cells, 10.7 GB per state), the largest
+3-D case and the one the north-star roofline claim is made on; --workload C3 is the largest 2-D case.
+Both are far larger than the 126 MB L2, so no L2 flush is needed between steps.
+
+Prints ONE JSON line (rank 0).  N > 1 (torchrun): one independent replica of the workload per GPU
+(the north-star path is single-GPU; replicas only), weak scaling, no collective
+on the data path; time = max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+from paper_2411_10372_b200 import inputs  # noqa: E402
+
+METRIC = "cell-updates/sec per MacCormack-TVD step (achieved HBM GB/s as fraction of roofline in `roofline`)"
+UNIT = "cell-updates/s"
+ORACLE_RATE_EST = 2.5e5          # cell-updates/s of the single-thread oracle, used only to SIZE its sample
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="C5", choices=sorted(inputs.CONFIGS))
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    return ap.parse_args()
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md, MEASURED_PEAKS.json absent)"
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons of one GPU every 100 ms while the timed region runs."""
+
+    def __init__(self, index: int):
+        self.index, self.samples, self.reasons, self.max_mhz = index, [], set(), None
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self.nv = None
+
+    def _run(self):
+        nv = self.nv
+        names = {"hw_slowdown": 0x8, "sw_thermal_slowdown": 0x20, "hw_thermal_slowdown": 0x40,
+                 "sw_power_cap": 0x4, "hw_power_brake_slowdown": 0x80, "sync_boost": 0x10}
+        while not self._stop.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                r = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                for n, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(n)
+            except Exception:
+                pass
+            self._stop.wait(0.1)
+
+    def __enter__(self):
+        if self.nv is not None:
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._thr is not None:
+            self._thr.join()
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["unavailable"]}
+        return {"sm_mhz": int(np.median(self.samples)), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+# ---------------------------------------------------------------------------------------------------
+# the CPU oracle on a bounded sample of the workload (cpu_baseline leg and --impl reference)
+# ---------------------------------------------------------------------------------------------------
+def oracle_sample(name: str, target_cells: float):
+    """A full-height window of the workload's seeded initial state holding about target_cells nodes:
+    the first w columns (2-D) or w x w columns (3-D), treated as a periodic box of the same spacing."""
+    grid, params, _ = inputs.config(name)
+    nz = grid["nz"]
+    if grid["ndim"] == 2:
+        w = int(min(grid["nx"], max(16, round(target_cells / nz / 8) * 8)))
+        gw = dict(grid, nx=w, lx=grid["lx"] * w / grid["nx"])
+        desc = f"{name} periodic window {w}x{nz} (same spacing, recipe and seed; full height)"
+    else:
+        w = int(min(grid["nx"], grid["ny"], max(16, round((target_cells / nz) ** 0.5 / 8) * 8)))
+        gw = dict(grid, nx=w, ny=w, lx=grid["lx"] * w / grid["nx"], ly=grid["ly"] * w / grid["ny"])
+        desc = f"{name} periodic window {w}x{w}x{nz} (same spacing, recipe and seed; full height)"
+    X = inputs.conduction_state(gw, params)      # same recipe, same seed; window of the same spacing
+    return gw, params, X, desc
+
+
+def time_oracle(name: str, steps: int, warmup: int, target_cells: float):
+    """Times the oracle, as it stands (single thread), step by step.  Returns (cells/s, s/step, desc)."""
+    import oracle
+    oracle.build()
+    gw, params, X, desc = oracle_sample(name, target_cells)
+    prob = oracle.Problem(gw, params)
+    cells = inputs.num_nodes(gw)
+    for _ in range(warmup):
+        X, _, _ = oracle.step(prob, X, 1)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        X, _, _ = oracle.step(prob, X, 1)
+    el = time.perf_counter() - t0
+    assert np.all(np.isfinite(X))
+    return cells * steps / el, el / steps, desc, cells
+
+
+def run_reference(args):
+    """--impl reference: the oracle (kind "oracle", one host core) on this arm's config and metric."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    name = args.workload
+    total = max(1, args.steps + args.warmup)
+    target = max(2.0e4, ORACLE_RATE_EST * 90.0 / total)       # whole run ~1.5 minutes
+    value, s_per_step, desc, cells = time_oracle(name, args.steps, args.warmup, target)
+    grid, params, _ = inputs.config(name)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": s_per_step * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic (seeded hydrostatic conduction state + T noise, DESIGN.md input recipe)",
+        "config": workload_config(name, grid, params),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle",
+                         "sample": f"{desc}; {args.steps} timed steps of {cells} cells after {args.warmup} warm-up"},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def workload_config(name, grid, params):
+    dims = f"{grid['nx']}x{grid['nz']}" if grid["ndim"] == 2 else f"{grid['nx']}x{grid['ny']}x{grid['nz']}"
+    return {"workload": f"{name}: {grid['ndim']}-D {dims} fp64, gamma=5/3, Pr=1, Ra={params['Ra']:g}, eps=0.1, D=0.4, CFL 0.5",
+            "cells": inputs.num_nodes(grid), "fields": inputs.num_fields(grid),
+            "operators_per_step": 4 if grid["ndim"] == 2 else 6,
+            "l2": "state (>= 2 GB) far larger than the 126 MB L2; no flush needed" if inputs.num_nodes(grid) > 3e7
+                  else "state comparable to L2: cache-resident case, not a roofline claim",
+            "seed": inputs.SEED}
+
+
+# ---------------------------------------------------------------------------------------------------
+# our arm: the CUDA path through the C ABI
+# ---------------------------------------------------------------------------------------------------
+KERNEL_NAMES = {"Lx+": "k_lane (L_x, dir +1)", "Lx-": "k_lane (L_x, dir -1)",
+                "Ly+": "k_march (L_y, dir +1)", "Ly-": "k_march (L_y, dir -1)",
+                "Lz+": "k_march (L_z, dir +1)", "Lz-": "k_march (L_z, dir -1)"}
+
+
+def ncu_traffic(name: str, kernel_key: str):
+    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full summary, or None."""
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    if not os.path.exists(path):
+        return None
+    try:
+        with open(path) as f:
+            return json.load(f).get(name, {}).get(kernel_key[:2])
+    except Exception:
+        return None
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (sm_100a); there is no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    from paper_2411_10372_b200 import binding
+    name = args.workload
+    grid, params, _ = inputs.config(name)
+    nf, N = inputs.num_fields(grid), inputs.num_nodes(grid)
+    state_bytes = nf * N * 8
+    X0 = inputs.conduction_state(grid, params)                       # host, seeded (identical on every rank)
+    h_in = torch.from_numpy(X0.reshape(-1))
+    del X0
+    try:
+        h_in = h_in.pin_memory()
+        h_out = torch.empty_like(h_in).pin_memory()
+        pinned = True
+    except Exception:
+        h_out = torch.empty_like(h_in)
+        pinned = False
+    solver = binding.MCTVD(grid, params, h_in, device=f"cuda:{local}")
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident throughput: W warm-up steps, then exactly K timed steps ------------------
+    solver.step(args.warmup)
+    barrier()
+    l0 = solver.launch_count()
+    solver.timing_enable(True)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local) as clocks:
+        barrier()
+        e0.record(solver.stream)
+        solver.step(args.steps)
+        e1.record(solver.stream)
+        barrier()
+    ms = e0.elapsed_time(e1)
+    launches = solver.launch_count() - l0
+    per_kernel = solver.timing_read()
+    solver.timing_enable(False)
+    dt_now = solver.dt()                                             # raises if the state went non-finite
+    diag, *_ = solver.diagnostics()
+
+    t = torch.tensor([ms], dtype=torch.float64, device=f"cuda:{local}")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_max = float(t.item())
+    value = world * N * args.steps / (ms_max * 1e-3)
+
+    # ---- end to end through the public host-buffer call (H2D + steps + D2H inside the timed region) --
+    e2e = None
+    if not args.no_e2e:
+        n_e2e = max(1, args.e2e_steps)
+        solver.step_host(h_in, h_out, 1)                             # warm-up of the copy path
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            solver.step_host(h_in, h_out, 1)                         # synchronises internally
+        barrier()
+        el = time.perf_counter() - t0
+        te = torch.tensor([el], dtype=torch.float64, device=f"cuda:{local}")
+        if world > 1:
+            dist.all_reduce(te, op=dist.ReduceOp.MAX)
+        e2e = {"value": world * N * n_e2e / float(te.item()), "unit": UNIT,
+               "h2d_bytes_per_step": state_bytes, "d2h_bytes_per_step": state_bytes,
+               "steps": n_e2e, "ms_per_step": float(te.item()) / n_e2e * 1e3,
+               "call": "mc_tvd_step_host(h_in, h_out, 1): H2D of the state, dt reduction, 1 step, D2H of the state",
+               "host_memory": "pinned" if pinned else "pageable"}
+    solver.close()
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel ------------------------------------------------------------
+    peak, peak_src = measured_peaks()
+    alg_bytes = 2 * nf * 8 * N                                       # read nf + write nf doubles per node per operator
+    dom = max(per_kernel, key=lambda k: per_kernel[k][0])
+    dom_ms = per_kernel[dom][0] / per_kernel[dom][1]
+    achieved = alg_bytes / (dom_ms * 1e-3) / 1e9
+    kernels = {KERNEL_NAMES[k]: {"avg_ms": v[0] / v[1], "launches": v[1], "share_of_step": v[0] / ms,
+                                 "achieved_GBps": alg_bytes / (v[0] / v[1] * 1e-3) / 1e9}
+               for k, v in per_kernel.items()}
+    step_gbps = (4 if grid["ndim"] == 2 else 6) * alg_bytes * args.steps / (ms * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": KERNEL_NAMES[dom], "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": ncu_traffic(name, dom), "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": alg_bytes,
+                "algorithmic_bytes_per_cell_per_operator": 2 * nf * 8,
+                "whole_step_achieved_GBps": step_gbps, "whole_step_frac": step_gbps / peak,
+                "kernels": kernels}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic (seeded hydrostatic conduction state + T noise, DESIGN.md input recipe)",
+        "config": workload_config(name, grid, params),
+        "clocks": clocks.summary(), "gpu_launches": int(launches),
+        "roofline": roofline,
+        "state_check": {"dt": dt_now, "nu_bar": diag["nu_bar"], "min_rho": diag["min_rho"], "min_T": diag["min_T"],
+                        "steps_taken": diag["step"]},
+    }
+    if e2e is not None:
+        line["e2e"] = e2e
+    if world == 1 and not args.no_cpu_baseline:
+        target = ORACLE_RATE_EST * 8.0                                # ~8 s per oracle step, 1 warm-up + 2 timed
+        v, s_per_step, desc, cells = time_oracle(name, 2, 1, target)
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                "sample": f"{desc}; 2 timed steps of {cells} cells after 1 warm-up, {s_per_step:.1f} s/step"}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

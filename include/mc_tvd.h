@@ -118,6 +118,16 @@ int mc_tvd_diagnostics(mc_tvd_state *s, mc_tvd_diag *out, double *T_prof, double
 /* Number of kernel launches this handle has enqueued so far (for bench.py's gpu_launches). */
 long long mc_tvd_launch_count(const mc_tvd_state *s);
 
+/* Per-kernel device timing (for the roofline figure of bench.py).  enable = 1: every
+ * operator launch of later mc_tvd_step / mc_tvd_step_host calls is bracketed by CUDA events on the
+ * handle's stream (at most MC_TVD_MAX_TIMED launches are recorded, later ones run untimed);
+ * enable = 0 stops recording.  mc_tvd_timing_read synchronises the stream, adds the recorded
+ * durations into ms_sum[6] and count[6] (HOST arrays, overwritten), indexed by
+ * kind = alpha + (dir < 0 ? 3 : 0) with alpha = 0,1,2 for L_x, L_y, L_z, and clears the records. */
+#define MC_TVD_MAX_TIMED 4096
+int mc_tvd_timing_enable(mc_tvd_state *s, int enable);
+int mc_tvd_timing_read(mc_tvd_state *s, double *ms_sum, long long *count);
+
 /* Free the handle (host memory only).  Synchronises the stream first. */
 int mc_tvd_destroy(mc_tvd_state *s);
 

@@ -51,6 +51,8 @@ SYMBOLS = {
     "mc_tvd_dt": (C.c_int, [C.c_void_p, _DP]),
     "mc_tvd_diagnostics": (C.c_int, [C.c_void_p, C.POINTER(Diag), _DP, _DP, _DP]),
     "mc_tvd_launch_count": (C.c_longlong, [C.c_void_p]),
+    "mc_tvd_timing_enable": (C.c_int, [C.c_void_p, C.c_int]),
+    "mc_tvd_timing_read": (C.c_int, [C.c_void_p, _DP, C.POINTER(C.c_longlong)]),
     "mc_tvd_destroy": (C.c_int, [C.c_void_p]),
     "mc_tvd_last_error": (C.c_char_p, []),
 }
@@ -183,6 +185,17 @@ class MCTVD:
 
     def launch_count(self) -> int:
         return int(self.lib.mc_tvd_launch_count(self._h))
+
+    def timing_enable(self, enable: bool = True):
+        self._check(self.lib.mc_tvd_timing_enable(self._h, int(bool(enable))))
+
+    def timing_read(self):
+        """{kernel name: (ms_sum, count)} of the operator launches recorded since the last read."""
+        ms = (C.c_double * 6)()
+        cnt = (C.c_longlong * 6)()
+        self._check(self.lib.mc_tvd_timing_read(self._h, ms, cnt))
+        names = ["Lx+", "Ly+", "Lz+", "Lx-", "Ly-", "Lz-"]
+        return {names[k]: (ms[k], int(cnt[k])) for k in range(6) if cnt[k]}
 
     def state(self) -> np.ndarray:
         """Download the current state as numpy (nf, N).  Synchronises."""

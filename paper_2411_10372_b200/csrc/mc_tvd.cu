@@ -54,6 +54,13 @@ struct mc_tvd_state {
     cudaStream_t stream;
     long long launches;
     int chunk_override;
+    // per-kernel timing (mc_tvd_timing_*): events ev[0..n_ev) recorded around operator launches;
+    // launch r ran between ev_pair[r] and ev_pair[r] + 1
+    bool timing;
+    cudaEvent_t *ev;
+    int n_ev, n_rec;
+    int *rec_kind, *rec_ev;
+    bool ev_open;                      // the last recorded event directly precedes the next launch
 };
 
 namespace {
@@ -148,6 +155,9 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
     mc::SweepArgs A;
     fill_common(s, A, in, out, alpha, dir, tau, use_dt, reduce);
     const int nx = s->grid.nx, ny = s->grid.ny, nz = s->grid.nz;
+    const bool timed = s->timing && s->n_rec < MC_TVD_MAX_TIMED;
+    if (timed && !s->ev_open) { cudaEventRecord(s->ev[s->n_ev], s->stream); s->n_ev += 1; }
+    s->ev_open = timed;                // the closing event of this launch opens the next one
     const int wl = s->walls ? 1 : 0;
     dim3 block, grid;
     size_t smem = 0;
@@ -203,7 +213,14 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
         }
     }
     s->launches += 1;
-    return cuda_check(cudaGetLastError(), "sweep launch");
+    int rc = cuda_check(cudaGetLastError(), "sweep launch");
+    if (rc == MC_TVD_OK && timed) {
+        cudaEventRecord(s->ev[s->n_ev], s->stream);
+        s->rec_kind[s->n_rec] = alpha + (dir < 0 ? 3 : 0);
+        s->rec_ev[s->n_rec] = s->n_ev - 1;
+        s->n_rec += 1; s->n_ev += 1;
+    }
+    return rc;
 }
 
 mc::PointArgs point_args(const mc_tvd_state *s)
@@ -318,6 +335,7 @@ int mc_tvd_step(mc_tvd_state *s, int n_steps)
         }
         { auto kfn = mc::k_dt_update; MC_LAUNCH(kfn, 1, 32, 0, s->stream, s->S, 1); }
         s->launches += 1;
+        s->ev_open = false;
         int rc = cuda_check(cudaGetLastError(), "dt launch");
         if (rc != MC_TVD_OK) return rc;
     }
@@ -400,10 +418,48 @@ int mc_tvd_diagnostics(mc_tvd_state *s, mc_tvd_diag *out, double *T_prof, double
 
 long long mc_tvd_launch_count(const mc_tvd_state *s) { return s ? s->launches : 0; }
 
+int mc_tvd_timing_enable(mc_tvd_state *s, int enable)
+{
+    if (!s) return fail(MC_TVD_EINVAL, "bad handle");
+    if (enable && !s->ev) {
+        const int cap = 2 * MC_TVD_MAX_TIMED + 2;
+        s->ev = (cudaEvent_t *)calloc(cap, sizeof(cudaEvent_t));
+        s->rec_kind = (int *)calloc(MC_TVD_MAX_TIMED, sizeof(int));
+        s->rec_ev = (int *)calloc(MC_TVD_MAX_TIMED, sizeof(int));
+        if (!s->ev || !s->rec_kind || !s->rec_ev) return fail(MC_TVD_ENOMEM, "host allocation failed");
+        for (int i = 0; i < cap; ++i) {
+            int rc = cuda_check(cudaEventCreate(&s->ev[i]), "event create");
+            if (rc != MC_TVD_OK) return rc;
+        }
+    }
+    s->timing = enable != 0;
+    s->ev_open = false;
+    return MC_TVD_OK;
+}
+
+int mc_tvd_timing_read(mc_tvd_state *s, double *ms_sum, long long *count)
+{
+    if (!s || !ms_sum || !count) return fail(MC_TVD_EINVAL, "bad handle or output pointer");
+    for (int k = 0; k < 6; ++k) { ms_sum[k] = 0.0; count[k] = 0; }
+    int rc = cuda_check(cudaStreamSynchronize(s->stream), "timing sync");
+    if (rc != MC_TVD_OK) return rc;
+    for (int r = 0; r < s->n_rec; ++r) {
+        float ms = 0.f;
+        rc = cuda_check(cudaEventElapsedTime(&ms, s->ev[s->rec_ev[r]], s->ev[s->rec_ev[r] + 1]), "event elapsed");
+        if (rc != MC_TVD_OK) return rc;
+        ms_sum[s->rec_kind[r]] += (double)ms;
+        count[s->rec_kind[r]] += 1;
+    }
+    s->n_rec = 0; s->n_ev = 0; s->ev_open = false;
+    return MC_TVD_OK;
+}
+
 int mc_tvd_destroy(mc_tvd_state *s)
 {
     if (!s) return MC_TVD_OK;
     cudaError_t e = cudaStreamSynchronize(s->stream);
+    if (s->ev) for (int i = 0; i < 2 * MC_TVD_MAX_TIMED + 2; ++i) if (s->ev[i]) cudaEventDestroy(s->ev[i]);
+    free(s->ev); free(s->rec_kind); free(s->rec_ev);
     delete s;
     return cuda_check(e, "destroy sync");
 }
