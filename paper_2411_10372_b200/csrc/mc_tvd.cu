@@ -9,6 +9,7 @@
 #include <stdlib.h>
 #include <string.h>
 #include <new>
+#include <type_traits>
 
 #include "mc_common.cuh"
 #include "reduce_kernels.cuh"
@@ -124,17 +125,21 @@ void fill_common(const mc_tvd_state *s, mc::SweepArgs &A, const double *in, doub
     A.N = s->N; A.nx = s->grid.nx;
     A.dir = dir;
     A.src = (alpha == 2);
-    A.tvd_form = s->par.tvd_form; A.tvd_off = s->par.tvd_off;
     A.reduce = reduce ? 1 : 0;
     A.d_a = s->d[alpha];
-    A.inv2d_x = 1.0 / (2.0 * s->d[0]);
+    A.inv_h = (dir > 0 ? 1.0 : -1.0) / s->d[alpha];
+    const double mu = s->mu, lam = s->par.lambda_coef;
+    A.mu_h = mu * A.inv_h; A.two_mu_h = 2.0 * mu * A.inv_h; A.lam_mu_h = lam * mu * A.inv_h; A.K_h = s->K * A.inv_h;
     for (int a = 0; a < 3; ++a) {
         if (s->nd == 2 && a == 1) continue;
-        A.inv_d[comp_of_axis(s->nd, a)] = 1.0 / s->d[a];
+        const int c = comp_of_axis(s->nd, a);
+        A.inv_d[c] = 1.0 / s->d[a];
+        A.mu_2c[c] = mu / (2.0 * s->d[a]);
+        A.lam_mu_2c[c] = lam * mu / (2.0 * s->d[a]);
     }
     A.dz = s->d[2];
-    A.R = s->R; A.cv = s->cv; A.icv = s->icv; A.g = s->g; A.mu = s->mu; A.K = s->K;
-    A.lam = s->par.lambda_coef; A.gamma = s->par.gamma;
+    A.R = s->R; A.cv = s->cv; A.icv = s->icv; A.g = s->g;
+    A.gamma = s->par.gamma; A.gammaR = s->par.gamma * s->R;
     A.Tw0 = s->par.T_bot; A.Tw1 = s->par.T_top;
     A.nz = s->grid.nz;
 }
@@ -148,6 +153,24 @@ int pick_chunk(const mc_tvd_state *s, int n_m, long long tiles)
     return chunk;
 }
 
+// compile-time dispatch of the kernels' switches
+template <class F> void with_bool(bool b, F f)
+{
+    if (b) f(std::true_type()); else f(std::false_type());
+}
+template <class F> void with_tvd(const mc_tvd_state *s, F f)
+{
+    if (s->par.tvd_off) f(std::integral_constant<int, -1>());
+    else if (s->par.tvd_form == 0) f(std::integral_constant<int, 0>());
+    else f(std::integral_constant<int, 1>());
+}
+
+template <class K> int launch_kernel(K kfn, dim3 grid, dim3 block, size_t smem, cudaStream_t st, const mc::SweepArgs &A)
+{
+    MC_LAUNCH(kfn, grid, block, smem, st, A);
+    return 0;
+}
+
 // Enqueue one operator L_alpha(tau): in -> out.
 int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int dir, double tau, bool use_dt,
                  bool reduce)
@@ -158,58 +181,63 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
     const bool timed = s->timing && s->n_rec < MC_TVD_MAX_TIMED;
     if (timed && !s->ev_open) { cudaEventRecord(s->ev[s->n_ev], s->stream); s->n_ev += 1; }
     s->ev_open = timed;                // the closing event of this launch opens the next one
-    const int wl = s->walls ? 1 : 0;
-    dim3 block, grid;
-    size_t smem = 0;
+    const bool wl = s->walls;
+    cudaStream_t st = s->stream;
     if (s->nd == 2) {
         if (alpha == 2) {            // z-sweep: march z, tile x
-            A.n_b = 1; A.s_b = 0; A.n_m = nz; A.s_m = nx; A.wall_m = wl; A.wall_b = 0;
-            block = dim3(MARCH_WX_2D, 1, 1);
-            long long tiles = (nx + MARCH_WX_2D - 5) / (MARCH_WX_2D - 4);
+            constexpr int WX = MARCH_WX_2D;
+            A.n_b = 1; A.s_b = 0; A.n_m = nz; A.s_m = nx;
+            long long tiles = (nx + WX - 5) / (WX - 4);
             A.chunk = pick_chunk(s, nz, tiles);
-            grid = dim3((unsigned)tiles, 1, (unsigned)((nz + A.chunk - 1) / A.chunk));
-            smem = (size_t)4 * 2 * MARCH_WX_2D * sizeof(double);
-            { auto kfn = mc::k_march<2, 1, -1>; MC_LAUNCH(kfn, grid, block, smem, s->stream, A); }
+            dim3 block(WX, 1, 1), grid((unsigned)tiles, 1, (unsigned)((nz + A.chunk - 1) / A.chunk));
+            size_t smem = ((size_t)4 * 2 * WX + 4) * sizeof(double);
+            with_bool(wl, [&](auto W) { with_tvd(s, [&](auto T) {
+                launch_kernel(mc::k_march<2, 1, -1, WX, 1, decltype(W)::value, false, decltype(T)::value>, grid, block, smem, st, A);
+            }); });
         } else if (alpha == 0) {     // x-sweep: lanes x, march z
-            A.n_b = 1; A.s_b = 0; A.n_m = nz; A.s_m = nx; A.wall_m = wl; A.wall_b = 0;
-            A.inv2d_m = 1.0 / (2.0 * s->d[2]);
-            block = dim3(32, LANE_WARPS_2D, 1);
+            constexpr int LW = LANE_WARPS_2D;
+            A.n_b = 1; A.s_b = 0; A.n_m = nz; A.s_m = nx;
             long long xt = (nx + mc::LANE_OUT - 1) / mc::LANE_OUT;
-            long long tiles = (xt + LANE_WARPS_2D - 1) / LANE_WARPS_2D;
+            long long tiles = (xt + LW - 1) / LW;
             A.chunk = pick_chunk(s, nz, tiles);
-            grid = dim3((unsigned)tiles, 1, (unsigned)((nz + A.chunk - 1) / A.chunk));
-            { auto kfn = mc::k_lane<2, -1, 1>; MC_LAUNCH(kfn, grid, block, 0, s->stream, A); }
+            dim3 block(32, LW, 1), grid((unsigned)tiles, 1, (unsigned)((nz + A.chunk - 1) / A.chunk));
+            with_bool(wl, [&](auto W) { with_tvd(s, [&](auto T) { with_bool(reduce, [&](auto Rd) {
+                launch_kernel(mc::k_lane<2, -1, 1, LW, decltype(W)::value, decltype(T)::value, decltype(Rd)::value>, grid, block, 0, st, A);
+            }); }); });
         } else {
             return fail(MC_TVD_EINVAL, "a 2-D problem has no y-sweep");
         }
     } else {
-        const int WB = TILE_WB_3D, OB = WB - 4;
-        block = dim3(32, WB, 1);
+        constexpr int WB = TILE_WB_3D, OB = WB - 4;
+        dim3 block(32, WB, 1);
         long long xt = (nx + mc::LANE_OUT - 1) / mc::LANE_OUT;
         if (alpha == 2) {            // z-sweep: march z, tile (x, y)
-            A.n_b = ny; A.s_b = nx; A.wall_b = 0; A.inv2d_b = 1.0 / (2.0 * s->d[1]);
-            A.n_m = nz; A.s_m = (long long)nx * ny; A.wall_m = wl;
+            A.n_b = ny; A.s_b = nx; A.n_m = nz; A.s_m = (long long)nx * ny;
             long long bt = (ny + OB - 1) / OB;
             A.chunk = pick_chunk(s, nz, xt * bt);
-            grid = dim3((unsigned)xt, (unsigned)bt, (unsigned)((nz + A.chunk - 1) / A.chunk));
-            smem = (size_t)4 * 3 * 32 * WB * sizeof(double);
-            { auto kfn = mc::k_march<3, 2, 1>; MC_LAUNCH(kfn, grid, block, smem, s->stream, A); }
+            dim3 grid((unsigned)xt, (unsigned)bt, (unsigned)((nz + A.chunk - 1) / A.chunk));
+            size_t smem = ((size_t)4 * 3 * 32 * WB + 4) * sizeof(double);
+            with_bool(wl, [&](auto W) { with_tvd(s, [&](auto T) {
+                launch_kernel(mc::k_march<3, 2, 1, 32, WB, decltype(W)::value, false, decltype(T)::value>, grid, block, smem, st, A);
+            }); });
         } else if (alpha == 1) {     // y-sweep: march y, tile (x, z)
-            A.n_b = nz; A.s_b = (long long)nx * ny; A.wall_b = wl; A.inv2d_b = 1.0 / (2.0 * s->d[2]);
-            A.n_m = ny; A.s_m = nx; A.wall_m = 0;
+            A.n_b = nz; A.s_b = (long long)nx * ny; A.n_m = ny; A.s_m = nx;
             long long bt = (nz + OB - 1) / OB;
             A.chunk = pick_chunk(s, ny, xt * bt);
-            grid = dim3((unsigned)xt, (unsigned)bt, (unsigned)((ny + A.chunk - 1) / A.chunk));
-            smem = (size_t)4 * 3 * 32 * WB * sizeof(double);
-            { auto kfn = mc::k_march<3, 1, 2>; MC_LAUNCH(kfn, grid, block, smem, s->stream, A); }
+            dim3 grid((unsigned)xt, (unsigned)bt, (unsigned)((ny + A.chunk - 1) / A.chunk));
+            size_t smem = ((size_t)4 * 3 * 32 * WB + 4) * sizeof(double);
+            with_bool(wl, [&](auto W) { with_tvd(s, [&](auto T) {
+                launch_kernel(mc::k_march<3, 1, 2, 32, WB, false, decltype(W)::value, decltype(T)::value>, grid, block, smem, st, A);
+            }); });
         } else {                     // x-sweep: lanes x, tile (x, y), march z
-            A.n_b = ny; A.s_b = nx; A.wall_b = 0; A.inv2d_b = 1.0 / (2.0 * s->d[1]);
-            A.n_m = nz; A.s_m = (long long)nx * ny; A.wall_m = wl; A.inv2d_m = 1.0 / (2.0 * s->d[2]);
+            A.n_b = ny; A.s_b = nx; A.n_m = nz; A.s_m = (long long)nx * ny;
             long long bt = (ny + OB - 1) / OB;
             A.chunk = pick_chunk(s, nz, xt * bt);
-            grid = dim3((unsigned)xt, (unsigned)bt, (unsigned)((nz + A.chunk - 1) / A.chunk));
-            smem = (size_t)4 * 2 * 32 * WB * sizeof(double);
-            { auto kfn = mc::k_lane<3, 1, 2>; MC_LAUNCH(kfn, grid, block, smem, s->stream, A); }
+            dim3 grid((unsigned)xt, (unsigned)bt, (unsigned)((nz + A.chunk - 1) / A.chunk));
+            size_t smem = (size_t)4 * 2 * 32 * WB * sizeof(double);
+            with_bool(wl, [&](auto W) { with_tvd(s, [&](auto T) { with_bool(reduce, [&](auto Rd) {
+                launch_kernel(mc::k_lane<3, 1, 2, WB, decltype(W)::value, decltype(T)::value, decltype(Rd)::value>, grid, block, smem, st, A);
+            }); }); });
         }
     }
     s->launches += 1;

@@ -8,147 +8,212 @@
 // flux (d_x, d_b of u, central, R7) travel through shared memory, one plane per level, double
 // buffered, ONE __syncthreads per level.  A block owns a (x, b) tile with a 2-node halo ring that is
 // recomputed (ring 2: primitives; ring 1: predictor) and a chunk of levels with a 4-level warm-up.
+// In 3-D a tile row is one warp, so the role of a row (ring 2 / ring 1 / plate row / interior) is warp
+// uniform and each role runs its own loop; the x-halo lanes of a row simply compute along (their
+// results are never stored), which keeps every warp free of divergence.
 // dir = -1 (R9) is the same code marching from the other end with a negated spacing: the mirror
 // identity of the scheme (tests/test_oracle_pins.py::test_mirror_identity) makes it bit-equivalent.
 //
-// Pipeline of iteration j (output level j):  W(j+2) -> F(j+1) -> P(j+1) | barrier | F^P(j+1) -> out(j)
+// The loop body exists in two instantiations: FAST (every level j-1 .. j+3 exists, no plate among them,
+// pipeline full: no predicates at all, unrolled by two so that the register pipeline needs no moves) and
+// the general one (warm-up levels, plates of the marching direction, the tail).
+//
+// Pipeline of iteration j (output level j):
+//   prefetch X(j+3) | W(j+2) -> TVD(j+1/2) -> F(j+1) -> P(j+1) | barrier | F^P(j+1) -> out(j)
 #pragma once
+#include <type_traits>
+
 #include "mc_common.cuh"
 
 namespace mc {
 
-// CA: velocity component of alpha; CB: velocity component of the tile's second direction b (-1 in 2-D).
-template <int ND, int CA, int CB>
-MC_KERNEL void k_march(SweepArgs A)
+enum { ROLE_NONE = 0, ROLE_R2 = 1, ROLE_WALLROW = 2, ROLE_R1 = 3, ROLE_IN = 4 };
+
+// CA: velocity component of alpha; CB: velocity component of the tile's second direction b (-1 in 2-D);
+// WX x WB: threads of a block (WB = 1 in 2-D); WALL_M / WALL_B: the marching / second direction is z
+// with plates; TVD: -1 no TVD term, 0 Eq. 34 as printed, 1 Davis/Yee (R4).
+template <int ND, int CA, int CB, int WX, int WB, bool WALL_M, bool WALL_B, int TVD>
+MC_KERNEL void __launch_bounds__(WX * WB, 1) k_march(SweepArgs A)
 {
     constexpr int NF = ND + 2;
     constexpr bool HAS_B = (CB >= 0);
     constexpr bool Z_IS_ALPHA = (CA == ND - 1);      // z is the last velocity component
-    MC_SHARED_DECL(double, smem);
+    constexpr int TILE = WX * WB;
+    constexpr int cb = HAS_B ? CB : 0;
+    MC_SHARED_DECL(double, smem_raw);
+    double *const smem = smem_raw + 2;                // two pad doubles in front: lane 0 may read [-1]
+    double *const slotU = smem;                       // [2][ND][TILE]  velocities of X     (levels j+1, j+2)
+    double *const slotP = smem + 2 * ND * TILE;       // [2][ND][TILE]  velocities of X^P   (level j+1)
 
-    const int tx = threadIdx.x, Wx = blockDim.x;
-    const int ty = HAS_B ? (int)threadIdx.y : 0, Wb = HAS_B ? (int)blockDim.y : 1;
-    const int tile_n = Wx * Wb, tidx = ty * Wx + tx;
-    double *slotU = smem;                             // [2][ND][tile_n]  velocities of X     (levels j+1, j+2)
-    double *slotP = smem + 2 * ND * tile_n;           // [2][ND][tile_n]  velocities of X^P   (level j+1)
+    const int tx = threadIdx.x;
+    const int ty = HAS_B ? (int)threadIdx.y : 0;
+    const int tidx = ty * WX + tx;
 
     // ---- tile geometry --------------------------------------------------------------------
-    const int gx = (int)blockIdx.x * (Wx - 4) + tx - 2;
-    const int ix = wrap(gx, A.nx);
-    const int rx = min(tx, Wx - 1 - tx);
-    int gb = 0, rb = 99, gb_raw = 0;
-    bool row_exists = true, wallrow = false;
+    const int gx = (int)blockIdx.x * (WX - 4) + tx - 2;
+    const int ix = wrap1(gx, A.nx);                   // nx >= 4 (mc_tvd_init) and gx in [-2, nx + WX)
+    const int rx = min(tx, WX - 1 - tx);
+    int gb = 0, rb = 99;
+    bool row_exists = true, wallrow = false, row_in_range = true;
     long long col = ix;
     if (HAS_B) {
-        gb = (int)blockIdx.y * (Wb - 4) + ty - 2;
-        gb_raw = gb;
-        rb = min(ty, Wb - 1 - ty);
-        if (A.wall_b) {
-            row_exists = (gb >= 0 && gb < A.n_b);
-            wallrow = (gb == 0 || gb == A.n_b - 1);
-            col += (long long)(row_exists ? gb : 0) * A.s_b;
+        const int gb_raw = (int)blockIdx.y * (WB - 4) + ty - 2;
+        rb = min(ty, WB - 1 - ty);
+        row_in_range = gb_raw < A.n_b;
+        if (WALL_B) {
+            row_exists = (gb_raw >= 0 && gb_raw < A.n_b);
+            wallrow = (gb_raw == 0 || gb_raw == A.n_b - 1);
+            gb = row_exists ? gb_raw : 0;
         } else {
-            gb = wrap(gb, A.n_b);                     // periodic b: the node's own index (z_k of Eq. 17)
-            col += (long long)gb * A.s_b;
+            gb = wrap1(gb_raw, A.n_b);                // periodic b: the node's own index
         }
+        col += (long long)gb * A.s_b;
     }
-    const bool needP = row_exists && !wallrow && rx >= 1 && rb >= 1 && (rx >= 2 || rb >= 2);
-    const bool owner = row_exists && rx >= 2 && rb >= 2 && gx < A.nx && (!HAS_B || gb_raw < A.n_b);
+    const bool owner = row_exists && rx >= 2 && rb >= 2 && gx < A.nx && row_in_range;
+    int role = ROLE_IN;
+    if (HAS_B) {
+        if (!row_exists) role = ROLE_NONE;
+        else if (wallrow) role = ROLE_WALLROW;
+        else if (rb == 0) role = ROLE_R2;
+        else if (rb == 1) role = ROLE_R1;
+    }
 
     // ---- sweep constants ------------------------------------------------------------------
     const double tau = A.dt_ptr ? 0.5 * (*A.dt_ptr) : A.tau_fixed;
-    const double h = (A.dir > 0) ? A.d_a : -A.d_a;    // signed spacing in marching coordinates
-    const double inv_h = 1.0 / h;
-    const double cdt = tau / h;                       // tau / dx_alpha of Eqs. 31-32
-    const double tau_over_d = tau / A.d_a;            // for Co (R5)
-    const double src_c = A.src ? -A.g : 0.0;          // S = -g rho in the rho u_z row
+    const double cdt = tau * A.inv_h;                 // tau / dx_alpha of Eqs. 31-32, signed
+    const double hcdt = 0.5 * cdt;
+    const double half_tod = 0.5 * tau / A.d_a;        // for Co (R5)
+    const double tsrc = A.src ? -(tau * A.g) : 0.0;   // tau S: S = -g rho in the rho u_z row
     const int n = A.n_m;
     const int l0 = (int)blockIdx.z * A.chunk;
     const int l1 = min(n, l0 + A.chunk);
+    const long long sm_signed = (A.dir > 0) ? A.s_m : -A.s_m;
+    const double *const pin = A.in + col + ((A.dir > 0) ? 0 : (long long)(n - 1) * A.s_m);
+    double *const pout = A.out + col + ((A.dir > 0) ? 0 : (long long)(n - 1) * A.s_m);
+    const double gz_fixed = A.g * ((double)gb * A.dz);                       // used when b is z
 
-    auto exists = [&](int l) { return A.wall_m ? (l >= 0 && l < n) : true; };
-    auto phys = [&](int l) { int w = wrap(l, n); return (A.dir > 0) ? w : n - 1 - w; };
+    auto exists = [&](int l) { return WALL_M ? (l >= 0 && l < n) : true; };
+    auto lev = [&](int l) { return WALL_M ? l : wrap1(l, n); };              // l in [-n, 2n)
     auto gz_of = [&](int l) {                         // g z_k of Eq. 17 for this thread's node at level l
-        int kz = Z_IS_ALPHA ? phys(l) : gb;
-        return A.g * ((double)kz * A.dz);
+        if (!Z_IS_ALPHA) return gz_fixed;
+        const int w = lev(l);
+        return A.g * ((double)((A.dir > 0) ? w : n - 1 - w) * A.dz);
     };
     auto load = [&](int l, double (&X)[NF]) {
-        const double *p = A.in + col + (long long)phys(l) * A.s_m;
+        const double *p = pin + (long long)lev(l) * sm_signed;
 #pragma unroll
         for (int f = 0; f < NF; ++f) X[f] = p[(long long)f * A.N];
     };
+    auto store = [&](int l, const double (&o)[NF]) {
+        double *q = pout + (long long)lev(l) * sm_signed;
+#pragma unroll
+        for (int f = 0; f < NF; ++f) q[(long long)f * A.N] = o[f];
+    };
     auto publish = [&](double *slot, int parity, const double (&u)[ND]) {
 #pragma unroll
-        for (int c = 0; c < ND; ++c) slot[(parity * ND + c) * tile_n + tidx] = u[c];
+        for (int c = 0; c < ND; ++c) slot[(parity * ND + c) * TILE + tidx] = u[c];
     };
-    // central cross derivatives of the velocities published in `slot` (R7)
-    auto cross = [&](const double *slot, int parity, double (&dcu_a)[ND], double (&dcu_c)[ND]) {
-        const double *s = slot + parity * ND * tile_n + tidx;
+    // central cross DIFFERENCES of the velocities published in `slot` (R7)
+    auto cross = [&](const double *slot, int parity, double (&dxa)[ND], double (&dxc)[ND]) {
+        const double *s = slot + parity * ND * TILE + tidx;
 #pragma unroll
-        for (int c = 0; c < ND; ++c) { dcu_a[c] = 0.0; dcu_c[c] = 0.0; }
-        dcu_a[0] = (s[CA * tile_n + 1] - s[CA * tile_n - 1]) * A.inv2d_x;
-        dcu_c[0] = (s[0 * tile_n + 1] - s[0 * tile_n - 1]) * A.inv2d_x;
+        for (int c = 0; c < ND; ++c) { dxa[c] = 0.0; dxc[c] = 0.0; }
+        dxa[0] = s[CA * TILE + 1] - s[CA * TILE - 1];
+        dxc[0] = s[1] - s[-1];
         if (HAS_B) {
-            constexpr int cb = HAS_B ? CB : 0;
-            dcu_a[cb] = (s[CA * tile_n + Wx] - s[CA * tile_n - Wx]) * A.inv2d_b;
-            dcu_c[cb] = (s[cb * tile_n + Wx] - s[cb * tile_n - Wx]) * A.inv2d_b;
+            dxa[cb] = s[CA * TILE + WX] - s[CA * TILE - WX];
+            dxc[cb] = s[cb * TILE + WX] - s[cb * TILE - WX];
         }
     };
     // plate values of a node on a plate of the marching direction: no slip,
     // T = T_w; only rho is free (R10)
     auto plate = [&](int l, double rho, double (&X)[NF]) {
-        int k = phys(l);
-        double Tw = (k == 0) ? A.Tw0 : A.Tw1;
+        const int k = (A.dir > 0) ? l : n - 1 - l;
+        const double Tw = (k == 0) ? A.Tw0 : A.Tw1;
         X[0] = rho;
 #pragma unroll
         for (int c = 0; c < ND; ++c) X[1 + c] = 0.0;
         X[NF - 1] = rho * (A.cv * Tw + A.g * ((double)k * A.dz));
     };
 
-    // ---- carried state ----------------------------------------------------------------------
-    double Xc[NF], F0[NF], FP0[NF], H0[NF], d0[NF];
-    double uP0[ND], TP0 = 0.0, a0 = 0.0, b0 = 0.0, C0 = 0.0, C1 = 0.0;
-    Prim<ND> w1;
+    // ---- carried state (levels relative to the current output level j) -------------------------
+    double Xn[NF];                 // X(j+2), prefetched during the previous iteration
+    double Xc[NF];                 // X(j+1)
+    double F0[NF], FP0[NF];        // F(j), F^P(j)
+    double H0[NF];                 // (X^P + X)/2 + tau S^P/2 - Dh_{j-1/2} of level j
+    double d0[NF];                 // dX_{j+1/2}
+    double uP0[ND], TP0 = 1.0;     // u, T of X^P(j)
+    double a0 = 0.0, b0 = 0.0;     // (dX_{j-1/2}, dX_{j+1/2}), |dX_{j+1/2}|^2
+    double hC0 = 0.0, hC1 = 0.0;   // C/2 of Eq. 39 at levels j, j+1
+    double gz1 = 0.0;              // g z of level j+1
+    Prim<ND> w1;                   // primitives of X(j+1)
 #pragma unroll
-    for (int f = 0; f < NF; ++f) { Xc[f] = 0.0; F0[f] = 0.0; FP0[f] = 0.0; H0[f] = 0.0; d0[f] = 0.0; }
+    for (int f = 0; f < NF; ++f) { Xn[f] = 0.0; Xc[f] = 0.0; F0[f] = 0.0; FP0[f] = 0.0; H0[f] = 0.0; d0[f] = 0.0; }
+    Xn[0] = 1.0; Xc[0] = 1.0;
 #pragma unroll
     for (int c = 0; c < ND; ++c) { uP0[c] = 0.0; w1.u[c] = 0.0; }
     w1.T = 1.0; w1.p = 0.0;
 
-    for (int j = l0 - 4; j < l1; ++j) {
-        const int p1 = (j + 1) & 1, p2 = (j + 2) & 1;
-        const bool ex1 = exists(j + 1), ex2 = exists(j + 2);
-        const bool ld1 = ex1 && (j + 1 >= l0 - 2);              // level j+1 is loaded (Xc, w1 valid)
-        const bool ld2 = ex2;                                   // level j+2 is loaded this iteration
-        const bool start_wall1 = A.wall_m && (j + 1 == 0);      // level j+1 is the plate the march starts on
-        const bool end_wall1 = A.wall_m && (j + 1 == n - 1);    // level j+1 is the plate the march ends on
+    // One iteration.  ROLE and FAST are compile-time tags; PAR is the compile-time parity of j in the
+    // unrolled FAST pair (-1: take it from j).
+    auto body = [&](auto role_tag, auto fast_tag, auto par_tag, const int j) {
+        constexpr int ROLE = decltype(role_tag)::value;
+        constexpr bool FAST = decltype(fast_tag)::value;
+        constexpr int PAR = decltype(par_tag)::value;
+        const int p1 = (PAR >= 0) ? (PAR ^ 1) : ((j + 1) & 1);   // parity of level j+1
+        const int p2 = p1 ^ 1;                                   // parity of level j+2
+        const bool ex1 = FAST || exists(j + 1), ex2 = FAST || exists(j + 2);
+        const bool ld1 = FAST || (ex1 && (j + 1 >= l0 - 2));     // level j+1 is loaded (Xc, w1 valid)
+        const bool ld2 = ex2;
+        const bool start_wall1 = !FAST && WALL_M && (j + 1 == 0);     // level j+1 is the plate the march starts on
+        const bool end_wall1 = !FAST && WALL_M && (j + 1 == n - 1);   // level j+1 is the plate the march ends on
 
-        // (1) W(j+2): load, primitives, Courant coefficient, publish velocities
-        double Xn[NF];
-        Prim<ND> w2;
-        double C2 = 0.0;
+        if (ROLE == ROLE_NONE) { __syncthreads(); return; }
+
+        // (0) prefetch X(j+3) for the next iteration
+        double Xq[NF];
 #pragma unroll
-        for (int f = 0; f < NF; ++f) Xn[f] = 0.0;
-#pragma unroll
-        for (int c = 0; c < ND; ++c) w2.u[c] = 0.0;
-        w2.T = 1.0; w2.p = 0.0;
-        if (ld2 && row_exists) {
-            load(j + 2, Xn);
-            w2 = primitives<ND>(Xn, gz_of(j + 2), A);
-            C2 = courant_coef(w2.u[CA], w2.T, tau_over_d, A);
+        for (int f = 0; f < NF; ++f) Xq[f] = Xn[f];
+        if (FAST || (exists(j + 3) && j + 3 <= l1 + 1)) load(j + 3, Xq);
+
+        // (1) W(j+2): primitives, Courant coefficient, publish velocities
+        Prim<ND> w2 = w1;
+        double hC2 = 0.0, gz2 = 0.0;
+        if (ld2) {
+            gz2 = gz_of(j + 2);
+            w2 = primitives<ND>(Xn, gz2, A);
+            if (ROLE == ROLE_IN && TVD >= 0) hC2 = half_courant_coef(w2.u[CA], w2.T, half_tod, A);
             publish(slotU, p2, w2.u);
+        }
+        if (ROLE == ROLE_R2) {
+            __syncthreads();
+#pragma unroll
+            for (int f = 0; f < NF; ++f) Xn[f] = Xq[f];
+            return;
+        }
+        if (ROLE == ROLE_WALLROW) {
+            // a plate row of b (y-sweep): X^P = X and the output is X (R10); publish u^P = u of level j+1
+            if (ld1) publish(slotP, p1, w1.u);
+            __syncthreads();
+            if (j >= l0 && owner) store(j, H0);
+#pragma unroll
+            for (int f = 0; f < NF; ++f) { H0[f] = Xc[f]; Xc[f] = Xn[f]; Xn[f] = Xq[f]; }
+            w1 = w2;
+            return;
         }
 
         // (2) TVD (Eqs. 34-39): Dh_{j+1/2} from dX_{j-1/2}, dX_{j+1/2}, dX_{j+3/2}
-        double d1[NF], a1 = 0.0, b1 = 0.0, Dh[NF];
+        double d1[NF], Dh[NF], a1 = 0.0, b1 = 0.0;
 #pragma unroll
-        for (int f = 0; f < NF; ++f) { d1[f] = (ld1 && ld2) ? Xn[f] - Xc[f] : 0.0; Dh[f] = 0.0; }
+        for (int f = 0; f < NF; ++f) { Dh[f] = 0.0; d1[f] = 0.0; }
+        if (ROLE == ROLE_IN && TVD >= 0) {
 #pragma unroll
-        for (int f = 0; f < NF; ++f) { b1 += d1[f] * d1[f]; a1 += d0[f] * d1[f]; }
-        {
-            bool have = (j >= l0 - 1) && exists(j - 1) && exists(j) && ex1 && ex2 && !A.tvd_off;   // R11 at plates
-            if (have && owner && !wallrow) {
-                double coef = tvd_coef(a0, a1, b0, C0, C1, A.tvd_form);
+            for (int f = 0; f < NF; ++f) d1[f] = (ld1 && ld2) ? Xn[f] - Xc[f] : 0.0;
+#pragma unroll
+            for (int f = 0; f < NF; ++f) { b1 = fma(d1[f], d1[f], b1); a1 = fma(d0[f], d1[f], a1); }
+            const bool have = FAST || ((j >= l0 - 1) && exists(j - 1) && exists(j) && ex1 && ex2);   // R11 at plates
+            if (have) {
+                const double coef = tvd_coef<(TVD >= 0 ? TVD : 0)>(a0, a1, b0, hC0, hC1);
 #pragma unroll
                 for (int f = 0; f < NF; ++f) { Dh[f] = coef * d0[f]; H0[f] += Dh[f]; }
             }
@@ -156,25 +221,23 @@ MC_KERNEL void k_march(SweepArgs A)
 
         // (3) F(j+1): flux of X at level j+1 (inner derivative forward in marching coordinates)
         double F1[NF], XP[NF], H1[NF];
-        Prim<ND> wP1;
+        Prim<ND> wP1 = w1;
 #pragma unroll
         for (int f = 0; f < NF; ++f) { F1[f] = 0.0; XP[f] = Xc[f]; H1[f] = Xc[f]; }
-        wP1 = w1;
-        const bool doF = ld1 && needP;
+        const bool doF = ld1;
         if (doF) {
             if (end_wall1) {
                 F1[0] = Xc[1 + CA];                   // only the mass flux is defined and needed (R10)
             } else {
-                double dau[ND], daT, dcu_a[ND], dcu_c[ND];
+                double du[ND], dxa[ND], dxc[ND];
 #pragma unroll
-                for (int c = 0; c < ND; ++c) dau[c] = (w2.u[c] - w1.u[c]) * inv_h;
-                daT = (w2.T - w1.T) * inv_h;
-                cross(slotU, p1, dcu_a, dcu_c);
-                flux<ND, CA>(Xc, w1, dau, daT, dcu_a, dcu_c, A, F1);
+                for (int c = 0; c < ND; ++c) du[c] = w2.u[c] - w1.u[c];
+                cross(slotU, p1, dxa, dxc);
+                flux<ND, CA>(Xc, w1, du, w2.T - w1.T, dxa, dxc, A, F1);
             }
         }
         // (4) P(j+1): predictor (Eq. 31), plate values, primitives of X^P, publish
-        const bool doP = doF && (j + 1 >= l0 - 1);
+        const bool doP = FAST || (doF && (j + 1 >= l0 - 1));
         if (doP) {
             if (start_wall1) {
                 plate(j + 1, Xc[0], XP);                                      // rho unchanged
@@ -182,59 +245,96 @@ MC_KERNEL void k_march(SweepArgs A)
                 plate(j + 1, Xc[0] - 2.0 * cdt * (F1[0] - F0[0]), XP);       // half-cell closure (R10)
             } else {
 #pragma unroll
-                for (int f = 0; f < NF; ++f) XP[f] = Xc[f] - cdt * (F1[f] - F0[f]);
-                XP[1 + CA] += tau * (src_c * Xc[0]);
+                for (int f = 0; f < NF; ++f) {
+                    const double dF = F1[f] - F0[f];
+                    XP[f] = fma(-cdt, dF, Xc[f]);
+                    H1[f] = fma(-hcdt, dF, Xc[f]) - Dh[f];                    // (X^P + X)/2 - Dh
+                }
+                XP[1 + CA] = fma(tsrc, Xc[0], XP[1 + CA]);
+                H1[1 + CA] = fma(0.5 * tsrc, Xc[0], H1[1 + CA]);
             }
-            wP1 = primitives<ND>(XP, gz_of(j + 1), A);
+            wP1 = primitives<ND>(XP, gz1, A);
+            if (start_wall1 || end_wall1) {
 #pragma unroll
-            for (int f = 0; f < NF; ++f) H1[f] = 0.5 * (XP[f] + Xc[f]) - Dh[f];
-            H1[1 + CA] += 0.5 * (tau * (src_c * XP[0]));
+                for (int f = 0; f < NF; ++f) H1[f] = 0.5 * (XP[f] + Xc[f]);
+            } else {
+                H1[1 + CA] = fma(0.5 * tsrc, XP[0], H1[1 + CA]);             // + tau S(X^P)/2
+            }
         }
-        if (ld1 && row_exists) publish(slotP, p1, wP1.u);      // plate rows of b publish u^P = u (X^P = X there)
+        if (ld1) publish(slotP, p1, wP1.u);
 
         __syncthreads();
 
-        // (5) F^P(j+1): flux of X^P at level j+1 (inner derivative backward in marching coordinates)
-        double FP1[NF];
+        if (ROLE == ROLE_IN) {
+            // (5) F^P(j+1): flux of X^P at level j+1 (inner derivative backward in marching coordinates)
+            double FP1[NF];
 #pragma unroll
-        for (int f = 0; f < NF; ++f) FP1[f] = 0.0;
-        const bool doFP = doP && owner && (j + 1 >= l0);
-        if (doFP) {
-            if (start_wall1) {
-                FP1[0] = XP[1 + CA];
-            } else {
-                double dau[ND], daT, dcu_a[ND], dcu_c[ND];
+            for (int f = 0; f < NF; ++f) FP1[f] = 0.0;
+            const bool doFP = FAST || (doP && (j + 1 >= l0));
+            if (doFP) {
+                if (start_wall1) {
+                    FP1[0] = XP[1 + CA];
+                } else {
+                    double du[ND], dxa[ND], dxc[ND];
 #pragma unroll
-                for (int c = 0; c < ND; ++c) dau[c] = (wP1.u[c] - uP0[c]) * inv_h;
-                daT = (wP1.T - TP0) * inv_h;
-                cross(slotP, p1, dcu_a, dcu_c);
-                flux<ND, CA>(XP, wP1, dau, daT, dcu_a, dcu_c, A, FP1);
+                    for (int c = 0; c < ND; ++c) du[c] = wP1.u[c] - uP0[c];
+                    cross(slotP, p1, dxa, dxc);
+                    flux<ND, CA>(XP, wP1, du, wP1.T - TP0, dxa, dxc, A, FP1);
+                }
             }
-        }
-        // (6) out(j): corrector (Eq. 32), average and TVD term (Eq. 33), plate values
-        if (j >= l0 && owner && exists(j)) {
-            double o[NF];
-            if (wallrow) {
+            // (6) out(j): corrector (Eq. 32), average and TVD term (Eq. 33), plate values
+            if (FAST || (j >= l0 && exists(j))) {
+                double o[NF];
+                if (!FAST && WALL_M && j == 0) {
+                    plate(j, H0[0] - cdt * (FP1[0] - FP0[0]), o);            // 0.5 * (2 tau/dz) * dF
+                } else if (!FAST && WALL_M && j == n - 1) {
+                    plate(j, H0[0], o);
+                } else {
 #pragma unroll
-                for (int f = 0; f < NF; ++f) o[f] = H0[f];            // plate rows of b: unchanged (R10)
-            } else if (A.wall_m && j == 0) {
-                plate(j, H0[0] - cdt * (FP1[0] - FP0[0]), o);        // 0.5 * (2 tau/dz) * dF
-            } else if (A.wall_m && j == n - 1) {
-                plate(j, H0[0], o);
-            } else {
-#pragma unroll
-                for (int f = 0; f < NF; ++f) o[f] = H0[f] - 0.5 * cdt * (FP1[f] - FP0[f]);
+                    for (int f = 0; f < NF; ++f) o[f] = fma(-hcdt, FP1[f] - FP0[f], H0[f]);
+                }
+                if (owner) store(j, o);
             }
-            double *q = A.out + col + (long long)phys(j) * A.s_m;
 #pragma unroll
-            for (int f = 0; f < NF; ++f) q[(long long)f * A.N] = o[f];
+            for (int f = 0; f < NF; ++f) { FP0[f] = FP1[f]; d0[f] = d1[f]; }
+            a0 = a1; b0 = b1; hC0 = hC1; hC1 = hC2;
+#pragma unroll
+            for (int c = 0; c < ND; ++c) uP0[c] = wP1.u[c];
+            TP0 = wP1.T;
         }
         // (7) rotate the pipeline
 #pragma unroll
-        for (int f = 0; f < NF; ++f) { Xc[f] = Xn[f]; F0[f] = F1[f]; FP0[f] = FP1[f]; H0[f] = H1[f]; d0[f] = d1[f]; }
-#pragma unroll
-        for (int c = 0; c < ND; ++c) uP0[c] = wP1.u[c];
-        TP0 = wP1.T; w1 = w2; C0 = C1; C1 = C2; a0 = a1; b0 = b1;
+        for (int f = 0; f < NF; ++f) { Xc[f] = Xn[f]; Xn[f] = Xq[f]; F0[f] = F1[f]; H0[f] = H1[f]; }
+        w1 = w2; gz1 = gz2;
+    };
+
+    // ---- the march -------------------------------------------------------------------------------
+    auto march = [&](auto role_tag) {
+        using std::integral_constant;
+        integral_constant<bool, false> slow;
+        integral_constant<bool, true> fast;
+        integral_constant<int, -1> par_any;
+        int j = l0 - 4;
+        if (exists(j + 2)) load(j + 2, Xn);
+        const int jf0 = WALL_M ? max(l0, 1) : l0;
+        const int jf1 = WALL_M ? min(l1, n - 3) : l1;
+        for (; j < l1 && (j < jf0 || (j & 1)); ++j) body(role_tag, slow, par_any, j);
+        for (; j + 1 < jf1; j += 2) {
+            body(role_tag, fast, integral_constant<int, 0>(), j);
+            body(role_tag, fast, integral_constant<int, 1>(), j + 1);
+        }
+        for (; j < l1; ++j) body(role_tag, slow, par_any, j);
+    };
+    if (!HAS_B) {
+        march(std::integral_constant<int, ROLE_IN>());
+    } else {
+        switch (role) {
+        case ROLE_NONE: march(std::integral_constant<int, ROLE_NONE>()); break;
+        case ROLE_R2: march(std::integral_constant<int, ROLE_R2>()); break;
+        case ROLE_WALLROW: march(std::integral_constant<int, WALL_B ? ROLE_WALLROW : ROLE_NONE>()); break;
+        case ROLE_R1: march(std::integral_constant<int, ROLE_R1>()); break;
+        default: march(std::integral_constant<int, ROLE_IN>()); break;
+        }
     }
 }
 
