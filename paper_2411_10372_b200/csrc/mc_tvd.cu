@@ -15,6 +15,7 @@
 #include "reduce_kernels.cuh"
 #include "sweep_lane.cuh"
 #include "sweep_march.cuh"
+#include "sweep_march3.cuh"
 
 namespace {
 
@@ -28,9 +29,34 @@ int fail(int code, const char *fmt, const char *detail = "")
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
-constexpr int MARCH_WX_2D = 128;       // k_march, 2-D: 124 outputs per block row
-constexpr int TILE_WB_3D = 12;         // 3-D tiles: 32 x 12 threads, 28 x 8 outputs (register-limited)
-constexpr int LANE_WARPS_2D = 4;       // k_lane, 2-D: independent warps per block
+// launch geometry (the -D overrides exist for tuning sweeps; the defaults are the measured best)
+#ifndef MC_MARCH_WX_2D
+#define MC_MARCH_WX_2D 128
+#endif
+#ifndef MC_MARCH_MINB_2D
+#define MC_MARCH_MINB_2D 4
+#endif
+#ifndef MC_TILE_WB_3D
+#define MC_TILE_WB_3D 12
+#endif
+#ifndef MC_MARCH3_WB
+#define MC_MARCH3_WB 12
+#endif
+#ifndef MC_MARCH3_MINB
+#define MC_MARCH3_MINB 1
+#endif
+#ifndef MC_LANE_WARPS_2D
+#define MC_LANE_WARPS_2D 4
+#endif
+#ifndef MC_LANE_MINB_2D
+#define MC_LANE_MINB_2D 4
+#endif
+constexpr int MARCH_WX_2D = MC_MARCH_WX_2D;      // k_march, 2-D: WX - 4 outputs per block row
+constexpr int MARCH_MINB_2D = MC_MARCH_MINB_2D;  // k_march, 2-D: resident blocks per SM the register budget allows
+constexpr int TILE_WB_3D = MC_TILE_WB_3D;        // 3-D tiles: 32 x WB threads, 28 x (WB - 4) outputs (register-limited)
+constexpr int MARCH3_WB = MC_MARCH3_WB;          // k_march3: 32 x WB threads, 28 x (WB - 2) outputs
+constexpr int LANE_WARPS_2D = MC_LANE_WARPS_2D;  // k_lane, 2-D: independent warps per block
+constexpr int LANE_MINB_2D = MC_LANE_MINB_2D;
 constexpr int DIAG_MAX_BLOCKS = 64;    // blocks per plane in the diagnostics pass
 
 struct Layout {                        // byte offsets inside the workspace
@@ -158,8 +184,20 @@ template <class F> void with_bool(bool b, F f)
 {
     if (b) f(std::true_type()); else f(std::false_type());
 }
+// MC_ONLY_DEFAULT_SWITCHES (tuning builds only): instantiate just the plates + Davis/Yee kernels
+template <class F> void with_walls(bool b, F f)
+{
+#ifdef MC_ONLY_DEFAULT_SWITCHES
+    (void)b; f(std::true_type());
+#else
+    with_bool(b, f);
+#endif
+}
 template <class F> void with_tvd(const mc_tvd_state *s, F f)
 {
+#ifdef MC_ONLY_DEFAULT_SWITCHES
+    (void)s; f(std::integral_constant<int, 1>()); return;
+#endif
     if (s->par.tvd_off) f(std::integral_constant<int, -1>());
     else if (s->par.tvd_form == 0) f(std::integral_constant<int, 0>());
     else f(std::integral_constant<int, 1>());
@@ -167,6 +205,16 @@ template <class F> void with_tvd(const mc_tvd_state *s, F f)
 
 template <class K> int launch_kernel(K kfn, dim3 grid, dim3 block, size_t smem, cudaStream_t st, const mc::SweepArgs &A)
 {
+    if (smem > 48 * 1024) {            // opt in to large dynamic shared memory, once per kernel
+        static K raised[64];
+        static int n_raised = 0;
+        bool seen = false;
+        for (int i = 0; i < n_raised; ++i) seen = seen || (raised[i] == kfn);
+        if (!seen) {
+            cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+            if (n_raised < 64) raised[n_raised++] = kfn;
+        }
+    }
     MC_LAUNCH(kfn, grid, block, smem, st, A);
     return 0;
 }
@@ -191,8 +239,8 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
             A.chunk = pick_chunk(s, nz, tiles);
             dim3 block(WX, 1, 1), grid((unsigned)tiles, 1, (unsigned)((nz + A.chunk - 1) / A.chunk));
             size_t smem = ((size_t)4 * 2 * WX + 4) * sizeof(double);
-            with_bool(wl, [&](auto W) { with_tvd(s, [&](auto T) {
-                launch_kernel(mc::k_march<2, 1, -1, WX, 1, decltype(W)::value, false, decltype(T)::value>, grid, block, smem, st, A);
+            with_walls(wl, [&](auto W) { with_tvd(s, [&](auto T) {
+                launch_kernel(mc::k_march<2, 1, -1, WX, 1, decltype(W)::value, false, decltype(T)::value, MARCH_MINB_2D>, grid, block, smem, st, A);
             }); });
         } else if (alpha == 0) {     // x-sweep: lanes x, march z
             constexpr int LW = LANE_WARPS_2D;
@@ -201,8 +249,8 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
             long long tiles = (xt + LW - 1) / LW;
             A.chunk = pick_chunk(s, nz, tiles);
             dim3 block(32, LW, 1), grid((unsigned)tiles, 1, (unsigned)((nz + A.chunk - 1) / A.chunk));
-            with_bool(wl, [&](auto W) { with_tvd(s, [&](auto T) { with_bool(reduce, [&](auto Rd) {
-                launch_kernel(mc::k_lane<2, -1, 1, LW, decltype(W)::value, decltype(T)::value, decltype(Rd)::value>, grid, block, 0, st, A);
+            with_walls(wl, [&](auto W) { with_tvd(s, [&](auto T) { with_bool(reduce, [&](auto Rd) {
+                launch_kernel(mc::k_lane<2, -1, 1, LW, decltype(W)::value, decltype(T)::value, decltype(Rd)::value, LANE_MINB_2D>, grid, block, 0, st, A);
             }); }); });
         } else {
             return fail(MC_TVD_EINVAL, "a 2-D problem has no y-sweep");
@@ -212,22 +260,24 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
         dim3 block(32, WB, 1);
         long long xt = (nx + mc::LANE_OUT - 1) / mc::LANE_OUT;
         if (alpha == 2) {            // z-sweep: march z, tile (x, y)
+            constexpr int MW = MARCH3_WB, MO = MW - 2;
             A.n_b = ny; A.s_b = nx; A.n_m = nz; A.s_m = (long long)nx * ny;
-            long long bt = (ny + OB - 1) / OB;
+            long long bt = (ny + MO - 1) / MO;
             A.chunk = pick_chunk(s, nz, xt * bt);
-            dim3 grid((unsigned)xt, (unsigned)bt, (unsigned)((nz + A.chunk - 1) / A.chunk));
-            size_t smem = ((size_t)4 * 3 * 32 * WB + 4) * sizeof(double);
-            with_bool(wl, [&](auto W) { with_tvd(s, [&](auto T) {
-                launch_kernel(mc::k_march<3, 2, 1, 32, WB, decltype(W)::value, false, decltype(T)::value>, grid, block, smem, st, A);
+            dim3 mblock(32, MW, 1), grid((unsigned)xt, (unsigned)bt, (unsigned)((nz + A.chunk - 1) / A.chunk));
+            size_t smem = ((size_t)4 * 3 * 32 * (MW + 2) + 8) * sizeof(double);
+            with_walls(wl, [&](auto W) { with_tvd(s, [&](auto T) {
+                launch_kernel(mc::k_march3<2, 1, MW, decltype(W)::value, false, decltype(T)::value, MC_MARCH3_MINB>, grid, mblock, smem, st, A);
             }); });
         } else if (alpha == 1) {     // y-sweep: march y, tile (x, z)
+            constexpr int MW = MARCH3_WB, MO = MW - 2;
             A.n_b = nz; A.s_b = (long long)nx * ny; A.n_m = ny; A.s_m = nx;
-            long long bt = (nz + OB - 1) / OB;
+            long long bt = (nz + MO - 1) / MO;
             A.chunk = pick_chunk(s, ny, xt * bt);
-            dim3 grid((unsigned)xt, (unsigned)bt, (unsigned)((ny + A.chunk - 1) / A.chunk));
-            size_t smem = ((size_t)4 * 3 * 32 * WB + 4) * sizeof(double);
-            with_bool(wl, [&](auto W) { with_tvd(s, [&](auto T) {
-                launch_kernel(mc::k_march<3, 1, 2, 32, WB, false, decltype(W)::value, decltype(T)::value>, grid, block, smem, st, A);
+            dim3 mblock(32, MW, 1), grid((unsigned)xt, (unsigned)bt, (unsigned)((ny + A.chunk - 1) / A.chunk));
+            size_t smem = ((size_t)4 * 3 * 32 * (MW + 2) + 8) * sizeof(double);
+            with_walls(wl, [&](auto W) { with_tvd(s, [&](auto T) {
+                launch_kernel(mc::k_march3<1, 2, MW, false, decltype(W)::value, decltype(T)::value, MC_MARCH3_MINB>, grid, mblock, smem, st, A);
             }); });
         } else {                     // x-sweep: lanes x, tile (x, y), march z
             A.n_b = ny; A.s_b = nx; A.n_m = nz; A.s_m = (long long)nx * ny;
@@ -235,7 +285,7 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
             A.chunk = pick_chunk(s, nz, xt * bt);
             dim3 grid((unsigned)xt, (unsigned)bt, (unsigned)((nz + A.chunk - 1) / A.chunk));
             size_t smem = (size_t)4 * 2 * 32 * WB * sizeof(double);
-            with_bool(wl, [&](auto W) { with_tvd(s, [&](auto T) { with_bool(reduce, [&](auto Rd) {
+            with_walls(wl, [&](auto W) { with_tvd(s, [&](auto T) { with_bool(reduce, [&](auto Rd) {
                 launch_kernel(mc::k_lane<3, 1, 2, WB, decltype(W)::value, decltype(T)::value, decltype(Rd)::value>, grid, block, smem, st, A);
             }); }); });
         }

@@ -43,8 +43,8 @@ MC_DEV void shfl_down_vec(const double (&v)[NF], double (&r)[NF])
 // CB: velocity component of the tile's second direction b (y; -1 in 2-D); CM: component of the
 // marching direction m (z); WB: warps (rows) per block; WALL_M: m is z with plates; TVD: -1 / 0 / 1 as
 // in k_march; REDUCE: fold the CFL max-reduction of the output into the epilogue (R12).  alpha is x.
-template <int ND, int CB, int CM, int WB, bool WALL_M, int TVD, bool REDUCE>
-MC_KERNEL void __launch_bounds__(32 * WB, 1) k_lane(SweepArgs A)
+template <int ND, int CB, int CM, int WB, bool WALL_M, int TVD, bool REDUCE, int MINB = 1>
+MC_KERNEL void __launch_bounds__(32 * WB, MINB) k_lane(SweepArgs A)
 {
     constexpr int NF = ND + 2;
     constexpr bool HAS_B = (CB >= 0);

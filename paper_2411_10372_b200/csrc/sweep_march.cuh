@@ -32,8 +32,8 @@ enum { ROLE_NONE = 0, ROLE_R2 = 1, ROLE_WALLROW = 2, ROLE_R1 = 3, ROLE_IN = 4 };
 // CA: velocity component of alpha; CB: velocity component of the tile's second direction b (-1 in 2-D);
 // WX x WB: threads of a block (WB = 1 in 2-D); WALL_M / WALL_B: the marching / second direction is z
 // with plates; TVD: -1 no TVD term, 0 Eq. 34 as printed, 1 Davis/Yee (R4).
-template <int ND, int CA, int CB, int WX, int WB, bool WALL_M, bool WALL_B, int TVD>
-MC_KERNEL void __launch_bounds__(WX * WB, 1) k_march(SweepArgs A)
+template <int ND, int CA, int CB, int WX, int WB, bool WALL_M, bool WALL_B, int TVD, int MINB = 1>
+MC_KERNEL void __launch_bounds__(WX * WB, MINB) k_march(SweepArgs A)
 {
     constexpr int NF = ND + 2;
     constexpr bool HAS_B = (CB >= 0);

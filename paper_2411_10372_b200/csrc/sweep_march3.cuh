@@ -1,0 +1,407 @@
+// sweep_march3.cuh -- kernel k_march3: one operator L_alpha(tau) of Eqs. 31-39 in
+// 3-D for a sweep axis alpha that is NOT the fastest (x) axis: the z-sweep and the y-sweep.
+//
+// Design.  As in k_march (sweep_march.cuh, which serves the 2-D z-sweep) one
+// thread owns one grid column along alpha and MARCHES along it with every along-alpha neighbour in
+// registers; consecutive threads own consecutive x, so each global access is a coalesced row segment.
+// A block owns a tile of 32 x WB columns in (x, b): tile row = one warp, so a row's role is warp
+// uniform.  Rows 1 .. WB-2 are OUTPUT rows (role IN: the whole operator); rows 0 and WB-1 are the
+// ring-1 halo (role R1: predictor only, because the corrector flux of an output row differentiates
+// u^P across b, R7).  The ring-2 halo (the predictor of a ring-1 row differentiates u across b) needs
+// only the velocities of X, so the ring-1 warp computes them for its outer neighbour row as a side
+// job instead of parking two more warps on it: 12 of 14 warps do full work (28 x 12 outputs per 448
+// threads).  In x, lanes 0, 1, 30, 31 are the halo: they compute along and never store.
+// Velocities travel through shared memory, one plane per level, double buffered, ONE barrier per level.
+//
+// Pipeline of iteration j (output level j), identical to k_march:
+//   prefetch X(j+3) | W(j+2) -> TVD(j+1/2) -> F(j+1) -> P(j+1) | barrier | F^P(j+1) -> out(j)
+#pragma once
+#include <type_traits>
+
+#include "mc_common.cuh"
+#include "sweep_march.cuh"
+
+namespace mc {
+
+// CA: velocity component of alpha; CB: velocity component of the tile's second direction b;
+// WB: tile rows (warps) per block; WALL_M / WALL_B: the marching / second direction is z with plates;
+// TVD: -1 no TVD term, 0 Eq. 34 as printed, 1 Davis/Yee (R4).
+// Register budget: one block per SM, 65536 / (32 WB) registers per thread rounded down to a multiple of 8
+// (__launch_bounds__ alone rounds the block up to 512 threads and would give 128).
+#ifndef MC_MARCH3_L2PF
+#define MC_MARCH3_L2PF 4
+#endif
+#ifndef MC_MARCH3_LATE_LOAD
+#define MC_MARCH3_LATE_LOAD 0
+#endif
+#ifndef MC_MARCH3_SYNC
+#define MC_MARCH3_SYNC 0
+#endif
+#ifndef MC_MARCH3_REGS
+#define MC_MARCH3_REGS ((65536 / (32 * WB * MINB)) / 8 * 8)
+#endif
+template <int CA, int CB, int WB, bool WALL_M, bool WALL_B, int TVD, int MINB = 1>
+MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
+{
+    constexpr int ND = 3, NF = 5;
+    constexpr bool Z_IS_ALPHA = (CA == ND - 1);
+    constexpr int OB = WB - 2;                        // output rows per tile
+    static_assert(WB >= 3 && WB <= 16, "the progress flags occupy 64 bytes");
+    constexpr int TILE = 32 * (WB + 2);               // shared-memory plane: tile rows plus the ring-2 rows
+    MC_SHARED_DECL(double, smem_raw);
+    double *const smem = smem_raw + 8;                // 64 bytes in front: the rows' progress flags
+    double *const slotU = smem;                       // [2][ND][TILE]  velocities of X     (levels j+1, j+2)
+    double *const slotP = smem + 2 * ND * TILE;       // [2][ND][TILE]  velocities of X^P   (level j+1)
+
+    const int tx = threadIdx.x;
+    const int ty = threadIdx.y;
+    const int tidx = (ty + 1) * 32 + tx;
+
+    // ---- tile geometry --------------------------------------------------------------------
+    const int gx = (int)blockIdx.x * 28 + tx - 2;
+    const int ix = wrap1(gx, A.nx);                   // nx >= 4 (mc_tvd_init) and gx in [-2, nx + 32)
+    const int rx = min(tx, 31 - tx);
+    const bool edge = (ty == 0 || ty == WB - 1);
+    const int gb_raw = (int)blockIdx.y * OB + ty - 1;
+    const int go_raw = gb_raw + (ty == 0 ? -1 : 1);   // the ring-2 row beyond an edge row
+    bool row_exists = true, wallrow = false, has_outer = edge;
+    int gb, go;
+    if (WALL_B) {
+        row_exists = (gb_raw >= 0 && gb_raw < A.n_b);
+        wallrow = (gb_raw == 0 || gb_raw == A.n_b - 1);
+        gb = row_exists ? gb_raw : 0;
+        has_outer = edge && row_exists && !wallrow && go_raw >= 0 && go_raw < A.n_b;
+        go = has_outer ? go_raw : 0;
+    } else {
+        gb = wrap1(gb_raw, A.n_b);                    // periodic b: the node's own index
+        go = wrap1(go_raw, A.n_b);
+    }
+    const long long col = ix + (long long)gb * A.s_b;
+    const long long col_o = ix + (long long)go * A.s_b;
+    const int tidx_o = tidx + (ty == 0 ? -32 : 32);
+    const bool owner = row_exists && rx >= 2 && !edge && gx < A.nx && gb_raw < A.n_b;
+    int role = ROLE_IN;
+    if (!row_exists) role = ROLE_NONE;
+    else if (wallrow) role = ROLE_WALLROW;
+    else if (edge) role = ROLE_R1;
+
+    // ---- sweep constants ------------------------------------------------------------------
+    const double tau = A.dt_ptr ? 0.5 * (*A.dt_ptr) : A.tau_fixed;
+    const double cdt = tau * A.inv_h;                 // tau / dx_alpha of Eqs. 31-32, signed
+    const double hcdt = 0.5 * cdt;
+    const double half_tod = 0.5 * tau / A.d_a;        // for Co (R5)
+    const double tsrc = A.src ? -(tau * A.g) : 0.0;   // tau S: S = -g rho in the rho u_z row
+    const int n = A.n_m;
+    const int l0 = (int)blockIdx.z * A.chunk;
+    const int l1 = min(n, l0 + A.chunk);
+    const long long sm_signed = (A.dir > 0) ? A.s_m : -A.s_m;
+    const long long org = (A.dir > 0) ? 0 : (long long)(n - 1) * A.s_m;
+    const double *const pin = A.in + col + org;
+    const double *const pin_o = A.in + col_o + org;
+    double *const pout = A.out + col + org;
+    const double gz_fixed = A.g * ((double)gb * A.dz);                       // used when b is z
+
+    auto exists = [&](int l) { return WALL_M ? (l >= 0 && l < n) : true; };
+    auto lev = [&](int l) { return WALL_M ? l : wrap1(l, n); };              // l in [-n, 2n)
+    auto gz_of = [&](int l) {                         // g z_k of Eq. 17 for this thread's node at level l
+        if (!Z_IS_ALPHA) return gz_fixed;
+        const int w = lev(l);
+        return A.g * ((double)((A.dir > 0) ? w : n - 1 - w) * A.dz);
+    };
+    auto load = [&](int l, double (&X)[NF]) {
+        const double *p = pin + (long long)lev(l) * sm_signed;
+#pragma unroll
+        for (int f = 0; f < NF; ++f) X[f] = p[(long long)f * A.N];
+    };
+    // L2 prefetch of the thread's node at level l (no register, no scoreboard): hides the HBM latency
+    // the one-level register prefetch cannot cover with 12 warps per SM
+    auto prefetch_l2 = [&](int l) {
+        const double *p = pin + (long long)lev(l) * sm_signed;
+#pragma unroll
+        for (int f = 0; f < NF; ++f) asm volatile("prefetch.global.L2 [%0];" ::"l"(p + (long long)f * A.N));
+    };
+    auto load_outer = [&](int l, double (&X)[ND + 1]) {                      // rho and the momenta only
+        const double *p = pin_o + (long long)lev(l) * sm_signed;
+#pragma unroll
+        for (int f = 0; f <= ND; ++f) X[f] = p[(long long)f * A.N];
+    };
+    auto store = [&](int l, const double (&o)[NF]) {
+        double *q = pout + (long long)lev(l) * sm_signed;
+#pragma unroll
+        for (int f = 0; f < NF; ++f) q[(long long)f * A.N] = o[f];
+    };
+    auto publish = [&](double *slot, int parity, int at, const double (&u)[ND]) {
+#pragma unroll
+        for (int c = 0; c < ND; ++c) slot[(parity * ND + c) * TILE + at] = u[c];
+    };
+    // central cross DIFFERENCES of the velocities published in `slot` (R7)
+    auto cross = [&](const double *slot, int parity, double (&dxa)[ND], double (&dxc)[ND]) {
+        const double *s = slot + parity * ND * TILE + tidx;
+#pragma unroll
+        for (int c = 0; c < ND; ++c) { dxa[c] = 0.0; dxc[c] = 0.0; }
+        dxa[0] = s[CA * TILE + 1] - s[CA * TILE - 1];
+        dxc[0] = s[1] - s[-1];
+        dxa[CB] = s[CA * TILE + 32] - s[CA * TILE - 32];
+        dxc[CB] = s[CB * TILE + 32] - s[CB * TILE - 32];
+    };
+    // plate values of a node on a plate of the marching direction: no slip,
+    // T = T_w; only rho is free (R10)
+    auto plate = [&](int l, double rho, double (&X)[NF]) {
+        const int k = (A.dir > 0) ? l : n - 1 - l;
+        const double Tw = (k == 0) ? A.Tw0 : A.Tw1;
+        X[0] = rho;
+#pragma unroll
+        for (int c = 0; c < ND; ++c) X[1 + c] = 0.0;
+        X[NF - 1] = rho * (A.cv * Tw + A.g * ((double)k * A.dz));
+    };
+
+    auto uslot = [&](int L) { return L & 1; };
+
+    // ---- per-level synchronisation ---------------------------------------------------------------
+    // A row exchanges velocities only with its two neighbour rows, so instead of a block-wide barrier
+    // each warp publishes "my planes of iteration j are written" in a shared flag (release) and waits
+    // for the flags of its two neighbour rows (acquire): rows drift apart instead of all waiting for
+    // the slowest one each level.  Slot reuse is safe with two planes per slot: a row that has passed
+    // the wait of iteration j-1 knows its neighbours finished every read of iteration j-2.
+    int *const flags = reinterpret_cast<int *>(smem_raw);           // [WB] ints in the 16 pad bytes..
+    const bool nb_lo = MC_MARCH3_SYNC && ty > 0 && (!WALL_B || (gb_raw - 1 >= 0 && gb_raw - 1 < A.n_b));
+    const bool nb_hi = MC_MARCH3_SYNC && ty < WB - 1 && (!WALL_B || (gb_raw + 1 >= 0 && gb_raw + 1 < A.n_b));
+    const unsigned flag_me = (unsigned)__cvta_generic_to_shared(flags + ty);
+    if (MC_MARCH3_SYNC) {
+        if (tx == 0) flags[ty] = l0 - 5;
+        __syncthreads();
+    }
+    auto level_sync = [&](int j) {
+        if (!MC_MARCH3_SYNC) { __syncthreads(); return; }
+        __syncwarp();
+        if (tx == 0) asm volatile("st.release.cta.shared.b32 [%0], %1;" ::"r"(flag_me), "r"(j) : "memory");
+        int v;
+        if (nb_lo) do { asm volatile("ld.acquire.cta.shared.b32 %0, [%1];" : "=r"(v) : "r"(flag_me - 4) : "memory"); } while (v < j);
+        if (nb_hi) do { asm volatile("ld.acquire.cta.shared.b32 %0, [%1];" : "=r"(v) : "r"(flag_me + 4) : "memory"); } while (v < j);
+        __syncwarp();
+    };
+
+    // ---- carried state (levels relative to the current output level j) -------------------------
+    double Xn[NF];                 // X(j+2)
+    double Xc[NF];                 // X(j+1)
+    double Xon[ND + 1];            // rho, m of the outer (ring-2) row at the level W works on next (ring-1 rows only)
+    double F0[NF];                 // F(j)
+    double H0[NF];                 // (X^P + X)/2 + tau S^P/2 - Dh_{j-1/2} + (tau/2dx) F^P(j) of level j (fast levels;
+    double FP0m = 0.0;             //  F^P(j) mass flux, kept apart for the plate closure, R10)
+    double d0[NF];                 // dX_{j+1/2}
+    double uP0[ND], TP0 = 1.0;     // u, T of X^P(j)
+    double a0 = 0.0, b0 = 0.0;     // (dX_{j-1/2}, dX_{j+1/2}), |dX_{j+1/2}|^2
+    double hC0 = 0.0, hC1 = 0.0;   // C/2 of Eq. 39 at levels j, j+1
+    double gz1 = 0.0;              // g z of level j+1
+    Prim<ND> w1;                   // primitives of X(j+1)
+#pragma unroll
+    for (int f = 0; f < NF; ++f) { Xn[f] = 0.0; Xc[f] = 0.0; F0[f] = 0.0; H0[f] = 0.0; d0[f] = 0.0; }
+    Xn[0] = 1.0; Xc[0] = 1.0;
+#pragma unroll
+    for (int f = 0; f <= ND; ++f) Xon[f] = (f == 0) ? 1.0 : 0.0;
+#pragma unroll
+    for (int c = 0; c < ND; ++c) { uP0[c] = 0.0; w1.u[c] = 0.0; }
+    w1.T = 1.0; w1.p = 0.0;
+
+    // W(L): primitives of X(L) (in `X`), Courant coefficient, velocities published into slot uslot(L);
+    // a ring-1 row also publishes the velocities of its ring-2 neighbour row (from `Xo`).
+    auto stage_W = [&](auto role_tag, int L, const double (&X)[NF], const double (&Xo)[ND + 1], Prim<ND> &w,
+                       double &hC, double &gz) {
+        constexpr int ROLE = decltype(role_tag)::value;
+        gz = gz_of(L);
+        w = primitives<ND>(X, gz, A);
+        if (ROLE == ROLE_IN && TVD >= 0) hC = half_courant_coef(w.u[CA], w.T, half_tod, A);
+        publish(slotU, uslot(L), tidx, w.u);
+        if (ROLE == ROLE_R1) {
+            const double inv = rcp(Xo[0]);
+            double uo[ND];
+#pragma unroll
+            for (int c = 0; c < ND; ++c) uo[c] = Xo[1 + c] * inv;
+            publish(slotU, uslot(L), tidx_o, uo);
+        }
+    };
+
+    // One iteration.  ROLE and FAST are compile-time tags.
+    auto body = [&](auto role_tag, auto fast_tag, const int j) {
+        constexpr int ROLE = decltype(role_tag)::value;
+        constexpr bool FAST = decltype(fast_tag)::value;
+        const int p1 = (j + 1) & 1;                              // parity of level j+1 (slotP)
+        const bool ex1 = FAST || exists(j + 1), ex2 = FAST || exists(j + 2), ex3 = FAST || exists(j + 3);
+        const bool ld1 = FAST || (ex1 && (j + 1 >= l0 - 2));     // level j+1 is loaded (Xc, w1 valid)
+        const bool ld2 = ex2;
+        const bool start_wall1 = !FAST && WALL_M && (j + 1 == 0);     // level j+1 is the plate the march starts on
+        const bool end_wall1 = !FAST && WALL_M && (j + 1 == n - 1);   // level j+1 is the plate the march ends on
+
+        if (ROLE == ROLE_NONE) { if (!MC_MARCH3_SYNC) __syncthreads(); return; }
+
+        // (0) prefetch X(j+3): far ahead into L2 here, into registers after the barrier (the loads then
+        // do not overlap the register peak of the flux / predictor stages)
+        const bool ld3 = FAST || (ex3 && j + 3 <= l1 + 1);
+#if MC_MARCH3_L2PF > 0
+        if (j + 3 + MC_MARCH3_L2PF <= l1 + 1 && exists(j + 3 + MC_MARCH3_L2PF)) prefetch_l2(j + 3 + MC_MARCH3_L2PF);
+#endif
+        double Xq[NF], Xoq[ND + 1];
+        auto fetch = [&]() {
+#pragma unroll
+            for (int f = 0; f < NF; ++f) Xq[f] = Xn[f];
+            if (ld3) load(j + 3, Xq);
+#pragma unroll
+            for (int f = 0; f <= ND; ++f) Xoq[f] = Xon[f];
+            if (ROLE == ROLE_R1 && ld3 && has_outer) load_outer(j + 3, Xoq);
+        };
+        if (MC_MARCH3_LATE_LOAD == 0 || ROLE != ROLE_IN) fetch();
+
+        // (1) W(j+2)
+        Prim<ND> w2 = w1;
+        double hC2 = 0.0, gz2 = 0.0;
+        if (ld2) stage_W(role_tag, j + 2, Xn, Xon, w2, hC2, gz2);
+
+        if (ROLE == ROLE_WALLROW) {
+            // a plate row of b (y-sweep): X^P = X and the output is X (R10); publish u^P = u of level j+1
+            if (ld1) publish(slotP, p1, tidx, w1.u);
+            level_sync(j);
+            if (j >= l0 && owner) store(j, H0);
+#pragma unroll
+            for (int f = 0; f < NF; ++f) { H0[f] = Xc[f]; Xc[f] = Xn[f]; Xn[f] = Xq[f]; }
+            w1 = w2;
+            return;
+        }
+
+        // (2) TVD (Eqs. 34-39): Dh_{j+1/2} from dX_{j-1/2}, dX_{j+1/2}, dX_{j+3/2}
+        double d1[NF], Dh[NF], a1 = 0.0, b1 = 0.0;
+#pragma unroll
+        for (int f = 0; f < NF; ++f) { Dh[f] = 0.0; d1[f] = 0.0; }
+        if (ROLE == ROLE_IN && TVD >= 0) {
+#pragma unroll
+            for (int f = 0; f < NF; ++f) d1[f] = (ld1 && ld2) ? Xn[f] - Xc[f] : 0.0;
+#pragma unroll
+            for (int f = 0; f < NF; ++f) { b1 = fma(d1[f], d1[f], b1); a1 = fma(d0[f], d1[f], a1); }
+            const bool have = FAST || ((j >= l0 - 1) && exists(j - 1) && exists(j) && ex1 && ex2);   // R11 at plates
+            if (have) {
+                const double coef = tvd_coef<(TVD >= 0 ? TVD : 0)>(a0, a1, b0, hC0, hC1);
+#pragma unroll
+                for (int f = 0; f < NF; ++f) { Dh[f] = coef * d0[f]; H0[f] += Dh[f]; }
+            }
+        }
+
+        // (3) F(j+1): flux of X at level j+1 (inner derivative forward in marching coordinates)
+        double F1[NF], XP[NF], H1[NF];
+        Prim<ND> wP1 = w1;
+#pragma unroll
+        for (int f = 0; f < NF; ++f) { F1[f] = 0.0; XP[f] = Xc[f]; H1[f] = Xc[f]; }
+        const bool doF = ld1;
+        if (doF) {
+            if (end_wall1) {
+                F1[0] = Xc[1 + CA];                   // only the mass flux is defined and needed (R10)
+            } else {
+                double du[ND], dxa[ND], dxc[ND];
+#pragma unroll
+                for (int c = 0; c < ND; ++c) du[c] = w2.u[c] - w1.u[c];
+                cross(slotU, uslot(j + 1), dxa, dxc);
+                flux<ND, CA>(Xc, w1, du, w2.T - w1.T, dxa, dxc, A, F1);
+            }
+        }
+        // (4) P(j+1): predictor (Eq. 31), plate values, primitives of X^P, publish
+        const bool doP = FAST || (doF && (j + 1 >= l0 - 1));
+        if (doP) {
+            if (start_wall1) {
+                plate(j + 1, Xc[0], XP);                                      // rho unchanged
+            } else if (end_wall1) {
+                plate(j + 1, Xc[0] - 2.0 * cdt * (F1[0] - F0[0]), XP);       // half-cell closure (R10)
+            } else {
+#pragma unroll
+                for (int f = 0; f < NF; ++f) {
+                    const double dF = F1[f] - F0[f];
+                    XP[f] = fma(-cdt, dF, Xc[f]);
+                    H1[f] = fma(-hcdt, dF, Xc[f]) - Dh[f];                    // (X^P + X)/2 - Dh
+                }
+                XP[1 + CA] = fma(tsrc, Xc[0], XP[1 + CA]);
+                H1[1 + CA] = fma(0.5 * tsrc, Xc[0], H1[1 + CA]);
+            }
+            wP1 = primitives<ND>(XP, gz1, A);
+            if (start_wall1 || end_wall1) {
+#pragma unroll
+                for (int f = 0; f < NF; ++f) H1[f] = 0.5 * (XP[f] + Xc[f]);
+            } else {
+                H1[1 + CA] = fma(0.5 * tsrc, XP[0], H1[1 + CA]);             // + tau S(X^P)/2
+            }
+        }
+        if (ld1) publish(slotP, p1, tidx, wP1.u);
+
+        level_sync(j);
+        if (MC_MARCH3_LATE_LOAD != 0 && ROLE == ROLE_IN) fetch();
+
+        if (ROLE == ROLE_IN) {
+            // (5) F^P(j+1): flux of X^P at level j+1 (inner derivative backward in marching coordinates)
+            double FP1[NF];
+#pragma unroll
+            for (int f = 0; f < NF; ++f) FP1[f] = 0.0;
+            const bool doFP = FAST || (doP && (j + 1 >= l0));
+            if (doFP) {
+                if (start_wall1) {
+                    FP1[0] = XP[1 + CA];
+                } else {
+                    double du[ND], dxa[ND], dxc[ND];
+#pragma unroll
+                    for (int c = 0; c < ND; ++c) du[c] = wP1.u[c] - uP0[c];
+                    cross(slotP, p1, dxa, dxc);
+                    flux<ND, CA>(XP, wP1, du, wP1.T - TP0, dxa, dxc, A, FP1);
+                }
+            }
+            // (6) out(j): corrector (Eq. 32), average and TVD term (Eq. 33), plate values.  H0 already
+            // holds + (tau/2dx) F^P(j), folded in when F^P(j) was computed.
+            if (FAST || (j >= l0 && exists(j))) {
+                double o[NF];
+                if (!FAST && WALL_M && j == 0) {
+                    plate(j, H0[0] - hcdt * FP0m - cdt * (FP1[0] - FP0m), o); // 0.5 * (2 tau/dz) * dF
+                } else if (!FAST && WALL_M && j == n - 1) {
+                    plate(j, H0[0] - hcdt * FP0m, o);
+                } else {
+#pragma unroll
+                    for (int f = 0; f < NF; ++f) o[f] = fma(-hcdt, FP1[f], H0[f]);
+                }
+                if (owner) store(j, o);
+            }
+            FP0m = FP1[0];
+#pragma unroll
+            for (int f = 0; f < NF; ++f) { H1[f] = fma(hcdt, FP1[f], H1[f]); d0[f] = d1[f]; }
+            a0 = a1; b0 = b1; hC0 = hC1; hC1 = hC2;
+#pragma unroll
+            for (int c = 0; c < ND; ++c) uP0[c] = wP1.u[c];
+            TP0 = wP1.T;
+        }
+        // (7) rotate the pipeline
+#pragma unroll
+        for (int f = 0; f < NF; ++f) { Xc[f] = Xn[f]; Xn[f] = Xq[f]; F0[f] = F1[f]; H0[f] = H1[f]; }
+#pragma unroll
+        for (int f = 0; f <= ND; ++f) Xon[f] = Xoq[f];
+        w1 = w2; gz1 = gz2;
+    };
+
+    // ---- the march -------------------------------------------------------------------------------
+    auto march = [&](auto role_tag) {
+        using std::integral_constant;
+        constexpr int ROLE = decltype(role_tag)::value;
+        integral_constant<bool, false> slow;
+        integral_constant<bool, true> fast;
+        int j = l0 - 4;
+        if (exists(j + 2)) {
+            load(j + 2, Xn);
+            if (ROLE == ROLE_R1 && has_outer) load_outer(j + 2, Xon);
+        }
+        const int jf0 = WALL_M ? max(l0, 1) : l0;
+        const int jf1 = WALL_M ? min(l1, n - 3) : l1;
+        for (; j < l1 && j < jf0; ++j) body(role_tag, slow, j);
+#pragma unroll 2
+        for (; j < jf1; ++j) body(role_tag, fast, j);
+        for (; j < l1; ++j) body(role_tag, slow, j);
+    };
+    switch (role) {
+    case ROLE_NONE: march(std::integral_constant<int, ROLE_NONE>()); break;
+    case ROLE_WALLROW: march(std::integral_constant<int, WALL_B ? ROLE_WALLROW : ROLE_IN>()); break;
+    case ROLE_R1: march(std::integral_constant<int, ROLE_R1>()); break;
+    default: march(std::integral_constant<int, ROLE_IN>()); break;
+    }
+}
+
+}  // namespace mc
