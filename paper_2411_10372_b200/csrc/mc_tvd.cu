@@ -14,6 +14,7 @@
 #include "mc_common.cuh"
 #include "reduce_kernels.cuh"
 #include "sweep_lane.cuh"
+#include "sweep_lane3.cuh"
 #include "sweep_march.cuh"
 #include "sweep_march3.cuh"
 
@@ -36,14 +37,14 @@ size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 #ifndef MC_MARCH_MINB_2D
 #define MC_MARCH_MINB_2D 4
 #endif
-#ifndef MC_TILE_WB_3D
-#define MC_TILE_WB_3D 12
-#endif
 #ifndef MC_MARCH3_WB
 #define MC_MARCH3_WB 12
 #endif
 #ifndef MC_MARCH3_MINB
 #define MC_MARCH3_MINB 1
+#endif
+#ifndef MC_LANE3_WB
+#define MC_LANE3_WB 12
 #endif
 #ifndef MC_LANE_WARPS_2D
 #define MC_LANE_WARPS_2D 4
@@ -53,8 +54,8 @@ size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 #endif
 constexpr int MARCH_WX_2D = MC_MARCH_WX_2D;      // k_march, 2-D: WX - 4 outputs per block row
 constexpr int MARCH_MINB_2D = MC_MARCH_MINB_2D;  // k_march, 2-D: resident blocks per SM the register budget allows
-constexpr int TILE_WB_3D = MC_TILE_WB_3D;        // 3-D tiles: 32 x WB threads, 28 x (WB - 4) outputs (register-limited)
 constexpr int MARCH3_WB = MC_MARCH3_WB;          // k_march3: 32 x WB threads, 28 x (WB - 2) outputs
+constexpr int LANE3_WB = MC_LANE3_WB;            // k_lane3: 32 x WB threads, 28 x (WB - 2) outputs
 constexpr int LANE_WARPS_2D = MC_LANE_WARPS_2D;  // k_lane, 2-D: independent warps per block
 constexpr int LANE_MINB_2D = MC_LANE_MINB_2D;
 constexpr int DIAG_MAX_BLOCKS = 64;    // blocks per plane in the diagnostics pass
@@ -101,6 +102,10 @@ bool valid_problem(const mc_tvd_grid *g, const mc_tvd_params *p, int *code)
     if (g->ndim == 2 && g->ny != 1) return fail(0, "ny must be 1 in 2-D"), false;
     if (g->ndim == 3 && g->ny < 4) return fail(0, "need ny >= 4 in 3-D"), false;
     if (!(g->lx > 0) || !(g->lz > 0) || (g->ndim == 3 && !(g->ly > 0))) return fail(0, "box size must be > 0"), false;
+    if ((long long)g->nx * g->ny * g->nz >= (1ll << 32)) {
+        *code = MC_TVD_EUNSUPPORTED;
+        return fail(0, "more than 2^32 - 1 nodes per field: the kernels index nodes with 32 bits"), false;
+    }
     if (g->z_nodes) { *code = MC_TVD_EUNSUPPORTED; return fail(0, "non-uniform z grid is not built (SURVEY 8f)"), false; }
     if (!(p->gamma > 1) || !(p->eps > 0) || !(p->D > 0) || !(p->Pr > 0) || !(p->Ra > 0))
         return fail(0, "need gamma > 1 and eps, D, Pr, Ra > 0"), false;
@@ -256,8 +261,6 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
             return fail(MC_TVD_EINVAL, "a 2-D problem has no y-sweep");
         }
     } else {
-        constexpr int WB = TILE_WB_3D, OB = WB - 4;
-        dim3 block(32, WB, 1);
         long long xt = (nx + mc::LANE_OUT - 1) / mc::LANE_OUT;
         if (alpha == 2) {            // z-sweep: march z, tile (x, y)
             constexpr int MW = MARCH3_WB, MO = MW - 2;
@@ -280,13 +283,14 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
                 launch_kernel(mc::k_march3<1, 2, MW, false, decltype(W)::value, decltype(T)::value, MC_MARCH3_MINB>, grid, mblock, smem, st, A);
             }); });
         } else {                     // x-sweep: lanes x, tile (x, y), march z
+            constexpr int LW = LANE3_WB, LO = LW - 2;
             A.n_b = ny; A.s_b = nx; A.n_m = nz; A.s_m = (long long)nx * ny;
-            long long bt = (ny + OB - 1) / OB;
+            long long bt = (ny + LO - 1) / LO;
             A.chunk = pick_chunk(s, nz, xt * bt);
-            dim3 grid((unsigned)xt, (unsigned)bt, (unsigned)((nz + A.chunk - 1) / A.chunk));
-            size_t smem = (size_t)4 * 2 * 32 * WB * sizeof(double);
+            dim3 lblock(32, LW, 1), grid((unsigned)xt, (unsigned)bt, (unsigned)((nz + A.chunk - 1) / A.chunk));
+            size_t smem = (size_t)4 * 2 * 32 * (LW + 2) * sizeof(double);
             with_walls(wl, [&](auto W) { with_tvd(s, [&](auto T) { with_bool(reduce, [&](auto Rd) {
-                launch_kernel(mc::k_lane<3, 1, 2, WB, decltype(W)::value, decltype(T)::value, decltype(Rd)::value>, grid, block, smem, st, A);
+                launch_kernel(mc::k_lane3<1, 2, LW, decltype(W)::value, decltype(T)::value, decltype(Rd)::value>, grid, lblock, smem, st, A);
             }); }); });
         }
     }

@@ -94,41 +94,46 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
     const int n = A.n_m;
     const int l0 = (int)blockIdx.z * A.chunk;
     const int l1 = min(n, l0 + A.chunk);
-    const long long sm_signed = (A.dir > 0) ? A.s_m : -A.s_m;
+    // Node offsets inside a field are 32-bit element counts (N < 2^32, mc_tvd_init) in modular arithmetic;
+    // the field bases A.in + f N are block uniform, so an address costs one IMAD.WIDE.
+    const unsigned sms = (unsigned)(int)((A.dir > 0) ? A.s_m : -A.s_m);
     const long long org = (A.dir > 0) ? 0 : (long long)(n - 1) * A.s_m;
-    const double *const pin = A.in + col + org;
-    const double *const pin_o = A.in + col_o + org;
-    double *const pout = A.out + col + org;
+    const unsigned off_base = (unsigned)(col + org);
+    const unsigned off_base_o = (unsigned)(col_o + org);
+    const double dsgn = (A.dir > 0) ? 1.0 : -1.0;
+    const int pf_last = min(l1 + 1, n - 1) - MC_MARCH3_L2PF;                // last j + 3 whose L2 prefetch is issued
     const double gz_fixed = A.g * ((double)gb * A.dz);                       // used when b is z
 
     auto exists = [&](int l) { return WALL_M ? (l >= 0 && l < n) : true; };
     auto lev = [&](int l) { return WALL_M ? l : wrap1(l, n); };              // l in [-n, 2n)
+    const double *inb[NF];
+    double *outb[NF];
+#pragma unroll
+    for (int f = 0; f < NF; ++f) { inb[f] = A.in + (long long)f * A.N; outb[f] = A.out + (long long)f * A.N; }
+    auto off_of = [&](int l) { return off_base + (unsigned)lev(l) * sms; };
+    auto phys_k = [&](int l) { const int w = lev(l); return (A.dir > 0) ? w : n - 1 - w; };
+    auto load_at = [&](unsigned o, double (&X)[NF]) {
+#pragma unroll
+        for (int f = 0; f < NF; ++f) X[f] = inb[f][o];
+    };
+    auto load = [&](int l, double (&X)[NF]) { load_at(off_of(l), X); };
     auto gz_of = [&](int l) {                         // g z_k of Eq. 17 for this thread's node at level l
         if (!Z_IS_ALPHA) return gz_fixed;
-        const int w = lev(l);
-        return A.g * ((double)((A.dir > 0) ? w : n - 1 - w) * A.dz);
-    };
-    auto load = [&](int l, double (&X)[NF]) {
-        const double *p = pin + (long long)lev(l) * sm_signed;
-#pragma unroll
-        for (int f = 0; f < NF; ++f) X[f] = p[(long long)f * A.N];
+        return A.g * ((double)phys_k(l) * A.dz);
     };
     // L2 prefetch of the thread's node at level l (no register, no scoreboard): hides the HBM latency
     // the one-level register prefetch cannot cover with 12 warps per SM
-    auto prefetch_l2 = [&](int l) {
-        const double *p = pin + (long long)lev(l) * sm_signed;
+    auto prefetch_l2 = [&](unsigned o) {
 #pragma unroll
-        for (int f = 0; f < NF; ++f) asm volatile("prefetch.global.L2 [%0];" ::"l"(p + (long long)f * A.N));
+        for (int f = 0; f < NF; ++f) asm volatile("prefetch.global.L2 [%0];" ::"l"(inb[f] + o));
     };
-    auto load_outer = [&](int l, double (&X)[ND + 1]) {                      // rho and the momenta only
-        const double *p = pin_o + (long long)lev(l) * sm_signed;
+    auto load_outer = [&](unsigned o, double (&X)[ND + 1]) {                 // rho and the momenta only
 #pragma unroll
-        for (int f = 0; f <= ND; ++f) X[f] = p[(long long)f * A.N];
+        for (int f = 0; f <= ND; ++f) X[f] = inb[f][o];
     };
-    auto store = [&](int l, const double (&o)[NF]) {
-        double *q = pout + (long long)lev(l) * sm_signed;
+    auto store_at = [&](unsigned o, const double (&v)[NF]) {
 #pragma unroll
-        for (int f = 0; f < NF; ++f) q[(long long)f * A.N] = o[f];
+        for (int f = 0; f < NF; ++f) outb[f][o] = v[f];
     };
     auto publish = [&](double *slot, int parity, int at, const double (&u)[ND]) {
 #pragma unroll
@@ -155,7 +160,6 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
         X[NF - 1] = rho * (A.cv * Tw + A.g * ((double)k * A.dz));
     };
 
-    auto uslot = [&](int L) { return L & 1; };
 
     // ---- per-level synchronisation ---------------------------------------------------------------
     // A row exchanges velocities only with its two neighbour rows, so instead of a block-wide barrier
@@ -194,6 +198,10 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
     double hC0 = 0.0, hC1 = 0.0;   // C/2 of Eq. 39 at levels j, j+1
     double gz1 = 0.0;              // g z of level j+1
     Prim<ND> w1;                   // primitives of X(j+1)
+    // fast levels only: node offsets of level j+3 (next load) and level j (next store), and the
+    // z index of level j+2 as a double (exact; saves the int-to-double conversions of g z_k)
+    unsigned o3c = 0, o0c = 0;
+    double kd2c = 0.0;
 #pragma unroll
     for (int f = 0; f < NF; ++f) { Xn[f] = 0.0; Xc[f] = 0.0; F0[f] = 0.0; H0[f] = 0.0; d0[f] = 0.0; }
     Xn[0] = 1.0; Xc[0] = 1.0;
@@ -205,27 +213,31 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
 
     // W(L): primitives of X(L) (in `X`), Courant coefficient, velocities published into slot uslot(L);
     // a ring-1 row also publishes the velocities of its ring-2 neighbour row (from `Xo`).
-    auto stage_W = [&](auto role_tag, int L, const double (&X)[NF], const double (&Xo)[ND + 1], Prim<ND> &w,
-                       double &hC, double &gz) {
+    auto stage_W = [&](auto role_tag, int par, double gz, const double (&X)[NF], const double (&Xo)[ND + 1],
+                       Prim<ND> &w, double &hC) {
         constexpr int ROLE = decltype(role_tag)::value;
-        gz = gz_of(L);
         w = primitives<ND>(X, gz, A);
         if (ROLE == ROLE_IN && TVD >= 0) hC = half_courant_coef(w.u[CA], w.T, half_tod, A);
-        publish(slotU, uslot(L), tidx, w.u);
+        publish(slotU, par, tidx, w.u);
         if (ROLE == ROLE_R1) {
             const double inv = rcp(Xo[0]);
             double uo[ND];
 #pragma unroll
             for (int c = 0; c < ND; ++c) uo[c] = Xo[1 + c] * inv;
-            publish(slotU, uslot(L), tidx_o, uo);
+            publish(slotU, par, tidx_o, uo);
         }
     };
 
-    // One iteration.  ROLE and FAST are compile-time tags.
-    auto body = [&](auto role_tag, auto fast_tag, const int j) {
+    // One iteration.  ROLE and FAST are compile-time tags; PAR is the compile-time parity of j in the
+    // unrolled FAST pair (-1: take it from j).
+    auto body = [&](auto role_tag, auto fast_tag, auto par_tag, const int j) {
         constexpr int ROLE = decltype(role_tag)::value;
         constexpr bool FAST = decltype(fast_tag)::value;
-        const int p1 = (j + 1) & 1;                              // parity of level j+1 (slotP)
+        constexpr int PAR = decltype(par_tag)::value;
+        const int p1 = (PAR >= 0) ? (PAR ^ 1) : ((j + 1) & 1);   // parity of level j+1
+        const int p2 = p1 ^ 1;                                   // parity of level j+2
+        const unsigned o3 = FAST ? o3c : off_of(j + 3);
+        const unsigned o0 = FAST ? o0c : off_of(j);
         const bool ex1 = FAST || exists(j + 1), ex2 = FAST || exists(j + 2), ex3 = FAST || exists(j + 3);
         const bool ld1 = FAST || (ex1 && (j + 1 >= l0 - 2));     // level j+1 is loaded (Xc, w1 valid)
         const bool ld2 = ex2;
@@ -238,32 +250,37 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
         // do not overlap the register peak of the flux / predictor stages)
         const bool ld3 = FAST || (ex3 && j + 3 <= l1 + 1);
 #if MC_MARCH3_L2PF > 0
-        if (j + 3 + MC_MARCH3_L2PF <= l1 + 1 && exists(j + 3 + MC_MARCH3_L2PF)) prefetch_l2(j + 3 + MC_MARCH3_L2PF);
+        if (FAST) { if (j + 3 <= pf_last) prefetch_l2(o3 + (unsigned)MC_MARCH3_L2PF * sms); }
+        else if (j + 3 + MC_MARCH3_L2PF <= l1 + 1 && exists(j + 3 + MC_MARCH3_L2PF)) prefetch_l2(off_of(j + 3 + MC_MARCH3_L2PF));
 #endif
         double Xq[NF], Xoq[ND + 1];
         auto fetch = [&]() {
 #pragma unroll
             for (int f = 0; f < NF; ++f) Xq[f] = Xn[f];
-            if (ld3) load(j + 3, Xq);
+            if (ld3) load_at(o3, Xq);
 #pragma unroll
             for (int f = 0; f <= ND; ++f) Xoq[f] = Xon[f];
-            if (ROLE == ROLE_R1 && ld3 && has_outer) load_outer(j + 3, Xoq);
+            if (ROLE == ROLE_R1 && ld3 && has_outer) load_outer(o3 - off_base + off_base_o, Xoq);
         };
         if (MC_MARCH3_LATE_LOAD == 0 || ROLE != ROLE_IN) fetch();
 
         // (1) W(j+2)
         Prim<ND> w2 = w1;
         double hC2 = 0.0, gz2 = 0.0;
-        if (ld2) stage_W(role_tag, j + 2, Xn, Xon, w2, hC2, gz2);
+        if (ld2) {
+            gz2 = (FAST && Z_IS_ALPHA) ? A.g * (kd2c * A.dz) : gz_of(j + 2);
+            stage_W(role_tag, p2, gz2, Xn, Xon, w2, hC2);
+        }
 
         if (ROLE == ROLE_WALLROW) {
             // a plate row of b (y-sweep): X^P = X and the output is X (R10); publish u^P = u of level j+1
             if (ld1) publish(slotP, p1, tidx, w1.u);
             level_sync(j);
-            if (j >= l0 && owner) store(j, H0);
+            if (j >= l0 && owner) store_at(o0, H0);
 #pragma unroll
             for (int f = 0; f < NF; ++f) { H0[f] = Xc[f]; Xc[f] = Xn[f]; Xn[f] = Xq[f]; }
             w1 = w2;
+            if (FAST) { o3c += sms; o0c += sms; kd2c += dsgn; }
             return;
         }
 
@@ -297,7 +314,7 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
                 double du[ND], dxa[ND], dxc[ND];
 #pragma unroll
                 for (int c = 0; c < ND; ++c) du[c] = w2.u[c] - w1.u[c];
-                cross(slotU, uslot(j + 1), dxa, dxc);
+                cross(slotU, p1, dxa, dxc);
                 flux<ND, CA>(Xc, w1, du, w2.T - w1.T, dxa, dxc, A, F1);
             }
         }
@@ -360,7 +377,7 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
 #pragma unroll
                     for (int f = 0; f < NF; ++f) o[f] = fma(-hcdt, FP1[f], H0[f]);
                 }
-                if (owner) store(j, o);
+                if (owner) store_at(o0, o);
             }
             FP0m = FP1[0];
 #pragma unroll
@@ -376,6 +393,7 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
 #pragma unroll
         for (int f = 0; f <= ND; ++f) Xon[f] = Xoq[f];
         w1 = w2; gz1 = gz2;
+        if (FAST) { o3c += sms; o0c += sms; kd2c += dsgn; }
     };
 
     // ---- the march -------------------------------------------------------------------------------
@@ -384,17 +402,22 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
         constexpr int ROLE = decltype(role_tag)::value;
         integral_constant<bool, false> slow;
         integral_constant<bool, true> fast;
+        integral_constant<int, -1> par_any;
         int j = l0 - 4;
         if (exists(j + 2)) {
             load(j + 2, Xn);
-            if (ROLE == ROLE_R1 && has_outer) load_outer(j + 2, Xon);
+            if (ROLE == ROLE_R1 && has_outer) load_outer(off_of(j + 2) - off_base + off_base_o, Xon);
         }
-        const int jf0 = WALL_M ? max(l0, 1) : l0;
-        const int jf1 = WALL_M ? min(l1, n - 3) : l1;
-        for (; j < l1 && j < jf0; ++j) body(role_tag, slow, j);
-#pragma unroll 2
-        for (; j < jf1; ++j) body(role_tag, fast, j);
-        for (; j < l1; ++j) body(role_tag, slow, j);
+        // fast levels: every level j-1 .. j+3 exists, none is a plate, none wraps around
+        const int jf0 = max(l0, 1);
+        const int jf1 = min(l1, n - 3);
+        for (; j < l1 && (j < jf0 || (j & 1)); ++j) body(role_tag, slow, par_any, j);
+        if (j + 1 < jf1) { o3c = off_of(j + 3); o0c = off_of(j); kd2c = (double)phys_k(j + 2); }
+        for (; j + 1 < jf1; j += 2) {
+            body(role_tag, fast, integral_constant<int, 0>(), j);
+            body(role_tag, fast, integral_constant<int, 1>(), j + 1);
+        }
+        for (; j < l1; ++j) body(role_tag, slow, par_any, j);
     };
     switch (role) {
     case ROLE_NONE: march(std::integral_constant<int, ROLE_NONE>()); break;
