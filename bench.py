@@ -181,21 +181,26 @@ def workload_config(name, grid, params):
 # ---------------------------------------------------------------------------------------------------
 # our arm: the CUDA path through the C ABI
 # ---------------------------------------------------------------------------------------------------
-KERNEL_NAMES = {"Lx+": "k_lane (L_x, dir +1)", "Lx-": "k_lane (L_x, dir -1)",
-                "Ly+": "k_march (L_y, dir +1)", "Ly-": "k_march (L_y, dir -1)",
-                "Lz+": "k_march (L_z, dir +1)", "Lz-": "k_march (L_z, dir -1)"}
+def kernel_names(ndim):
+    """Kernel behind each operator (csrc/mc_tvd.cu launch_sweep): the 3-D box has its own pair."""
+    lane, march = ("k_lane", "k_march") if ndim == 2 else ("k_lane3", "k_march3")
+    return {"Lx+": f"{lane} (L_x, dir +1)", "Lx-": f"{lane} (L_x, dir -1)",
+            "Ly+": f"{march} (L_y, dir +1)", "Ly-": f"{march} (L_y, dir -1)",
+            "Lz+": f"{march} (L_z, dir +1)", "Lz-": f"{march} (L_z, dir -1)"}
 
 
-def ncu_traffic(name: str, kernel_key: str):
-    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full summary, or None."""
+def ncu_counters(name: str, kernel_key: str):
+    """(DRAM bytes, fp64 thread instructions) per launch of a kernel from the committed ncu --set full
+    capture (profiles/traffic.json, written from profiles/*_ncu_full.txt), or (None, None)."""
     path = os.path.join(ROOT, "profiles", "traffic.json")
     if not os.path.exists(path):
-        return None
+        return None, None
     try:
         with open(path) as f:
-            return json.load(f).get(name, {}).get(kernel_key[:2])
+            rec = json.load(f).get(name, {}).get(kernel_key[:2], {})
+        return rec.get("dram_bytes"), rec.get("fp64_thread_insts")
     except Exception:
-        return None
+        return None, None
 
 
 def run_ours(args):
@@ -290,12 +295,22 @@ def run_ours(args):
     dom = max(per_kernel, key=lambda k: per_kernel[k][0])
     dom_ms = per_kernel[dom][0] / per_kernel[dom][1]
     achieved = alg_bytes / (dom_ms * 1e-3) / 1e9
+    KERNEL_NAMES = kernel_names(grid["ndim"])
     kernels = {KERNEL_NAMES[k]: {"avg_ms": v[0] / v[1], "launches": v[1], "share_of_step": v[0] / ms,
                                  "achieved_GBps": alg_bytes / (v[0] / v[1] * 1e-3) / 1e9}
                for k, v in per_kernel.items()}
     step_gbps = (4 if grid["ndim"] == 2 else 6) * alg_bytes * args.steps / (ms * 1e-3) / 1e9
+    traffic, fp64_insts = ncu_counters(name, dom)
+    sm_mhz = clocks.summary().get("sm_mhz") or 1965
+    fp64_peak = 148 * 64 * sm_mhz * 1e6                               # DFMA/s: 64 fp64 lanes per SM per clock
+    fp64 = None
+    if fp64_insts:
+        fp64 = {"thread_insts_per_launch": fp64_insts, "per_cell": fp64_insts / N,
+                "achieved_Ginst_s": fp64_insts / (dom_ms * 1e-3) / 1e9, "peak_Ginst_s": fp64_peak / 1e9,
+                "frac": fp64_insts / (dom_ms * 1e-3) / fp64_peak,
+                "note": "co-bound: the fp64 pipe time of this kernel is close to its HBM time (DESIGN.md 7)"}
     roofline = {"bound": "hbm", "kernel": KERNEL_NAMES[dom], "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": ncu_traffic(name, dom), "peak_source": peak_src,
+                "frac": achieved / peak, "traffic": traffic, "fp64_pipe": fp64, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": alg_bytes,
                 "algorithmic_bytes_per_cell_per_operator": 2 * nf * 8,
                 "whole_step_achieved_GBps": step_gbps, "whole_step_frac": step_gbps / peak,

@@ -14,7 +14,8 @@ _PKG = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_PKG, "csrc")
 LIB_PATH = os.path.join(_PKG, "libmc_tvd.so")
 _SOURCES = ["mc_tvd.cu"]
-_DEPS = ["mc_tvd.cu", "mc_common.cuh", "sweep_march.cuh", "sweep_lane.cuh", "reduce_kernels.cuh",
+_DEPS = ["mc_tvd.cu", "mc_common.cuh", "sweep_march.cuh", "sweep_lane.cuh", "sweep_march3.cuh", "sweep_lane3.cuh",
+         "reduce_kernels.cuh",
          os.path.join("..", "..", "include", "mc_tvd.h")]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

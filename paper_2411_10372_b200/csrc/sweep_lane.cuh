@@ -21,6 +21,10 @@
 
 #include "mc_common.cuh"
 
+#ifndef MC_SWEEP_L2PF
+#define MC_SWEEP_L2PF 4
+#endif
+
 namespace mc {
 
 constexpr int LANE_OUT = 28;      // outputs per warp: 32 lanes minus the 2+2 halo
@@ -140,6 +144,13 @@ MC_KERNEL void __launch_bounds__(32 * WB, MINB) k_lane(SweepArgs A)
 #pragma unroll
         for (int f = 0; f < NF; ++f) Xq[f] = Xn[f];
         if (FAST || (exists(j + 3) && j + 3 <= l1 + 1)) load(j + 3, Xq);
+#if MC_SWEEP_L2PF > 0
+        if (j + 3 + MC_SWEEP_L2PF <= l1 + 1 && exists(j + 3 + MC_SWEEP_L2PF)) {
+            const double *pp = pin + (long long)lev(j + 3 + MC_SWEEP_L2PF) * A.s_m;
+#pragma unroll
+            for (int f = 0; f < NF; ++f) asm volatile("prefetch.global.L2 [%0];" ::"l"(pp + (long long)f * A.N));
+        }
+#endif
 
         if (HAS_B) __syncthreads();
 

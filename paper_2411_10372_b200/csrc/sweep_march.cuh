@@ -25,6 +25,10 @@
 
 #include "mc_common.cuh"
 
+#ifndef MC_SWEEP_L2PF
+#define MC_SWEEP_L2PF 4
+#endif
+
 namespace mc {
 
 enum { ROLE_NONE = 0, ROLE_R2 = 1, ROLE_WALLROW = 2, ROLE_R1 = 3, ROLE_IN = 4 };
@@ -175,6 +179,14 @@ MC_KERNEL void __launch_bounds__(WX * WB, MINB) k_march(SweepArgs A)
 #pragma unroll
         for (int f = 0; f < NF; ++f) Xq[f] = Xn[f];
         if (FAST || (exists(j + 3) && j + 3 <= l1 + 1)) load(j + 3, Xq);
+#if MC_SWEEP_L2PF > 0
+        // far-ahead L2 prefetch: the one-level register prefetch alone leaves the HBM latency exposed
+        if (j + 3 + MC_SWEEP_L2PF <= l1 + 1 && exists(j + 3 + MC_SWEEP_L2PF)) {
+            const double *pp = pin + (long long)lev(j + 3 + MC_SWEEP_L2PF) * sm_signed;
+#pragma unroll
+            for (int f = 0; f < NF; ++f) asm volatile("prefetch.global.L2 [%0];" ::"l"(pp + (long long)f * A.N));
+        }
+#endif
 
         // (1) W(j+2): primitives, Courant coefficient, publish velocities
         Prim<ND> w2 = w1;
