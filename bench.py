@@ -203,6 +203,22 @@ def ncu_counters(name: str, kernel_key: str):
         return None, None
 
 
+def max_over_ranks(x: float, world: int, device: str) -> float:
+    """Slowest rank's value (replicas only: the job is as slow as its slowest replica)."""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_value(world: int, cells_per_rank: int, steps: int, ms: float) -> float:
+    """Whole-job cell-updates/s: every rank advanced its own replica `steps` steps in `ms` milliseconds."""
+    return world * cells_per_rank * steps / (ms * 1e-3)
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -257,11 +273,8 @@ def run_ours(args):
     dt_now = solver.dt()                                             # raises if the state went non-finite
     diag, *_ = solver.diagnostics()
 
-    t = torch.tensor([ms], dtype=torch.float64, device=f"cuda:{local}")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_max = float(t.item())
-    value = world * N * args.steps / (ms_max * 1e-3)
+    ms_max = max_over_ranks(ms, world, f"cuda:{local}")
+    value = job_value(world, N, args.steps, ms_max)
 
     # ---- end to end through the public host-buffer call (H2D + steps + D2H inside the timed region) --
     e2e = None
@@ -274,12 +287,10 @@ def run_ours(args):
             solver.step_host(h_in, h_out, 1)                         # synchronises internally
         barrier()
         el = time.perf_counter() - t0
-        te = torch.tensor([el], dtype=torch.float64, device=f"cuda:{local}")
-        if world > 1:
-            dist.all_reduce(te, op=dist.ReduceOp.MAX)
-        e2e = {"value": world * N * n_e2e / float(te.item()), "unit": UNIT,
+        el_max = max_over_ranks(el, world, f"cuda:{local}")
+        e2e = {"value": job_value(world, N, n_e2e, el_max * 1e3), "unit": UNIT,
                "h2d_bytes_per_step": state_bytes, "d2h_bytes_per_step": state_bytes,
-               "steps": n_e2e, "ms_per_step": float(te.item()) / n_e2e * 1e3,
+               "steps": n_e2e, "ms_per_step": el_max / n_e2e * 1e3,
                "call": "mc_tvd_step_host(h_in, h_out, 1): H2D of the state, dt reduction, 1 step, D2H of the state",
                "host_memory": "pinned" if pinned else "pageable"}
     solver.close()

@@ -59,6 +59,9 @@ def test_workspace_bytes_and_validation(lib):
     assert lib.mc_tvd_workspace_bytes(C.byref(g), C.byref(pb)) == 0
     pb = binding.make_params(inputs.make_params(tvd_form=2))
     assert lib.mc_tvd_workspace_bytes(C.byref(g), C.byref(pb)) == 0
+    huge = binding.make_grid(inputs.make_grid(3, 2048, 1024, 2048))   # 2^32 nodes per field: 32-bit node offsets
+    assert lib.mc_tvd_workspace_bytes(C.byref(huge), C.byref(p)) == 0
+    assert b"2^32" in lib.mc_tvd_last_error()
 
 
 def test_init_rejects_bad_arguments_before_touching_the_device(lib):
