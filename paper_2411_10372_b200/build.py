@@ -29,6 +29,24 @@ def _stale() -> bool:
     return any(os.path.getmtime(os.path.join(_CSRC, d)) > t for d in _DEPS)
 
 
+MAX_STACK_BYTES = 256
+
+
+def _check_stack_frames(ptxas_log: str) -> None:
+    """A sweep kernel whose march lambdas were not inlined keeps its register pipeline in local memory
+    (seen once: 1472-byte frame, 6x slower).  ptxas -v reports the frame of every entry: refuse such a build."""
+    import re
+    entry = None
+    for line in ptxas_log.splitlines():
+        m = re.search(r"Compiling entry function '([^']+)'", line)
+        if m:
+            entry = m.group(1)
+        m = re.search(r"(\d+) bytes stack frame", line)
+        if m and entry and int(m.group(1)) > MAX_STACK_BYTES:
+            raise RuntimeError(f"kernel {entry} has a {m.group(1)}-byte stack frame (> {MAX_STACK_BYTES}): "
+                               "a lambda was not inlined or the register budget is too small")
+
+
 def build_library(force: bool = False, verbose: bool = False) -> str:
     if not (force or _stale()):
         return LIB_PATH
@@ -42,6 +60,7 @@ def build_library(force: bool = False, verbose: bool = False) -> str:
     if res.returncode != 0:
         sys.stderr.write(log)
         raise RuntimeError("nvcc failed building libmc_tvd.so")
+    _check_stack_frames(log)
     os.replace(tmp, LIB_PATH)
     if verbose:
         print(log)

@@ -82,6 +82,7 @@ struct mc_tvd_state {
     cudaStream_t stream;
     long long launches;
     int chunk_override;
+    int sm_count;
     // per-kernel timing (mc_tvd_timing_*): events ev[0..n_ev) recorded around operator launches;
     // launch r ran between ev_pair[r] and ev_pair[r] + 1
     bool timing;
@@ -175,13 +176,23 @@ void fill_common(const mc_tvd_state *s, mc::SweepArgs &A, const double *in, doub
     A.nz = s->grid.nz;
 }
 
-int pick_chunk(const mc_tvd_state *s, int n_m, long long tiles)
+// Marching levels per block.  Cutting the march into c chunks multiplies the blocks (fills the SMs, evens
+// out the last wave) but every chunk repeats a 4-level warm-up.  Model: blocks run in waves of
+// (SMs x resident blocks per SM); cost(c) = waves(c) x (levels per chunk + 4).  Take the cheapest c.
+int pick_chunk(const mc_tvd_state *s, int n_m, long long tiles, int blocks_per_sm)
 {
     if (s->chunk_override > 0) return s->chunk_override < n_m ? s->chunk_override : n_m;
-    // enough blocks for a few waves over 148 SMs, but chunks long enough to amortise the 4-level warm-up
-    int chunk = n_m;
-    while (chunk > 64 && tiles * ((n_m + chunk - 1) / chunk) < 148 * 8) chunk = (chunk + 1) / 2;
-    return chunk;
+    const long long slots = (long long)s->sm_count * blocks_per_sm;
+    const int c_max = n_m / 32 > 1 ? n_m / 32 : 1;
+    long long best_cost = -1;
+    int best_chunk = n_m;
+    for (int c = 1; c <= c_max; ++c) {
+        const int chunk = (n_m + c - 1) / c;
+        const long long blocks = tiles * ((n_m + chunk - 1) / chunk);
+        const long long cost = ((blocks + slots - 1) / slots) * (chunk + 4);
+        if (best_cost < 0 || cost < best_cost) { best_cost = cost; best_chunk = chunk; }
+    }
+    return best_chunk;
 }
 
 // compile-time dispatch of the kernels' switches
@@ -241,7 +252,7 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
             constexpr int WX = MARCH_WX_2D;
             A.n_b = 1; A.s_b = 0; A.n_m = nz; A.s_m = nx;
             long long tiles = (nx + WX - 5) / (WX - 4);
-            A.chunk = pick_chunk(s, nz, tiles);
+            A.chunk = pick_chunk(s, nz, tiles, MARCH_MINB_2D);
             dim3 block(WX, 1, 1), grid((unsigned)tiles, 1, (unsigned)((nz + A.chunk - 1) / A.chunk));
             size_t smem = ((size_t)4 * 2 * WX + 4) * sizeof(double);
             with_walls(wl, [&](auto W) { with_tvd(s, [&](auto T) {
@@ -252,7 +263,7 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
             A.n_b = 1; A.s_b = 0; A.n_m = nz; A.s_m = nx;
             long long xt = (nx + mc::LANE_OUT - 1) / mc::LANE_OUT;
             long long tiles = (xt + LW - 1) / LW;
-            A.chunk = pick_chunk(s, nz, tiles);
+            A.chunk = pick_chunk(s, nz, tiles, LANE_MINB_2D);
             dim3 block(32, LW, 1), grid((unsigned)tiles, 1, (unsigned)((nz + A.chunk - 1) / A.chunk));
             with_walls(wl, [&](auto W) { with_tvd(s, [&](auto T) { with_bool(reduce, [&](auto Rd) {
                 launch_kernel(mc::k_lane<2, -1, 1, LW, decltype(W)::value, decltype(T)::value, decltype(Rd)::value, LANE_MINB_2D>, grid, block, 0, st, A);
@@ -266,7 +277,7 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
             constexpr int MW = MARCH3_WB, MO = MW - 2;
             A.n_b = ny; A.s_b = nx; A.n_m = nz; A.s_m = (long long)nx * ny;
             long long bt = (ny + MO - 1) / MO;
-            A.chunk = pick_chunk(s, nz, xt * bt);
+            A.chunk = pick_chunk(s, nz, xt * bt, 1);
             dim3 mblock(32, MW, 1), grid((unsigned)xt, (unsigned)bt, (unsigned)((nz + A.chunk - 1) / A.chunk));
             size_t smem = ((size_t)4 * 3 * 32 * (MW + 2) + 8) * sizeof(double);
             with_walls(wl, [&](auto W) { with_tvd(s, [&](auto T) {
@@ -276,7 +287,7 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
             constexpr int MW = MARCH3_WB, MO = MW - 2;
             A.n_b = nz; A.s_b = (long long)nx * ny; A.n_m = ny; A.s_m = nx;
             long long bt = (nz + MO - 1) / MO;
-            A.chunk = pick_chunk(s, ny, xt * bt);
+            A.chunk = pick_chunk(s, ny, xt * bt, 1);
             dim3 mblock(32, MW, 1), grid((unsigned)xt, (unsigned)bt, (unsigned)((ny + A.chunk - 1) / A.chunk));
             size_t smem = ((size_t)4 * 3 * 32 * (MW + 2) + 8) * sizeof(double);
             with_walls(wl, [&](auto W) { with_tvd(s, [&](auto T) {
@@ -286,7 +297,7 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
             constexpr int LW = LANE3_WB, LO = LW - 2;
             A.n_b = ny; A.s_b = nx; A.n_m = nz; A.s_m = (long long)nx * ny;
             long long bt = (ny + LO - 1) / LO;
-            A.chunk = pick_chunk(s, nz, xt * bt);
+            A.chunk = pick_chunk(s, nz, xt * bt, 1);
             dim3 lblock(32, LW, 1), grid((unsigned)xt, (unsigned)bt, (unsigned)((nz + A.chunk - 1) / A.chunk));
             size_t smem = (size_t)4 * 2 * 32 * (LW + 2) * sizeof(double);
             with_walls(wl, [&](auto W) { with_tvd(s, [&](auto T) { with_bool(reduce, [&](auto Rd) {
@@ -387,6 +398,12 @@ int mc_tvd_init(const mc_tvd_grid *grid, const mc_tvd_params *params, double *d_
     s->stream = (cudaStream_t)cuda_stream;
     const char *ce = getenv("MC_TVD_CHUNK");
     s->chunk_override = ce ? atoi(ce) : 0;
+    {
+        int dev = 0, sms = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1)
+            sms = 148;
+        s->sm_count = sms;
+    }
 
     mc::Scalars h;
     memset(&h, 0, sizeof(h));

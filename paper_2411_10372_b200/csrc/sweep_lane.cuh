@@ -90,23 +90,23 @@ MC_KERNEL void __launch_bounds__(32 * WB, MINB) k_lane(SweepArgs A)
     const double *const pin = A.in + col;
     double *const pout = A.out + col;
 
-    auto exists = [&](int l) { return WALL_M ? (l >= 0 && l < n) : true; };
-    auto is_plate = [&](int l) { return WALL_M && (l == 0 || l == n - 1); };
-    auto lev = [&](int l) { return WALL_M ? l : wrap1(l, n); };
-    auto gz_of = [&](int l) { return A.g * ((double)lev(l) * A.dz); };       // m is z
-    auto load = [&](int l, double (&X)[NF]) {
+    auto exists = [&](int l) MC_INL { return WALL_M ? (l >= 0 && l < n) : true; };
+    auto is_plate = [&](int l) MC_INL { return WALL_M && (l == 0 || l == n - 1); };
+    auto lev = [&](int l) MC_INL { return WALL_M ? l : wrap1(l, n); };
+    auto gz_of = [&](int l) MC_INL { return A.g * ((double)lev(l) * A.dz); };       // m is z
+    auto load = [&](int l, double (&X)[NF]) MC_INL {
         const double *p = pin + (long long)lev(l) * A.s_m;
 #pragma unroll
         for (int f = 0; f < NF; ++f) X[f] = p[(long long)f * A.N];
     };
-    auto publish = [&](double *slot, int parity, const double (&u)[ND]) {
+    auto publish = [&](double *slot, int parity, const double (&u)[ND]) MC_INL {
         if (HAS_B) {
             slot[(parity * 2 + 0) * TILE + tidx] = u[0];
             slot[(parity * 2 + 1) * TILE + tidx] = u[cb];
         }
     };
     // central b-differences of (u_x, u_b) published in `slot`
-    auto cross_b = [&](const double *slot, int parity, double (&dxa)[ND], double (&dxc)[ND]) {
+    auto cross_b = [&](const double *slot, int parity, double (&dxa)[ND], double (&dxc)[ND]) MC_INL {
         if (HAS_B) {
             const double *s = slot + parity * 2 * TILE + tidx;
             dxa[cb] = s[32] - s[-32];
@@ -131,7 +131,7 @@ MC_KERNEL void __launch_bounds__(32 * WB, MINB) k_lane(SweepArgs A)
     for (int c = 0; c < ND; ++c) { w1.u[c] = 0.0; wP0.u[c] = 0.0; }
     w1.T = 1.0; w1.p = 0.0; wP0.T = 1.0; wP0.p = 0.0;
 
-    auto body = [&](auto role_tag, auto fast_tag, auto par_tag, const int j) {
+    auto body = [&](auto role_tag, auto fast_tag, auto par_tag, const int j) MC_INL {
         constexpr int ROLE = decltype(role_tag)::value;
         constexpr bool FAST = decltype(fast_tag)::value;
         constexpr int PAR = decltype(par_tag)::value;
@@ -266,7 +266,7 @@ MC_KERNEL void __launch_bounds__(32 * WB, MINB) k_lane(SweepArgs A)
         w1 = w2; wP0 = wP1; hC0 = hC1; hC1 = hC2; gz1 = gz2;
     };
 
-    auto march = [&](auto role_tag) {
+    auto march = [&](auto role_tag) MC_INL {
         using std::integral_constant;
         integral_constant<bool, false> slow;
         integral_constant<bool, true> fast;

@@ -96,29 +96,29 @@ MC_KERNEL void __launch_bounds__(WX * WB, MINB) k_march(SweepArgs A)
     double *const pout = A.out + col + ((A.dir > 0) ? 0 : (long long)(n - 1) * A.s_m);
     const double gz_fixed = A.g * ((double)gb * A.dz);                       // used when b is z
 
-    auto exists = [&](int l) { return WALL_M ? (l >= 0 && l < n) : true; };
-    auto lev = [&](int l) { return WALL_M ? l : wrap1(l, n); };              // l in [-n, 2n)
-    auto gz_of = [&](int l) {                         // g z_k of Eq. 17 for this thread's node at level l
+    auto exists = [&](int l) MC_INL { return WALL_M ? (l >= 0 && l < n) : true; };
+    auto lev = [&](int l) MC_INL { return WALL_M ? l : wrap1(l, n); };              // l in [-n, 2n)
+    auto gz_of = [&](int l) MC_INL {                         // g z_k of Eq. 17 for this thread's node at level l
         if (!Z_IS_ALPHA) return gz_fixed;
         const int w = lev(l);
         return A.g * ((double)((A.dir > 0) ? w : n - 1 - w) * A.dz);
     };
-    auto load = [&](int l, double (&X)[NF]) {
+    auto load = [&](int l, double (&X)[NF]) MC_INL {
         const double *p = pin + (long long)lev(l) * sm_signed;
 #pragma unroll
         for (int f = 0; f < NF; ++f) X[f] = p[(long long)f * A.N];
     };
-    auto store = [&](int l, const double (&o)[NF]) {
+    auto store = [&](int l, const double (&o)[NF]) MC_INL {
         double *q = pout + (long long)lev(l) * sm_signed;
 #pragma unroll
         for (int f = 0; f < NF; ++f) q[(long long)f * A.N] = o[f];
     };
-    auto publish = [&](double *slot, int parity, const double (&u)[ND]) {
+    auto publish = [&](double *slot, int parity, const double (&u)[ND]) MC_INL {
 #pragma unroll
         for (int c = 0; c < ND; ++c) slot[(parity * ND + c) * TILE + tidx] = u[c];
     };
     // central cross DIFFERENCES of the velocities published in `slot` (R7)
-    auto cross = [&](const double *slot, int parity, double (&dxa)[ND], double (&dxc)[ND]) {
+    auto cross = [&](const double *slot, int parity, double (&dxa)[ND], double (&dxc)[ND]) MC_INL {
         const double *s = slot + parity * ND * TILE + tidx;
 #pragma unroll
         for (int c = 0; c < ND; ++c) { dxa[c] = 0.0; dxc[c] = 0.0; }
@@ -131,7 +131,7 @@ MC_KERNEL void __launch_bounds__(WX * WB, MINB) k_march(SweepArgs A)
     };
     // plate values of a node on a plate of the marching direction: no slip,
     // T = T_w; only rho is free (R10)
-    auto plate = [&](int l, double rho, double (&X)[NF]) {
+    auto plate = [&](int l, double rho, double (&X)[NF]) MC_INL {
         const int k = (A.dir > 0) ? l : n - 1 - l;
         const double Tw = (k == 0) ? A.Tw0 : A.Tw1;
         X[0] = rho;
@@ -160,7 +160,7 @@ MC_KERNEL void __launch_bounds__(WX * WB, MINB) k_march(SweepArgs A)
 
     // One iteration.  ROLE and FAST are compile-time tags; PAR is the compile-time parity of j in the
     // unrolled FAST pair (-1: take it from j).
-    auto body = [&](auto role_tag, auto fast_tag, auto par_tag, const int j) {
+    auto body = [&](auto role_tag, auto fast_tag, auto par_tag, const int j) MC_INL {
         constexpr int ROLE = decltype(role_tag)::value;
         constexpr bool FAST = decltype(fast_tag)::value;
         constexpr int PAR = decltype(par_tag)::value;
@@ -321,7 +321,7 @@ MC_KERNEL void __launch_bounds__(WX * WB, MINB) k_march(SweepArgs A)
     };
 
     // ---- the march -------------------------------------------------------------------------------
-    auto march = [&](auto role_tag) {
+    auto march = [&](auto role_tag) MC_INL {
         using std::integral_constant;
         integral_constant<bool, false> slow;
         integral_constant<bool, true> fast;

@@ -104,43 +104,43 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
     const int pf_last = min(l1 + 1, n - 1) - MC_MARCH3_L2PF;                // last j + 3 whose L2 prefetch is issued
     const double gz_fixed = A.g * ((double)gb * A.dz);                       // used when b is z
 
-    auto exists = [&](int l) { return WALL_M ? (l >= 0 && l < n) : true; };
-    auto lev = [&](int l) { return WALL_M ? l : wrap1(l, n); };              // l in [-n, 2n)
+    auto exists = [&](int l) MC_INL { return WALL_M ? (l >= 0 && l < n) : true; };
+    auto lev = [&](int l) MC_INL { return WALL_M ? l : wrap1(l, n); };              // l in [-n, 2n)
     const double *inb[NF];
     double *outb[NF];
 #pragma unroll
     for (int f = 0; f < NF; ++f) { inb[f] = A.in + (long long)f * A.N; outb[f] = A.out + (long long)f * A.N; }
-    auto off_of = [&](int l) { return off_base + (unsigned)lev(l) * sms; };
-    auto phys_k = [&](int l) { const int w = lev(l); return (A.dir > 0) ? w : n - 1 - w; };
-    auto load_at = [&](unsigned o, double (&X)[NF]) {
+    auto off_of = [&](int l) MC_INL { return off_base + (unsigned)lev(l) * sms; };
+    auto phys_k = [&](int l) MC_INL { const int w = lev(l); return (A.dir > 0) ? w : n - 1 - w; };
+    auto load_at = [&](unsigned o, double (&X)[NF]) MC_INL {
 #pragma unroll
         for (int f = 0; f < NF; ++f) X[f] = inb[f][o];
     };
-    auto load = [&](int l, double (&X)[NF]) { load_at(off_of(l), X); };
-    auto gz_of = [&](int l) {                         // g z_k of Eq. 17 for this thread's node at level l
+    auto load = [&](int l, double (&X)[NF]) MC_INL { load_at(off_of(l), X); };
+    auto gz_of = [&](int l) MC_INL {                         // g z_k of Eq. 17 for this thread's node at level l
         if (!Z_IS_ALPHA) return gz_fixed;
         return A.g * ((double)phys_k(l) * A.dz);
     };
     // L2 prefetch of the thread's node at level l (no register, no scoreboard): hides the HBM latency
     // the one-level register prefetch cannot cover with 12 warps per SM
-    auto prefetch_l2 = [&](unsigned o) {
+    auto prefetch_l2 = [&](unsigned o) MC_INL {
 #pragma unroll
         for (int f = 0; f < NF; ++f) asm volatile("prefetch.global.L2 [%0];" ::"l"(inb[f] + o));
     };
-    auto load_outer = [&](unsigned o, double (&X)[ND + 1]) {                 // rho and the momenta only
+    auto load_outer = [&](unsigned o, double (&X)[ND + 1]) MC_INL {                 // rho and the momenta only
 #pragma unroll
         for (int f = 0; f <= ND; ++f) X[f] = inb[f][o];
     };
-    auto store_at = [&](unsigned o, const double (&v)[NF]) {
+    auto store_at = [&](unsigned o, const double (&v)[NF]) MC_INL {
 #pragma unroll
         for (int f = 0; f < NF; ++f) outb[f][o] = v[f];
     };
-    auto publish = [&](double *slot, int parity, int at, const double (&u)[ND]) {
+    auto publish = [&](double *slot, int parity, int at, const double (&u)[ND]) MC_INL {
 #pragma unroll
         for (int c = 0; c < ND; ++c) slot[(parity * ND + c) * TILE + at] = u[c];
     };
     // central cross DIFFERENCES of the velocities published in `slot` (R7)
-    auto cross = [&](const double *slot, int parity, double (&dxa)[ND], double (&dxc)[ND]) {
+    auto cross = [&](const double *slot, int parity, double (&dxa)[ND], double (&dxc)[ND]) MC_INL {
         const double *s = slot + parity * ND * TILE + tidx;
 #pragma unroll
         for (int c = 0; c < ND; ++c) { dxa[c] = 0.0; dxc[c] = 0.0; }
@@ -151,7 +151,7 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
     };
     // plate values of a node on a plate of the marching direction: no slip,
     // T = T_w; only rho is free (R10)
-    auto plate = [&](int l, double rho, double (&X)[NF]) {
+    auto plate = [&](int l, double rho, double (&X)[NF]) MC_INL {
         const int k = (A.dir > 0) ? l : n - 1 - l;
         const double Tw = (k == 0) ? A.Tw0 : A.Tw1;
         X[0] = rho;
@@ -175,7 +175,7 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
         if (tx == 0) flags[ty] = l0 - 5;
         __syncthreads();
     }
-    auto level_sync = [&](int j) {
+    auto level_sync = [&](int j) MC_INL {
         if (!MC_MARCH3_SYNC) { __syncthreads(); return; }
         __syncwarp();
         if (tx == 0) asm volatile("st.release.cta.shared.b32 [%0], %1;" ::"r"(flag_me), "r"(j) : "memory");
@@ -214,7 +214,7 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
     // W(L): primitives of X(L) (in `X`), Courant coefficient, velocities published into slot uslot(L);
     // a ring-1 row also publishes the velocities of its ring-2 neighbour row (from `Xo`).
     auto stage_W = [&](auto role_tag, int par, double gz, const double (&X)[NF], const double (&Xo)[ND + 1],
-                       Prim<ND> &w, double &hC) {
+                       Prim<ND> &w, double &hC) MC_INL {
         constexpr int ROLE = decltype(role_tag)::value;
         w = primitives<ND>(X, gz, A);
         if (ROLE == ROLE_IN && TVD >= 0) hC = half_courant_coef(w.u[CA], w.T, half_tod, A);
@@ -230,7 +230,7 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
 
     // One iteration.  ROLE and FAST are compile-time tags; PAR is the compile-time parity of j in the
     // unrolled FAST pair (-1: take it from j).
-    auto body = [&](auto role_tag, auto fast_tag, auto par_tag, const int j) {
+    auto body = [&](auto role_tag, auto fast_tag, auto par_tag, const int j) MC_INL {
         constexpr int ROLE = decltype(role_tag)::value;
         constexpr bool FAST = decltype(fast_tag)::value;
         constexpr int PAR = decltype(par_tag)::value;
@@ -254,7 +254,7 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
         else if (j + 3 + MC_MARCH3_L2PF <= l1 + 1 && exists(j + 3 + MC_MARCH3_L2PF)) prefetch_l2(off_of(j + 3 + MC_MARCH3_L2PF));
 #endif
         double Xq[NF], Xoq[ND + 1];
-        auto fetch = [&]() {
+        auto fetch = [&]() MC_INL {
 #pragma unroll
             for (int f = 0; f < NF; ++f) Xq[f] = Xn[f];
             if (ld3) load_at(o3, Xq);
@@ -397,7 +397,7 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
     };
 
     // ---- the march -------------------------------------------------------------------------------
-    auto march = [&](auto role_tag) {
+    auto march = [&](auto role_tag) MC_INL {
         using std::integral_constant;
         constexpr int ROLE = decltype(role_tag)::value;
         integral_constant<bool, false> slow;
