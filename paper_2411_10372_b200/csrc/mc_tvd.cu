@@ -174,11 +174,16 @@ void fill_common(const mc_tvd_state *s, mc::SweepArgs &A, const double *in, doub
     A.gamma = s->par.gamma; A.gammaR = s->par.gamma * s->R;
     A.Tw0 = s->par.T_bot; A.Tw1 = s->par.T_top;
     A.nz = s->grid.nz;
+    double D = 0.0;
+    for (int c = 0; c < s->nd; ++c) D = A.inv_d[c] > D ? A.inv_d[c] : D;
+    A.cfl_wQ = s->par.gamma * (s->par.gamma - 1.0) * (1.0 + 1.0 / 16.0) * D * D;
+    A.cfl_wm = (1.0 + 16.0) * D * D;
 }
 
 // Marching levels per block.  Cutting the march into c chunks multiplies the blocks (fills the SMs, evens
 // out the last wave) but every chunk repeats a 4-level warm-up.  Model: blocks run in waves of
-// (SMs x resident blocks per SM); cost(c) = waves(c) x (levels per chunk + 4).  Take the cheapest c.
+// (SMs x resident blocks per SM) and the last wave costs about half a block more than its share;
+// cost(c) = max(whole waves, waves + 1/2) x (levels per chunk + 4).  Take the cheapest c.
 int pick_chunk(const mc_tvd_state *s, int n_m, long long tiles, int blocks_per_sm)
 {
     if (s->chunk_override > 0) return s->chunk_override < n_m ? s->chunk_override : n_m;
@@ -189,7 +194,8 @@ int pick_chunk(const mc_tvd_state *s, int n_m, long long tiles, int blocks_per_s
     for (int c = 1; c <= c_max; ++c) {
         const int chunk = (n_m + c - 1) / c;
         const long long blocks = tiles * ((n_m + chunk - 1) / chunk);
-        const long long cost = ((blocks + slots - 1) / slots) * (chunk + 4);
+        const long long whole = 2 * ((blocks + slots - 1) / slots), frac = (2 * blocks + slots - 1) / slots + 1;
+        const long long cost = (whole > frac ? whole : frac) * (chunk + 4);      // in half waves
         if (best_cost < 0 || cost < best_cost) { best_cost = cost; best_chunk = chunk; }
     }
     return best_chunk;

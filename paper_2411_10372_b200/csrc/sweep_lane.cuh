@@ -123,7 +123,13 @@ MC_KERNEL void __launch_bounds__(32 * WB, MINB) k_lane(SweepArgs A)
     double uPm[2] = {0.0, 0.0};    // (u_x, u_m) of X^P(j-1)
     double hC0 = 0.0, hC1 = 0.0;   // C/2 of Eq. 39 at levels j, j+1
     double gz1 = 0.0;
-    double smax = 0.0;
+    double smax = 0.0, smax2 = 0.0;   // running CFL maximum and smax^2 (1 - 1e-6) for the filter
+    if (REDUCE) {
+        // start the filter from the maximum other blocks have already recorded (the bottom, hottest chunks
+        // are scheduled first): a node below a recorded value cannot be the maximum
+        const double g0 = __longlong_as_double((long long)*(volatile unsigned long long *)A.smax_bits);
+        smax2 = (g0 * g0) * (1.0 - 1e-6);
+    }
 #pragma unroll
     for (int f = 0; f < NF; ++f) { Xn[f] = 0.0; X0[f] = 0.0; X1[f] = 0.0; XP0[f] = 0.0; }
     Xn[0] = 1.0; X0[0] = 1.0; X1[0] = 1.0; XP0[0] = 1.0;
@@ -248,13 +254,12 @@ MC_KERNEL void __launch_bounds__(32 * WB, MINB) k_lane(SweepArgs A)
                     for (int f = 0; f < NF; ++f) q[(long long)f * A.N] = o[f];
                 }
                 if (REDUCE) {                                        // CFL max-reduction of the new state (R12)
-                    Prim<ND> wo = primitives<ND>(o, gz_of(j), A);
-                    double s = 0.0;
-                    const double cs = sqrt_pos(A.gammaR * wo.T);
-#pragma unroll
-                    for (int c = 0; c < ND; ++c) s = fmax_nan(s, (fabs(wo.u[c]) + cs) * A.inv_d[c]);
-                    if (!(o[0] > 0.0) || !(wo.T > 0.0)) s = NAN;
-                    if (owner) smax = fmax_nan(smax, s);
+                    const double gzj = gz_of(j);
+                    const bool need = owner && !cfl_can_skip<ND>(o, gzj, smax2, A);
+                    if (__any_sync(0xffffffffu, need)) {             // rare once the running maximum has settled
+                        const double s = cfl_speed<ND>(o, gzj, A);
+                        if (owner) { smax = fmax_nan(smax, s); smax2 = fmax_nan(smax2, (smax * smax) * (1.0 - 1e-6)); }
+                    }
                 }
             }
         }

@@ -65,6 +65,7 @@ MC_KERNEL void __maxnreg__((65536 / (32 * WB)) / 8 * 8) k_lane3(SweepArgs A)
     const int l0 = (int)blockIdx.z * A.chunk;
     const int l1 = min(n, l0 + A.chunk);
     const unsigned sm = (unsigned)A.s_m;              // node offsets are 32-bit (N < 2^32, mc_tvd_init)
+    const int pf_last = min(l1 + 1, n - 1) - MC_LANE3_L2PF;   // last j + 3 whose L2 prefetch is issued
     const double *inb[NF];
     double *outb[NF];
 #pragma unroll
@@ -74,17 +75,16 @@ MC_KERNEL void __maxnreg__((65536 / (32 * WB)) / 8 * 8) k_lane3(SweepArgs A)
     auto is_plate = [&](int l) MC_INL { return WALL_M && (l == 0 || l == n - 1); };
     auto lev = [&](int l) MC_INL { return WALL_M ? l : wrap1(l, n); };
     auto gz_of = [&](int l) MC_INL { return A.g * ((double)lev(l) * A.dz); };       // m is z
-    auto load = [&](int l, double (&X)[NF]) MC_INL {
-        const unsigned o = off_base + (unsigned)lev(l) * sm;
+    auto load_at = [&](unsigned o, double (&X)[NF]) MC_INL {
 #pragma unroll
         for (int f = 0; f < NF; ++f) X[f] = inb[f][o];
     };
-    auto load_outer = [&](int l, double (&X)[3]) MC_INL {      // rho, m_x, m_b of the ring-2 row
-        const unsigned o = off_base_o + (unsigned)lev(l) * sm;
+    auto load = [&](int l, double (&X)[NF]) MC_INL { load_at(off_base + (unsigned)lev(l) * sm, X); };
+    auto load_outer_at = [&](unsigned o, double (&X)[3]) MC_INL {   // rho, m_x, m_b of the ring-2 row
         X[0] = inb[0][o]; X[1] = inb[1][o]; X[2] = inb[1 + cb][o];
     };
-    auto prefetch_l2 = [&](int l) MC_INL {
-        const unsigned o = off_base + (unsigned)lev(l) * sm;
+    auto load_outer = [&](int l, double (&X)[3]) MC_INL { load_outer_at(off_base_o + (unsigned)lev(l) * sm, X); };
+    auto prefetch_l2 = [&](unsigned o) MC_INL {
 #pragma unroll
         for (int f = 0; f < NF; ++f) asm volatile("prefetch.global.L2 [%0];" ::"l"(inb[f] + o));
     };
@@ -110,8 +110,17 @@ MC_KERNEL void __maxnreg__((65536 / (32 * WB)) / 8 * 8) k_lane3(SweepArgs A)
     double um0[2] = {0.0, 0.0};    // (u_x, u_m) of X(j)
     double uPm[2] = {0.0, 0.0};    // (u_x, u_m) of X^P(j-1)
     double hC0 = 0.0, hC1 = 0.0;   // C/2 of Eq. 39 at levels j, j+1
-    double gz1 = 0.0;
-    double smax = 0.0;
+    double gz1 = 0.0, gz0 = 0.0;   // g z of levels j+1, j
+    // fast levels only: node offsets of level j+3 (next load) and level j (next store), z index of level j+2
+    unsigned o3c = 0, o0c = 0;
+    double kd2c = 0.0;
+    double smax = 0.0, smax2 = 0.0;   // running CFL maximum and smax^2 (1 - 1e-6) for the filter
+    if (REDUCE) {
+        // start the filter from the maximum other blocks have already recorded (the bottom, hottest chunks
+        // are scheduled first): a node below a recorded value cannot be the maximum
+        const double g0 = __longlong_as_double((long long)*(volatile unsigned long long *)A.smax_bits);
+        smax2 = (g0 * g0) * (1.0 - 1e-6);
+    }
 #pragma unroll
     for (int f = 0; f < NF; ++f) { Xn[f] = 0.0; X0[f] = 0.0; X1[f] = 0.0; XP0[f] = 0.0; }
     Xn[0] = 1.0; X0[0] = 1.0; X1[0] = 1.0; XP0[0] = 1.0;
@@ -132,11 +141,14 @@ MC_KERNEL void __maxnreg__((65536 / (32 * WB)) / 8 * 8) k_lane3(SweepArgs A)
 #pragma unroll
         for (int f = 0; f < NF; ++f) Xq[f] = Xn[f];
         const bool ld3 = FAST || (exists(j + 3) && j + 3 <= l1 + 1);
-        if (ld3) load(j + 3, Xq);
+        const unsigned o3 = FAST ? o3c : off_base + (unsigned)lev(j + 3) * sm;
+        if (ld3) load_at(o3, Xq);
         double Xoq[3] = {Xon[0], Xon[1], Xon[2]};
-        if (ROLE == LROLE_R1 && ld3) load_outer(j + 3, Xoq);
+        if (ROLE == LROLE_R1 && ld3) load_outer_at(o3 - off_base + off_base_o, Xoq);
 #if MC_LANE3_L2PF > 0
-        if (j + 3 + MC_LANE3_L2PF <= l1 + 1 && exists(j + 3 + MC_LANE3_L2PF)) prefetch_l2(j + 3 + MC_LANE3_L2PF);
+        if (FAST) { if (j + 3 <= pf_last) prefetch_l2(o3 + (unsigned)MC_LANE3_L2PF * sm); }
+        else if (j + 3 + MC_LANE3_L2PF <= l1 + 1 && exists(j + 3 + MC_LANE3_L2PF))
+            prefetch_l2(off_base + (unsigned)lev(j + 3 + MC_LANE3_L2PF) * sm);
 #endif
 
         if (HAS_B) __syncthreads();
@@ -145,7 +157,7 @@ MC_KERNEL void __maxnreg__((65536 / (32 * WB)) / 8 * 8) k_lane3(SweepArgs A)
         Prim<ND> w2 = w1;
         double hC2 = 0.0, gz2 = 0.0;
         if (ex2) {
-            gz2 = gz_of(j + 2);
+            gz2 = FAST ? A.g * (kd2c * A.dz) : gz_of(j + 2);
             w2 = primitives<ND>(Xn, gz2, A);
             if (ROLE == LROLE_IN && TVD >= 0) hC2 = half_courant_coef(w2.u[CA], w2.T, half_tod, A);
             publish(slotU, p0, w2.u);                   // parity of level j+2
@@ -230,18 +242,17 @@ MC_KERNEL void __maxnreg__((65536 / (32 * WB)) / 8 * 8) k_lane3(SweepArgs A)
                     }
                 }
                 if (owner) {
-                    const unsigned oo = off_base + (unsigned)lev(j) * sm;
+                    const unsigned oo = FAST ? o0c : off_base + (unsigned)lev(j) * sm;
 #pragma unroll
                     for (int f = 0; f < NF; ++f) outb[f][oo] = o[f];
                 }
                 if (REDUCE) {                                        // CFL max-reduction of the new state (R12)
-                    Prim<ND> wo = primitives<ND>(o, gz_of(j), A);
-                    double s = 0.0;
-                    const double cs = sqrt_pos(A.gammaR * wo.T);
-#pragma unroll
-                    for (int c = 0; c < ND; ++c) s = fmax_nan(s, (fabs(wo.u[c]) + cs) * A.inv_d[c]);
-                    if (!(o[0] > 0.0) || !(wo.T > 0.0)) s = NAN;
-                    if (owner) smax = fmax_nan(smax, s);
+                    const double gzj = gz0;
+                    const bool need = owner && !cfl_can_skip<ND>(o, gzj, smax2, A);
+                    if (__any_sync(0xffffffffu, need)) {             // rare once the running maximum has settled
+                        const double s = cfl_speed<ND>(o, gzj, A);
+                        if (owner) { smax = fmax_nan(smax, s); smax2 = fmax_nan(smax2, (smax * smax) * (1.0 - 1e-6)); }
+                    }
                 }
             }
         }
@@ -251,7 +262,8 @@ MC_KERNEL void __maxnreg__((65536 / (32 * WB)) / 8 * 8) k_lane3(SweepArgs A)
         Xon[0] = Xoq[0]; Xon[1] = Xoq[1]; Xon[2] = Xoq[2];
         um0[0] = w1.u[CA]; um0[1] = w1.u[CM];
         uPm[0] = wP0.u[CA]; uPm[1] = wP0.u[CM];
-        w1 = w2; wP0 = wP1; hC0 = hC1; hC1 = hC2; gz1 = gz2;
+        w1 = w2; wP0 = wP1; hC0 = hC1; hC1 = hC2; gz0 = gz1; gz1 = gz2;
+        if (FAST) { o3c += sm; o0c += sm; kd2c += 1.0; }
     };
 
     auto march = [&](auto role_tag) MC_INL {
@@ -264,9 +276,11 @@ MC_KERNEL void __maxnreg__((65536 / (32 * WB)) / 8 * 8) k_lane3(SweepArgs A)
             load(j + 2, Xn);
             if (decltype(role_tag)::value == LROLE_R1) load_outer(j + 2, Xon);
         }
-        const int jf0 = WALL_M ? max(l0, 1) : l0;
-        const int jf1 = WALL_M ? min(l1, n - 3) : l1;
+        // fast levels: every level j-1 .. j+3 exists, none is a plate, none wraps around
+        const int jf0 = max(l0, 1);
+        const int jf1 = min(l1, n - 3);
         for (; j < l1 && (j < jf0 || (j & 1)); ++j) body(role_tag, slow, par_any, j);
+        if (j + 1 < jf1) { o3c = off_base + (unsigned)(j + 3) * sm; o0c = off_base + (unsigned)j * sm; kd2c = (double)(j + 2); }
         for (; j + 1 < jf1; j += 2) {
             body(role_tag, fast, integral_constant<int, 0>(), j);
             body(role_tag, fast, integral_constant<int, 1>(), j + 1);

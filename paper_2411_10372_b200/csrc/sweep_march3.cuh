@@ -90,7 +90,7 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
     const double cdt = tau * A.inv_h;                 // tau / dx_alpha of Eqs. 31-32, signed
     const double hcdt = 0.5 * cdt;
     const double half_tod = 0.5 * tau / A.d_a;        // for Co (R5)
-    const double tsrc = A.src ? -(tau * A.g) : 0.0;   // tau S: S = -g rho in the rho u_z row
+    const double tsrc = -(tau * A.g);                 // tau S: S = -g rho in the rho u_z row of the z-sweep only
     const int n = A.n_m;
     const int l0 = (int)blockIdx.z * A.chunk;
     const int l1 = min(n, l0 + A.chunk);
@@ -332,15 +332,17 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
                     XP[f] = fma(-cdt, dF, Xc[f]);
                     H1[f] = fma(-hcdt, dF, Xc[f]) - Dh[f];                    // (X^P + X)/2 - Dh
                 }
-                XP[1 + CA] = fma(tsrc, Xc[0], XP[1 + CA]);
-                H1[1 + CA] = fma(0.5 * tsrc, Xc[0], H1[1 + CA]);
+                if (Z_IS_ALPHA) {
+                    XP[1 + CA] = fma(tsrc, Xc[0], XP[1 + CA]);
+                    H1[1 + CA] = fma(0.5 * tsrc, Xc[0], H1[1 + CA]);
+                }
             }
             wP1 = primitives<ND>(XP, gz1, A);
             if (start_wall1 || end_wall1) {
 #pragma unroll
                 for (int f = 0; f < NF; ++f) H1[f] = 0.5 * (XP[f] + Xc[f]);
             } else {
-                H1[1 + CA] = fma(0.5 * tsrc, XP[0], H1[1 + CA]);             // + tau S(X^P)/2
+                if (Z_IS_ALPHA) H1[1 + CA] = fma(0.5 * tsrc, XP[0], H1[1 + CA]);   // + tau S(X^P)/2
             }
         }
         if (ld1) publish(slotP, p1, tidx, wP1.u);
