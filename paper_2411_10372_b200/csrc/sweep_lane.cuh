@@ -87,18 +87,25 @@ MC_KERNEL void __launch_bounds__(32 * WB, MINB) k_lane(SweepArgs A)
     const int n = A.n_m;
     const int l0 = (int)blockIdx.z * A.chunk;
     const int l1 = min(n, l0 + A.chunk);
-    const double *const pin = A.in + col;
-    double *const pout = A.out + col;
+    // Node offsets inside a field are 32-bit element counts (N < 2^32, mc_tvd_init).
+    const unsigned sm = (unsigned)A.s_m;
+    const unsigned off_base = (unsigned)col;
+    const int pf_last = min(l1 + 1, n - 1) - MC_SWEEP_L2PF;                  // last j + 3 whose L2 prefetch is issued
+    const double *inb[NF];
+    double *outb[NF];
+#pragma unroll
+    for (int f = 0; f < NF; ++f) { inb[f] = A.in + (long long)f * A.N; outb[f] = A.out + (long long)f * A.N; }
 
     auto exists = [&](int l) MC_INL { return WALL_M ? (l >= 0 && l < n) : true; };
     auto is_plate = [&](int l) MC_INL { return WALL_M && (l == 0 || l == n - 1); };
     auto lev = [&](int l) MC_INL { return WALL_M ? l : wrap1(l, n); };
     auto gz_of = [&](int l) MC_INL { return A.g * ((double)lev(l) * A.dz); };       // m is z
-    auto load = [&](int l, double (&X)[NF]) MC_INL {
-        const double *p = pin + (long long)lev(l) * A.s_m;
+    auto off_of = [&](int l) MC_INL { return off_base + (unsigned)lev(l) * sm; };
+    auto load_at = [&](unsigned o, double (&X)[NF]) MC_INL {
 #pragma unroll
-        for (int f = 0; f < NF; ++f) X[f] = p[(long long)f * A.N];
+        for (int f = 0; f < NF; ++f) X[f] = inb[f][o];
     };
+    auto load = [&](int l, double (&X)[NF]) MC_INL { load_at(off_of(l), X); };
     auto publish = [&](double *slot, int parity, const double (&u)[ND]) MC_INL {
         if (HAS_B) {
             slot[(parity * 2 + 0) * TILE + tidx] = u[0];
@@ -122,7 +129,10 @@ MC_KERNEL void __launch_bounds__(32 * WB, MINB) k_lane(SweepArgs A)
     double um0[2] = {0.0, 0.0};    // (u_x, u_m) of X(j)
     double uPm[2] = {0.0, 0.0};    // (u_x, u_m) of X^P(j-1)
     double hC0 = 0.0, hC1 = 0.0;   // C/2 of Eq. 39 at levels j, j+1
-    double gz1 = 0.0;
+    double gz1 = 0.0, gz0 = 0.0;   // g z of levels j+1, j
+    // fast levels only: node offsets of level j+3 (next load) and level j (next store), z index of level j+2
+    unsigned o3c = 0, o0c = 0;
+    double kd2c = 0.0;
     double smax = 0.0, smax2 = 0.0;   // running CFL maximum and smax^2 (1 - 1e-6) for the filter
     if (REDUCE) {
         // start the filter from the maximum other blocks have already recorded (the bottom, hottest chunks
@@ -149,12 +159,13 @@ MC_KERNEL void __launch_bounds__(32 * WB, MINB) k_lane(SweepArgs A)
         double Xq[NF];
 #pragma unroll
         for (int f = 0; f < NF; ++f) Xq[f] = Xn[f];
-        if (FAST || (exists(j + 3) && j + 3 <= l1 + 1)) load(j + 3, Xq);
+        const unsigned o3 = FAST ? o3c : off_of(j + 3);
+        if (FAST || (exists(j + 3) && j + 3 <= l1 + 1)) load_at(o3, Xq);
 #if MC_SWEEP_L2PF > 0
-        if (j + 3 + MC_SWEEP_L2PF <= l1 + 1 && exists(j + 3 + MC_SWEEP_L2PF)) {
-            const double *pp = pin + (long long)lev(j + 3 + MC_SWEEP_L2PF) * A.s_m;
+        if (FAST ? (j + 3 <= pf_last) : (j + 3 + MC_SWEEP_L2PF <= l1 + 1 && exists(j + 3 + MC_SWEEP_L2PF))) {
+            const unsigned op = FAST ? o3 + (unsigned)MC_SWEEP_L2PF * sm : off_of(j + 3 + MC_SWEEP_L2PF);
 #pragma unroll
-            for (int f = 0; f < NF; ++f) asm volatile("prefetch.global.L2 [%0];" ::"l"(pp + (long long)f * A.N));
+            for (int f = 0; f < NF; ++f) asm volatile("prefetch.global.L2 [%0];" ::"l"(inb[f] + op));
         }
 #endif
 
@@ -164,7 +175,7 @@ MC_KERNEL void __launch_bounds__(32 * WB, MINB) k_lane(SweepArgs A)
         Prim<ND> w2 = w1;
         double hC2 = 0.0, gz2 = 0.0;
         if (ex2) {
-            gz2 = gz_of(j + 2);
+            gz2 = FAST ? A.g * (kd2c * A.dz) : gz_of(j + 2);
             w2 = primitives<ND>(Xn, gz2, A);
             if (ROLE == LROLE_IN && TVD >= 0) hC2 = half_courant_coef(w2.u[CA], w2.T, half_tod, A);
             publish(slotU, p0, w2.u);                   // parity of level j+2
@@ -172,6 +183,8 @@ MC_KERNEL void __launch_bounds__(32 * WB, MINB) k_lane(SweepArgs A)
         if (ROLE == LROLE_R2) {
 #pragma unroll
             for (int f = 0; f < NF; ++f) Xn[f] = Xq[f];
+            gz0 = gz1; gz1 = gz2;
+            if (FAST) { o3c += sm; o0c += sm; kd2c += 1.0; }
             return;
         }
 
@@ -249,12 +262,12 @@ MC_KERNEL void __launch_bounds__(32 * WB, MINB) k_lane(SweepArgs A)
                     }
                 }
                 if (owner) {
-                    double *q = pout + (long long)lev(j) * A.s_m;
+                    const unsigned oo = FAST ? o0c : off_of(j);
 #pragma unroll
-                    for (int f = 0; f < NF; ++f) q[(long long)f * A.N] = o[f];
+                    for (int f = 0; f < NF; ++f) outb[f][oo] = o[f];
                 }
                 if (REDUCE) {                                        // CFL max-reduction of the new state (R12)
-                    const double gzj = gz_of(j);
+                    const double gzj = gz0;
                     const bool need = owner && !cfl_can_skip<ND>(o, gzj, smax2, A);
                     if (__any_sync(0xffffffffu, need)) {             // rare once the running maximum has settled
                         const double s = cfl_speed<ND>(o, gzj, A);
@@ -268,7 +281,8 @@ MC_KERNEL void __launch_bounds__(32 * WB, MINB) k_lane(SweepArgs A)
         for (int f = 0; f < NF; ++f) { X0[f] = X1[f]; X1[f] = Xn[f]; Xn[f] = Xq[f]; XP0[f] = XP1[f]; }
         um0[0] = w1.u[CA]; um0[1] = w1.u[CM];
         uPm[0] = wP0.u[CA]; uPm[1] = wP0.u[CM];
-        w1 = w2; wP0 = wP1; hC0 = hC1; hC1 = hC2; gz1 = gz2;
+        w1 = w2; wP0 = wP1; hC0 = hC1; hC1 = hC2; gz0 = gz1; gz1 = gz2;
+        if (FAST) { o3c += sm; o0c += sm; kd2c += 1.0; }
     };
 
     auto march = [&](auto role_tag) MC_INL {
@@ -278,9 +292,11 @@ MC_KERNEL void __launch_bounds__(32 * WB, MINB) k_lane(SweepArgs A)
         integral_constant<int, -1> par_any;
         int j = l0 - 4;
         if (exists(j + 2)) load(j + 2, Xn);
-        const int jf0 = WALL_M ? max(l0, 1) : l0;
-        const int jf1 = WALL_M ? min(l1, n - 3) : l1;
+        // fast levels: every level j-1 .. j+3 exists, none is a plate, none wraps around
+        const int jf0 = max(l0, 1);
+        const int jf1 = min(l1, n - 3);
         for (; j < l1 && (j < jf0 || (j & 1)); ++j) body(role_tag, slow, par_any, j);
+        if (j + 1 < jf1) { o3c = off_of(j + 3); o0c = off_of(j); kd2c = (double)(j + 2); }
         for (; j + 1 < jf1; j += 2) {
             body(role_tag, fast, integral_constant<int, 0>(), j);
             body(role_tag, fast, integral_constant<int, 1>(), j + 1);

@@ -91,27 +91,33 @@ MC_KERNEL void __launch_bounds__(WX * WB, MINB) k_march(SweepArgs A)
     const int n = A.n_m;
     const int l0 = (int)blockIdx.z * A.chunk;
     const int l1 = min(n, l0 + A.chunk);
-    const long long sm_signed = (A.dir > 0) ? A.s_m : -A.s_m;
-    const double *const pin = A.in + col + ((A.dir > 0) ? 0 : (long long)(n - 1) * A.s_m);
-    double *const pout = A.out + col + ((A.dir > 0) ? 0 : (long long)(n - 1) * A.s_m);
+    // Node offsets inside a field are 32-bit element counts (N < 2^32, mc_tvd_init) in modular arithmetic.
+    const unsigned sms = (unsigned)(int)((A.dir > 0) ? A.s_m : -A.s_m);
+    const unsigned off_base = (unsigned)(col + ((A.dir > 0) ? 0 : (long long)(n - 1) * A.s_m));
+    const double dsgn = (A.dir > 0) ? 1.0 : -1.0;
+    const int pf_last = min(l1 + 1, n - 1) - MC_SWEEP_L2PF;                  // last j + 3 whose L2 prefetch is issued
+    const double *inb[NF];
+    double *outb[NF];
+#pragma unroll
+    for (int f = 0; f < NF; ++f) { inb[f] = A.in + (long long)f * A.N; outb[f] = A.out + (long long)f * A.N; }
     const double gz_fixed = A.g * ((double)gb * A.dz);                       // used when b is z
 
     auto exists = [&](int l) MC_INL { return WALL_M ? (l >= 0 && l < n) : true; };
     auto lev = [&](int l) MC_INL { return WALL_M ? l : wrap1(l, n); };              // l in [-n, 2n)
+    auto off_of = [&](int l) MC_INL { return off_base + (unsigned)lev(l) * sms; };
+    auto phys_k = [&](int l) MC_INL { const int w = lev(l); return (A.dir > 0) ? w : n - 1 - w; };
     auto gz_of = [&](int l) MC_INL {                         // g z_k of Eq. 17 for this thread's node at level l
         if (!Z_IS_ALPHA) return gz_fixed;
-        const int w = lev(l);
-        return A.g * ((double)((A.dir > 0) ? w : n - 1 - w) * A.dz);
+        return A.g * ((double)phys_k(l) * A.dz);
     };
-    auto load = [&](int l, double (&X)[NF]) MC_INL {
-        const double *p = pin + (long long)lev(l) * sm_signed;
+    auto load_at = [&](unsigned o, double (&X)[NF]) MC_INL {
 #pragma unroll
-        for (int f = 0; f < NF; ++f) X[f] = p[(long long)f * A.N];
+        for (int f = 0; f < NF; ++f) X[f] = inb[f][o];
     };
-    auto store = [&](int l, const double (&o)[NF]) MC_INL {
-        double *q = pout + (long long)lev(l) * sm_signed;
+    auto load = [&](int l, double (&X)[NF]) MC_INL { load_at(off_of(l), X); };
+    auto store_at = [&](unsigned o, const double (&v)[NF]) MC_INL {
 #pragma unroll
-        for (int f = 0; f < NF; ++f) q[(long long)f * A.N] = o[f];
+        for (int f = 0; f < NF; ++f) outb[f][o] = v[f];
     };
     auto publish = [&](double *slot, int parity, const double (&u)[ND]) MC_INL {
 #pragma unroll
@@ -151,6 +157,10 @@ MC_KERNEL void __launch_bounds__(WX * WB, MINB) k_march(SweepArgs A)
     double hC0 = 0.0, hC1 = 0.0;   // C/2 of Eq. 39 at levels j, j+1
     double gz1 = 0.0;              // g z of level j+1
     Prim<ND> w1;                   // primitives of X(j+1)
+    // fast levels only: node offsets of level j+3 (next load) and level j (next store), and the
+    // z index of level j+2 as a double (exact; saves the int-to-double conversions of g z_k)
+    unsigned o3c = 0, o0c = 0;
+    double kd2c = 0.0;
 #pragma unroll
     for (int f = 0; f < NF; ++f) { Xn[f] = 0.0; Xc[f] = 0.0; F0[f] = 0.0; FP0[f] = 0.0; H0[f] = 0.0; d0[f] = 0.0; }
     Xn[0] = 1.0; Xc[0] = 1.0;
@@ -172,27 +182,30 @@ MC_KERNEL void __launch_bounds__(WX * WB, MINB) k_march(SweepArgs A)
         const bool start_wall1 = !FAST && WALL_M && (j + 1 == 0);     // level j+1 is the plate the march starts on
         const bool end_wall1 = !FAST && WALL_M && (j + 1 == n - 1);   // level j+1 is the plate the march ends on
 
-        if (ROLE == ROLE_NONE) { __syncthreads(); return; }
+        if (ROLE == ROLE_NONE) { __syncthreads(); if (FAST) { o3c += sms; o0c += sms; kd2c += dsgn; } return; }
 
         // (0) prefetch X(j+3) for the next iteration
         double Xq[NF];
 #pragma unroll
         for (int f = 0; f < NF; ++f) Xq[f] = Xn[f];
-        if (FAST || (exists(j + 3) && j + 3 <= l1 + 1)) load(j + 3, Xq);
+        const unsigned o3 = FAST ? o3c : off_of(j + 3);
+        const unsigned o0 = FAST ? o0c : off_of(j);
+        if (FAST || (exists(j + 3) && j + 3 <= l1 + 1)) load_at(o3, Xq);
 #if MC_SWEEP_L2PF > 0
         // far-ahead L2 prefetch: the one-level register prefetch alone leaves the HBM latency exposed
-        if (j + 3 + MC_SWEEP_L2PF <= l1 + 1 && exists(j + 3 + MC_SWEEP_L2PF)) {
-            const double *pp = pin + (long long)lev(j + 3 + MC_SWEEP_L2PF) * sm_signed;
+        if (FAST ? (j + 3 <= pf_last) : (j + 3 + MC_SWEEP_L2PF <= l1 + 1 && exists(j + 3 + MC_SWEEP_L2PF))) {
+            const unsigned op = FAST ? o3 + (unsigned)MC_SWEEP_L2PF * sms : off_of(j + 3 + MC_SWEEP_L2PF);
 #pragma unroll
-            for (int f = 0; f < NF; ++f) asm volatile("prefetch.global.L2 [%0];" ::"l"(pp + (long long)f * A.N));
+            for (int f = 0; f < NF; ++f) asm volatile("prefetch.global.L2 [%0];" ::"l"(inb[f] + op));
         }
 #endif
+        auto advance = [&]() MC_INL { if (FAST) { o3c += sms; o0c += sms; kd2c += dsgn; } };
 
         // (1) W(j+2): primitives, Courant coefficient, publish velocities
         Prim<ND> w2 = w1;
         double hC2 = 0.0, gz2 = 0.0;
         if (ld2) {
-            gz2 = gz_of(j + 2);
+            gz2 = (FAST && Z_IS_ALPHA) ? A.g * (kd2c * A.dz) : gz_of(j + 2);
             w2 = primitives<ND>(Xn, gz2, A);
             if (ROLE == ROLE_IN && TVD >= 0) hC2 = half_courant_coef(w2.u[CA], w2.T, half_tod, A);
             publish(slotU, p2, w2.u);
@@ -201,16 +214,18 @@ MC_KERNEL void __launch_bounds__(WX * WB, MINB) k_march(SweepArgs A)
             __syncthreads();
 #pragma unroll
             for (int f = 0; f < NF; ++f) Xn[f] = Xq[f];
+            advance();
             return;
         }
         if (ROLE == ROLE_WALLROW) {
             // a plate row of b (y-sweep): X^P = X and the output is X (R10); publish u^P = u of level j+1
             if (ld1) publish(slotP, p1, w1.u);
             __syncthreads();
-            if (j >= l0 && owner) store(j, H0);
+            if (j >= l0 && owner) store_at(o0, H0);
 #pragma unroll
             for (int f = 0; f < NF; ++f) { H0[f] = Xc[f]; Xc[f] = Xn[f]; Xn[f] = Xq[f]; }
             w1 = w2;
+            advance();
             return;
         }
 
@@ -305,7 +320,7 @@ MC_KERNEL void __launch_bounds__(WX * WB, MINB) k_march(SweepArgs A)
 #pragma unroll
                     for (int f = 0; f < NF; ++f) o[f] = fma(-hcdt, FP1[f] - FP0[f], H0[f]);
                 }
-                if (owner) store(j, o);
+                if (owner) store_at(o0, o);
             }
 #pragma unroll
             for (int f = 0; f < NF; ++f) { FP0[f] = FP1[f]; d0[f] = d1[f]; }
@@ -318,6 +333,7 @@ MC_KERNEL void __launch_bounds__(WX * WB, MINB) k_march(SweepArgs A)
 #pragma unroll
         for (int f = 0; f < NF; ++f) { Xc[f] = Xn[f]; Xn[f] = Xq[f]; F0[f] = F1[f]; H0[f] = H1[f]; }
         w1 = w2; gz1 = gz2;
+        advance();
     };
 
     // ---- the march -------------------------------------------------------------------------------
@@ -328,9 +344,11 @@ MC_KERNEL void __launch_bounds__(WX * WB, MINB) k_march(SweepArgs A)
         integral_constant<int, -1> par_any;
         int j = l0 - 4;
         if (exists(j + 2)) load(j + 2, Xn);
-        const int jf0 = WALL_M ? max(l0, 1) : l0;
-        const int jf1 = WALL_M ? min(l1, n - 3) : l1;
+        // fast levels: every level j-1 .. j+3 exists, none is a plate, none wraps around
+        const int jf0 = max(l0, 1);
+        const int jf1 = min(l1, n - 3);
         for (; j < l1 && (j < jf0 || (j & 1)); ++j) body(role_tag, slow, par_any, j);
+        if (j + 1 < jf1) { o3c = off_of(j + 3); o0c = off_of(j); kd2c = (double)phys_k(j + 2); }
         for (; j + 1 < jf1; j += 2) {
             body(role_tag, fast, integral_constant<int, 0>(), j);
             body(role_tag, fast, integral_constant<int, 1>(), j + 1);
