@@ -162,7 +162,7 @@ MC_KERNEL void __maxnreg__((65536 / (32 * WB)) / 8 * 8) k_lane3(SweepArgs A)
             if (ROLE == LROLE_IN && TVD >= 0) hC2 = half_courant_coef(w2.u[CA], w2.T, half_tod, A);
             publish(slotU, p0, w2.u);                   // parity of level j+2
             if (ROLE == LROLE_R1) {                     // side job: (u_x, u_b) of the ring-2 row
-                const double inv = rcp(Xon[0]);
+                const double inv = rcp_fast(Xon[0]);
                 slotU[(p0 * 2 + 0) * TILE + tidx_o] = Xon[1] * inv;
                 slotU[(p0 * 2 + 1) * TILE + tidx_o] = Xon[2] * inv;
             }

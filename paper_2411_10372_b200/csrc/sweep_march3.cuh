@@ -220,7 +220,7 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
         if (ROLE == ROLE_IN && TVD >= 0) hC = half_courant_coef(w.u[CA], w.T, half_tod, A);
         publish(slotU, par, tidx, w.u);
         if (ROLE == ROLE_R1) {
-            const double inv = rcp(Xo[0]);
+            const double inv = rcp_fast(Xo[0]);
             double uo[ND];
 #pragma unroll
             for (int c = 0; c < ND; ++c) uo[c] = Xo[1 + c] * inv;
