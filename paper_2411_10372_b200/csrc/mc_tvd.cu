@@ -285,7 +285,7 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
             long long bt = (ny + MO - 1) / MO;
             A.chunk = pick_chunk(s, nz, xt * bt, 1);
             dim3 mblock(32, MW, 1), grid((unsigned)xt, (unsigned)bt, (unsigned)((nz + A.chunk - 1) / A.chunk));
-            size_t smem = ((size_t)4 * 3 * 32 * (MW + 2) + 8) * sizeof(double);
+            size_t smem = ((size_t)4 * 3 * 32 * (MW + 2) + 4) * sizeof(double);
             with_walls(wl, [&](auto W) { with_tvd(s, [&](auto T) {
                 launch_kernel(mc::k_march3<2, 1, MW, decltype(W)::value, false, decltype(T)::value, MC_MARCH3_MINB>, grid, mblock, smem, st, A);
             }); });
@@ -295,7 +295,7 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
             long long bt = (nz + MO - 1) / MO;
             A.chunk = pick_chunk(s, ny, xt * bt, 1);
             dim3 mblock(32, MW, 1), grid((unsigned)xt, (unsigned)bt, (unsigned)((ny + A.chunk - 1) / A.chunk));
-            size_t smem = ((size_t)4 * 3 * 32 * (MW + 2) + 8) * sizeof(double);
+            size_t smem = ((size_t)4 * 3 * 32 * (MW + 2) + 4) * sizeof(double);
             with_walls(wl, [&](auto W) { with_tvd(s, [&](auto T) {
                 launch_kernel(mc::k_march3<1, 2, MW, false, decltype(W)::value, decltype(T)::value, MC_MARCH3_MINB>, grid, mblock, smem, st, A);
             }); });

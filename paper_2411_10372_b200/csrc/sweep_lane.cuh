@@ -1,5 +1,7 @@
 // sweep_lane.cuh -- kernel k_lane: the operator L_x(tau) of Eqs. 31-39, i.e. the
-// sweep along the fastest (x) axis, in 2-D and 3-D.
+// sweep along the fastest (x) axis.  The library launches it for the 2-D box (independent warps, no
+// barrier, no shared memory); the 3-D box has its own kernel (k_lane3, sweep_lane3.cuh), so the tile
+// rows along b below (HAS_B) are instantiated only by developer builds.
 //
 // Design: a warp owns 32 consecutive x columns (28 outputs + a 2-node halo on
 // each side), so every along-alpha neighbour -- the predictor flux F_{i-1}, the corrector flux

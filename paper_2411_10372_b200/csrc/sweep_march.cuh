@@ -1,5 +1,7 @@
 // sweep_march.cuh -- kernel k_march: one operator L_alpha(tau) of Eqs. 31-39
-// for a sweep axis alpha that is NOT the fastest (x) axis: the z-sweep (2-D, 3-D) and the y-sweep (3-D).
+// for a sweep axis alpha that is NOT the fastest (x) axis.  The library launches it for the 2-D z-sweep
+// (blocks of 128 columns, 124 outputs); the 3-D box has its own kernel (k_march3, sweep_march3.cuh), so
+// the (x, b) tile roles below (HAS_B) are instantiated only by developer builds.
 //
 // Design: one thread owns one grid column along alpha and MARCHES along it,
 // keeping every along-alpha neighbour (predictor flux F_{k-1}, corrector flux F^P_{k+1}, the five-node

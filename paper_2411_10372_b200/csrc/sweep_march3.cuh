@@ -9,8 +9,9 @@
 // ring-1 halo (role R1: predictor only, because the corrector flux of an output row differentiates
 // u^P across b, R7).  The ring-2 halo (the predictor of a ring-1 row differentiates u across b) needs
 // only the velocities of X, so the ring-1 warp computes them for its outer neighbour row as a side
-// job instead of parking two more warps on it: 12 of 14 warps do full work (28 x 12 outputs per 448
-// threads).  In x, lanes 0, 1, 30, 31 are the halo: they compute along and never store.
+// job instead of parking two more warps on it: 10 of 12 warps do full work (28 x 10 outputs per 384
+// threads; the SM allocates warps in fours, and 16 rows at 128 registers spill -- measured slower).
+// In x, lanes 0, 1, 30, 31 are the halo: they compute along and never store.
 // Velocities travel through shared memory, one plane per level, double buffered, ONE barrier per level.
 //
 // Pipeline of iteration j (output level j), identical to k_march:
@@ -26,16 +27,11 @@ namespace mc {
 // CA: velocity component of alpha; CB: velocity component of the tile's second direction b;
 // WB: tile rows (warps) per block; WALL_M / WALL_B: the marching / second direction is z with plates;
 // TVD: -1 no TVD term, 0 Eq. 34 as printed, 1 Davis/Yee (R4).
-// Register budget: one block per SM, 65536 / (32 WB) registers per thread rounded down to a multiple of 8
-// (__launch_bounds__ alone rounds the block up to 512 threads and would give 128).
+// Register budget: MINB blocks per SM, 65536 / (32 WB MINB) registers per thread rounded down to a multiple
+// of 8 (__maxnreg__, because __launch_bounds__ rounds the block size up to a multiple of 128 threads).
+// MC_MARCH3_L2PF: levels between the register prefetch and the L2 prefetch (4 measured best of 2..8).
 #ifndef MC_MARCH3_L2PF
 #define MC_MARCH3_L2PF 4
-#endif
-#ifndef MC_MARCH3_LATE_LOAD
-#define MC_MARCH3_LATE_LOAD 0
-#endif
-#ifndef MC_MARCH3_SYNC
-#define MC_MARCH3_SYNC 0
 #endif
 #ifndef MC_MARCH3_REGS
 #define MC_MARCH3_REGS ((65536 / (32 * WB * MINB)) / 8 * 8)
@@ -46,10 +42,10 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
     constexpr int ND = 3, NF = 5;
     constexpr bool Z_IS_ALPHA = (CA == ND - 1);
     constexpr int OB = WB - 2;                        // output rows per tile
-    static_assert(WB >= 3 && WB <= 16, "the progress flags occupy 64 bytes");
+    static_assert(WB >= 3 && WB % 4 == 0, "the SM allocates warps in fours: other row counts waste registers");
     constexpr int TILE = 32 * (WB + 2);               // shared-memory plane: tile rows plus the ring-2 rows
     MC_SHARED_DECL(double, smem_raw);
-    double *const smem = smem_raw + 8;                // 64 bytes in front: the rows' progress flags
+    double *const smem = smem_raw + 2;                // two pad doubles in front
     double *const slotU = smem;                       // [2][ND][TILE]  velocities of X     (levels j+1, j+2)
     double *const slotP = smem + 2 * ND * TILE;       // [2][ND][TILE]  velocities of X^P   (level j+1)
 
@@ -161,30 +157,6 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
     };
 
 
-    // ---- per-level synchronisation ---------------------------------------------------------------
-    // A row exchanges velocities only with its two neighbour rows, so instead of a block-wide barrier
-    // each warp publishes "my planes of iteration j are written" in a shared flag (release) and waits
-    // for the flags of its two neighbour rows (acquire): rows drift apart instead of all waiting for
-    // the slowest one each level.  Slot reuse is safe with two planes per slot: a row that has passed
-    // the wait of iteration j-1 knows its neighbours finished every read of iteration j-2.
-    int *const flags = reinterpret_cast<int *>(smem_raw);           // [WB] ints in the 16 pad bytes..
-    const bool nb_lo = MC_MARCH3_SYNC && ty > 0 && (!WALL_B || (gb_raw - 1 >= 0 && gb_raw - 1 < A.n_b));
-    const bool nb_hi = MC_MARCH3_SYNC && ty < WB - 1 && (!WALL_B || (gb_raw + 1 >= 0 && gb_raw + 1 < A.n_b));
-    const unsigned flag_me = (unsigned)__cvta_generic_to_shared(flags + ty);
-    if (MC_MARCH3_SYNC) {
-        if (tx == 0) flags[ty] = l0 - 5;
-        __syncthreads();
-    }
-    auto level_sync = [&](int j) MC_INL {
-        if (!MC_MARCH3_SYNC) { __syncthreads(); return; }
-        __syncwarp();
-        if (tx == 0) asm volatile("st.release.cta.shared.b32 [%0], %1;" ::"r"(flag_me), "r"(j) : "memory");
-        int v;
-        if (nb_lo) do { asm volatile("ld.acquire.cta.shared.b32 %0, [%1];" : "=r"(v) : "r"(flag_me - 4) : "memory"); } while (v < j);
-        if (nb_hi) do { asm volatile("ld.acquire.cta.shared.b32 %0, [%1];" : "=r"(v) : "r"(flag_me + 4) : "memory"); } while (v < j);
-        __syncwarp();
-    };
-
     // ---- carried state (levels relative to the current output level j) -------------------------
     double Xn[NF];                 // X(j+2)
     double Xc[NF];                 // X(j+1)
@@ -244,10 +216,9 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
         const bool start_wall1 = !FAST && WALL_M && (j + 1 == 0);     // level j+1 is the plate the march starts on
         const bool end_wall1 = !FAST && WALL_M && (j + 1 == n - 1);   // level j+1 is the plate the march ends on
 
-        if (ROLE == ROLE_NONE) { if (!MC_MARCH3_SYNC) __syncthreads(); return; }
+        if (ROLE == ROLE_NONE) { __syncthreads(); return; }
 
-        // (0) prefetch X(j+3): far ahead into L2 here, into registers after the barrier (the loads then
-        // do not overlap the register peak of the flux / predictor stages)
+        // (0) prefetch X(j+3) into registers and X(j+3+MC_MARCH3_L2PF) into L2
         const bool ld3 = FAST || (ex3 && j + 3 <= l1 + 1);
 #if MC_MARCH3_L2PF > 0
         if (FAST) { if (j + 3 <= pf_last) prefetch_l2(o3 + (unsigned)MC_MARCH3_L2PF * sms); }
@@ -262,7 +233,7 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
             for (int f = 0; f <= ND; ++f) Xoq[f] = Xon[f];
             if (ROLE == ROLE_R1 && ld3 && has_outer) load_outer(o3 - off_base + off_base_o, Xoq);
         };
-        if (MC_MARCH3_LATE_LOAD == 0 || ROLE != ROLE_IN) fetch();
+        fetch();
 
         // (1) W(j+2)
         Prim<ND> w2 = w1;
@@ -275,7 +246,7 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
         if (ROLE == ROLE_WALLROW) {
             // a plate row of b (y-sweep): X^P = X and the output is X (R10); publish u^P = u of level j+1
             if (ld1) publish(slotP, p1, tidx, w1.u);
-            level_sync(j);
+            __syncthreads();
             if (j >= l0 && owner) store_at(o0, H0);
 #pragma unroll
             for (int f = 0; f < NF; ++f) { H0[f] = Xc[f]; Xc[f] = Xn[f]; Xn[f] = Xq[f]; }
@@ -347,8 +318,7 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
         }
         if (ld1) publish(slotP, p1, tidx, wP1.u);
 
-        level_sync(j);
-        if (MC_MARCH3_LATE_LOAD != 0 && ROLE == ROLE_IN) fetch();
+        __syncthreads();
 
         if (ROLE == ROLE_IN) {
             // (5) F^P(j+1): flux of X^P at level j+1 (inner derivative backward in marching coordinates)
