@@ -183,7 +183,8 @@ void fill_common(const mc_tvd_state *s, mc::SweepArgs &A, const double *in, doub
 // Marching levels per block.  Cutting the march into c chunks multiplies the blocks (fills the SMs, evens
 // out the last wave) but every chunk repeats a 4-level warm-up.  Model: blocks run in waves of
 // (SMs x resident blocks per SM) and the last wave costs about half a block more than its share;
-// cost(c) = max(whole waves, waves + 1/2) x (levels per chunk + 4).  Take the cheapest c.
+// cost(c) = max(whole waves, waves + 1/2) x (levels per chunk + 8): the 4 warm-up levels run the general
+// loop body, about twice the cost of a fast level.  Take the cheapest c.
 int pick_chunk(const mc_tvd_state *s, int n_m, long long tiles, int blocks_per_sm)
 {
     if (s->chunk_override > 0) return s->chunk_override < n_m ? s->chunk_override : n_m;
@@ -195,7 +196,7 @@ int pick_chunk(const mc_tvd_state *s, int n_m, long long tiles, int blocks_per_s
         const int chunk = (n_m + c - 1) / c;
         const long long blocks = tiles * ((n_m + chunk - 1) / chunk);
         const long long whole = 2 * ((blocks + slots - 1) / slots), frac = (2 * blocks + slots - 1) / slots + 1;
-        const long long cost = (whole > frac ? whole : frac) * (chunk + 4);      // in half waves
+        const long long cost = (whole > frac ? whole : frac) * (chunk + 8);      // in half waves
         if (best_cost < 0 || cost < best_cost) { best_cost = cost; best_chunk = chunk; }
     }
     return best_chunk;

@@ -33,6 +33,9 @@ namespace mc {
 #ifndef MC_MARCH3_L2PF
 #define MC_MARCH3_L2PF 4
 #endif
+#ifndef MC_MARCH3_TVD_LATE
+#define MC_MARCH3_TVD_LATE 0
+#endif
 #ifndef MC_MARCH3_REGS
 #define MC_MARCH3_REGS ((65536 / (32 * WB * MINB)) / 8 * 8)
 #endif
@@ -259,18 +262,21 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
         double d1[NF], Dh[NF], a1 = 0.0, b1 = 0.0;
 #pragma unroll
         for (int f = 0; f < NF; ++f) { Dh[f] = 0.0; d1[f] = 0.0; }
-        if (ROLE == ROLE_IN && TVD >= 0) {
+        auto stage_TVD = [&]() MC_INL {
+            if (ROLE == ROLE_IN && TVD >= 0) {
 #pragma unroll
-            for (int f = 0; f < NF; ++f) d1[f] = (ld1 && ld2) ? Xn[f] - Xc[f] : 0.0;
+                for (int f = 0; f < NF; ++f) d1[f] = (ld1 && ld2) ? Xn[f] - Xc[f] : 0.0;
 #pragma unroll
-            for (int f = 0; f < NF; ++f) { b1 = fma(d1[f], d1[f], b1); a1 = fma(d0[f], d1[f], a1); }
-            const bool have = FAST || ((j >= l0 - 1) && exists(j - 1) && exists(j) && ex1 && ex2);   // R11 at plates
-            if (have) {
-                const double coef = tvd_coef<(TVD >= 0 ? TVD : 0)>(a0, a1, b0, hC0, hC1);
+                for (int f = 0; f < NF; ++f) { b1 = fma(d1[f], d1[f], b1); a1 = fma(d0[f], d1[f], a1); }
+                const bool have = FAST || ((j >= l0 - 1) && exists(j - 1) && exists(j) && ex1 && ex2);   // R11 at plates
+                if (have) {
+                    const double coef = tvd_coef<(TVD >= 0 ? TVD : 0)>(a0, a1, b0, hC0, hC1);
 #pragma unroll
-                for (int f = 0; f < NF; ++f) { Dh[f] = coef * d0[f]; H0[f] += Dh[f]; }
+                    for (int f = 0; f < NF; ++f) { Dh[f] = coef * d0[f]; H0[f] += Dh[f]; }
+                }
             }
-        }
+        };
+        if (!MC_MARCH3_TVD_LATE) stage_TVD();
 
         // (3) F(j+1): flux of X at level j+1 (inner derivative forward in marching coordinates)
         double F1[NF], XP[NF], H1[NF];
@@ -301,7 +307,8 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
                 for (int f = 0; f < NF; ++f) {
                     const double dF = F1[f] - F0[f];
                     XP[f] = fma(-cdt, dF, Xc[f]);
-                    H1[f] = fma(-hcdt, dF, Xc[f]) - Dh[f];                    // (X^P + X)/2 - Dh
+                    H1[f] = fma(-hcdt, dF, Xc[f]);                            // (X^P + X)/2
+                    if (!MC_MARCH3_TVD_LATE) H1[f] -= Dh[f];                  // - Dh
                 }
                 if (Z_IS_ALPHA) {
                     XP[1 + CA] = fma(tsrc, Xc[0], XP[1 + CA]);
@@ -320,6 +327,11 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
 
         __syncthreads();
 
+        if (MC_MARCH3_TVD_LATE) {      // the TVD term after the barrier: its temporaries stay out of the predictor's way
+            stage_TVD();
+#pragma unroll
+            for (int f = 0; f < NF; ++f) H1[f] -= Dh[f];
+        }
         if (ROLE == ROLE_IN) {
             // (5) F^P(j+1): flux of X^P at level j+1 (inner derivative backward in marching coordinates)
             double FP1[NF];

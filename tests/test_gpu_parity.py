@@ -185,6 +185,27 @@ def test_3d_steps(gpu, orc):
     s.close()
 
 
+@pytest.mark.parametrize("ndim,nx,ny,nz,chunk", [(2, 300, 1, 70, 0), (2, 300, 1, 70, 9), (3, 60, 21, 19, 0), (3, 60, 21, 19, 5)])
+def test_cfl_reduction_is_exact_every_step(gpu, orc, monkeypatch, ndim, nx, ny, nz, chunk):
+    """The CFL max-reduction is folded into the last operator behind a division-free filter that skips
+    nodes which cannot raise the maximum already recorded (csrc/mc_common.cuh cfl_can_skip).  It must stay
+    EXACT: after every step dt equals the oracle's dt of the same (downloaded) state to an ulp or two, on a
+    state whose fastest node is in the interior and moves, with several marching chunks per column."""
+    if chunk:
+        monkeypatch.setenv("MC_TVD_CHUNK", str(chunk))
+    grid = inputs.make_grid(ndim, nx, nz, ny)
+    params = inputs.make_params(Ra=1e4)
+    X0 = inputs.smooth_random_state(grid, params, seed=23)
+    prob = orc.Problem(grid, params)
+    s = _solver(gpu, grid, params, X0)
+    assert abs(s.dt() - orc.dt(prob, X0)) <= 4e-16 * s.dt()
+    for _ in range(6):
+        s.step(1)
+        dt_gpu = s.dt()
+        assert abs(dt_gpu - orc.dt(prob, s.state())) <= 4e-16 * dt_gpu
+    s.close()
+
+
 # ---- properties that hold at any size --------------------------------------------------------------
 def test_uniform_state_is_a_fixed_point(gpu):
     """Every flux difference and dX is exactly zero: the state must not change in a single bit."""
