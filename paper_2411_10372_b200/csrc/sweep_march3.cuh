@@ -33,9 +33,6 @@ namespace mc {
 #ifndef MC_MARCH3_L2PF
 #define MC_MARCH3_L2PF 4
 #endif
-#ifndef MC_MARCH3_TVD_LATE
-#define MC_MARCH3_TVD_LATE 0
-#endif
 #ifndef MC_MARCH3_REGS
 #define MC_MARCH3_REGS ((65536 / (32 * WB * MINB)) / 8 * 8)
 #endif
@@ -262,7 +259,7 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
         double d1[NF], Dh[NF], a1 = 0.0, b1 = 0.0;
 #pragma unroll
         for (int f = 0; f < NF; ++f) { Dh[f] = 0.0; d1[f] = 0.0; }
-        auto stage_TVD = [&]() MC_INL {
+        {
             if (ROLE == ROLE_IN && TVD >= 0) {
 #pragma unroll
                 for (int f = 0; f < NF; ++f) d1[f] = (ld1 && ld2) ? Xn[f] - Xc[f] : 0.0;
@@ -275,8 +272,7 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
                     for (int f = 0; f < NF; ++f) { Dh[f] = coef * d0[f]; H0[f] += Dh[f]; }
                 }
             }
-        };
-        if (!MC_MARCH3_TVD_LATE) stage_TVD();
+        }
 
         // (3) F(j+1): flux of X at level j+1 (inner derivative forward in marching coordinates)
         double F1[NF], XP[NF], H1[NF];
@@ -307,8 +303,7 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
                 for (int f = 0; f < NF; ++f) {
                     const double dF = F1[f] - F0[f];
                     XP[f] = fma(-cdt, dF, Xc[f]);
-                    H1[f] = fma(-hcdt, dF, Xc[f]);                            // (X^P + X)/2
-                    if (!MC_MARCH3_TVD_LATE) H1[f] -= Dh[f];                  // - Dh
+                    H1[f] = fma(-hcdt, dF, Xc[f]) - Dh[f];                    // (X^P + X)/2 - Dh
                 }
                 if (Z_IS_ALPHA) {
                     XP[1 + CA] = fma(tsrc, Xc[0], XP[1 + CA]);
@@ -327,11 +322,6 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
 
         __syncthreads();
 
-        if (MC_MARCH3_TVD_LATE) {      // the TVD term after the barrier: its temporaries stay out of the predictor's way
-            stage_TVD();
-#pragma unroll
-            for (int f = 0; f < NF; ++f) H1[f] -= Dh[f];
-        }
         if (ROLE == ROLE_IN) {
             // (5) F^P(j+1): flux of X^P at level j+1 (inner derivative backward in marching coordinates)
             double FP1[NF];
