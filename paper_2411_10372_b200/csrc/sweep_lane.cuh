@@ -76,7 +76,7 @@ MC_KERNEL void __launch_bounds__(32 * WB, MINB) k_lane(SweepArgs A)
     if (HAS_B) {
         gb = (int)blockIdx.y * (WB - 4) + ty - 2;
         rb = min(ty, WB - 1 - ty);
-        col += (long long)wrap1(gb, A.n_b) * A.s_b;
+        col += (long long)wrap(gb, A.n_b) * A.s_b;
     }
     const bool owner = warp_on && rb >= 2 && (!HAS_B || gb < A.n_b) && xi >= 2 && xi < 2 + LANE_OUT && gx >= 0 &&
                        gx < A.nx;

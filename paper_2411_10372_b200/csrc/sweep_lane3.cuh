@@ -52,8 +52,8 @@ MC_KERNEL void __maxnreg__((65536 / (32 * WB)) / 8 * 8) k_lane3(SweepArgs A)
     const bool edge = (ty == 0 || ty == WB - 1);
     const int gb = (int)blockIdx.y * OB + ty - 1;
     const int go = gb + (ty == 0 ? -1 : 1);             // the ring-2 row beyond an edge row
-    const unsigned off_base = (unsigned)(ix + (long long)wrap1(gb, A.n_b) * A.s_b);
-    const unsigned off_base_o = (unsigned)(ix + (long long)wrap1(go, A.n_b) * A.s_b);
+    const unsigned off_base = (unsigned)(ix + (long long)wrap(gb, A.n_b) * A.s_b);
+    const unsigned off_base_o = (unsigned)(ix + (long long)wrap(go, A.n_b) * A.s_b);
     const int tidx_o = tidx + (ty == 0 ? -32 : 32);
     const bool owner = warp_on && !edge && gb < A.n_b && xi >= 2 && xi < 2 + LANE_OUT && gx >= 0 && gx < A.nx;
 

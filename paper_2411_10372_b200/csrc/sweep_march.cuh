@@ -57,7 +57,7 @@ MC_KERNEL void __launch_bounds__(WX * WB, MINB) k_march(SweepArgs A)
 
     // ---- tile geometry --------------------------------------------------------------------
     const int gx = (int)blockIdx.x * (WX - 4) + tx - 2;
-    const int ix = wrap1(gx, A.nx);                   // nx >= 4 (mc_tvd_init) and gx in [-2, nx + WX)
+    const int ix = wrap(gx, A.nx);                    // any nx >= 4: a tile may wrap the seam more than once
     const int rx = min(tx, WX - 1 - tx);
     int gb = 0, rb = 99;
     bool row_exists = true, wallrow = false, row_in_range = true;
@@ -71,7 +71,7 @@ MC_KERNEL void __launch_bounds__(WX * WB, MINB) k_march(SweepArgs A)
             wallrow = (gb_raw == 0 || gb_raw == A.n_b - 1);
             gb = row_exists ? gb_raw : 0;
         } else {
-            gb = wrap1(gb_raw, A.n_b);                // periodic b: the node's own index
+            gb = wrap(gb_raw, A.n_b);                 // periodic b: the node's own index
         }
         col += (long long)gb * A.s_b;
     }

@@ -55,7 +55,7 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
 
     // ---- tile geometry --------------------------------------------------------------------
     const int gx = (int)blockIdx.x * 28 + tx - 2;
-    const int ix = wrap1(gx, A.nx);                   // nx >= 4 (mc_tvd_init) and gx in [-2, nx + 32)
+    const int ix = wrap(gx, A.nx);                    // any nx >= 4: a tile may wrap the seam more than once
     const int rx = min(tx, 31 - tx);
     const bool edge = (ty == 0 || ty == WB - 1);
     const int gb_raw = (int)blockIdx.y * OB + ty - 1;
@@ -69,8 +69,8 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
         has_outer = edge && row_exists && !wallrow && go_raw >= 0 && go_raw < A.n_b;
         go = has_outer ? go_raw : 0;
     } else {
-        gb = wrap1(gb_raw, A.n_b);                    // periodic b: the node's own index
-        go = wrap1(go_raw, A.n_b);
+        gb = wrap(gb_raw, A.n_b);                     // periodic b: the node's own index
+        go = wrap(go_raw, A.n_b);
     }
     const long long col = ix + (long long)gb * A.s_b;
     const long long col_o = ix + (long long)go * A.s_b;

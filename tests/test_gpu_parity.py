@@ -38,6 +38,8 @@ SWEEP_GRIDS = [
     (2, 29, 1, 5),        # smallest plate problem, one ragged tile
     (3, 60, 21, 19),      # 3-D: 3 x-tiles, 3 b-tiles (8 outputs) with ragged tails, walls in b for Ly
     (3, 30, 9, 33),       # ragged the other way
+    (2, 4, 1, 5),         # the smallest boxes the ABI accepts: a tile wraps the periodic seam several times
+    (3, 6, 4, 6),
 ]
 
 
