@@ -272,6 +272,10 @@ def run_ours(args):
     solver.timing_enable(False)
     dt_now = solver.dt()                                             # raises if the state went non-finite
     diag, *_ = solver.diagnostics()
+    torch.cuda.synchronize()
+    t_d = time.perf_counter()
+    diag, *_ = solver.diagnostics()                                  # synchronises: plane sums + finish + D2H
+    diag_ms = (time.perf_counter() - t_d) * 1e3
 
     ms_max = max_over_ranks(ms, world, f"cuda:{local}")
     value = job_value(world, N, args.steps, ms_max)
@@ -335,6 +339,7 @@ def run_ours(args):
         "config": workload_config(name, grid, params),
         "clocks": clocks.summary(), "gpu_launches": int(launches),
         "roofline": roofline,
+        "diagnostics_ms": diag_ms,
         "state_check": {"dt": dt_now, "nu_bar": diag["nu_bar"], "min_rho": diag["min_rho"], "min_T": diag["min_T"],
                         "steps_taken": diag["step"]},
     }

@@ -58,10 +58,10 @@ constexpr int MARCH3_WB = MC_MARCH3_WB;          // k_march3: 32 x WB threads, 2
 constexpr int LANE3_WB = MC_LANE3_WB;            // k_lane3: 32 x WB threads, 28 x (WB - 2) outputs
 constexpr int LANE_WARPS_2D = MC_LANE_WARPS_2D;  // k_lane, 2-D: independent warps per block
 constexpr int LANE_MINB_2D = MC_LANE_MINB_2D;
-constexpr int DIAG_MAX_BLOCKS = 64;    // blocks per plane in the diagnostics pass
+constexpr int DIAG_MAX_BLOCKS = 16;    // blocks per plane in the diagnostics pass (the finish kernel walks them)
 
 struct Layout {                        // byte offsets inside the workspace
-    size_t Y, scalars, partial, ext, plane_sums, diag_out, total;
+    size_t Y, scalars, partial, ext, plane_sums, plane_ext, diag_out, total;
     int diag_blocks;
 };
 
@@ -77,7 +77,7 @@ struct mc_tvd_state {
     bool walls;
     double *X, *Y;
     mc::Scalars *S;
-    double *partial, *ext, *plane_sums, *diag_out;
+    double *partial, *ext, *plane_sums, *plane_ext, *diag_out;
     int diag_blocks;
     cudaStream_t stream;
     long long launches;
@@ -131,6 +131,7 @@ Layout make_layout(const mc_tvd_grid *g)
     L.partial = o;    o = align_up(o + (size_t)g->nz * nb * 2 * mc::DQ_MAXQ * sizeof(double), 256);
     L.ext = o;        o = align_up(o + (size_t)g->nz * nb * 3 * sizeof(double), 256);
     L.plane_sums = o; o = align_up(o + (size_t)g->nz * mc::DQ_MAXQ * sizeof(double), 256);
+    L.plane_ext = o;  o = align_up(o + (size_t)g->nz * 3 * sizeof(double), 256);
     L.diag_out = o;   o = align_up(o + (19 + 3 * (size_t)g->nz) * sizeof(double), 256);
     L.total = o;
     return L;
@@ -400,6 +401,7 @@ int mc_tvd_init(const mc_tvd_grid *grid, const mc_tvd_params *params, double *d_
     s->partial = (double *)(w + L.partial);
     s->ext = (double *)(w + L.ext);
     s->plane_sums = (double *)(w + L.plane_sums);
+    s->plane_ext = (double *)(w + L.plane_ext);
     s->diag_out = (double *)(w + L.diag_out);
     s->diag_blocks = L.diag_blocks;
     s->stream = (cudaStream_t)cuda_stream;
@@ -502,8 +504,9 @@ int mc_tvd_diagnostics(mc_tvd_state *s, mc_tvd_diag *out, double *T_prof, double
     G.nplane = (double)s->grid.nx * (double)s->grid.ny;
     G.dz = s->d[2]; G.dxdy = s->d[0] * s->d[1];
     G.eps = s->par.eps; G.D = s->par.D; G.Ra = s->par.Ra; G.Pr = s->par.Pr;
-    { auto kfn = mc::k_diag_finish; MC_LAUNCH(kfn, 1, mc::DIAG_THREADS, 0, s->stream, G); }
-    s->launches += 2;
+    { auto kfn = mc::k_diag_planes; MC_LAUNCH(kfn, (unsigned)((s->grid.nz + 3) / 4), 128, 0, s->stream, G, s->plane_ext); }
+    { auto kfn = mc::k_diag_finish; MC_LAUNCH(kfn, 1, mc::DIAG_THREADS, 0, s->stream, G, s->plane_ext); }
+    s->launches += 3;
     int rc = cuda_check(cudaGetLastError(), "diagnostics launch");
     if (rc != MC_TVD_OK) return rc;
     const size_t nz = (size_t)s->grid.nz;

@@ -29,7 +29,7 @@ MC_DEV void node_primitives(const PointArgs &P, long long n, int k, double (&X)[
 {
 #pragma unroll
     for (int f = 0; f < ND + 2; ++f) X[f] = P.X[(long long)f * P.N + n];
-    double inv = 1.0 / X[0], ke = 0.0;
+    double inv = rcp(X[0]), ke = 0.0;
 #pragma unroll
     for (int c = 0; c < ND; ++c) { u[c] = X[1 + c] * inv; ke += u[c] * u[c]; }
     T = (X[ND + 1] * inv - 0.5 * ke - P.g * ((double)k * P.dz)) * P.icv;       // Eq. 17
@@ -90,74 +90,88 @@ constexpr int DQ_MAXQ = 11;            // 6 + nf (nf <= 5)
 constexpr int DIAG_THREADS = 256;
 
 // Per-plane partial sums: grid (blocks_per_plane, nz).  partial[(k*gridDim.x + b)*2*DQ_MAXQ + 2*q] = (s, c);
-// ext[(k*gridDim.x + b)*3] = (max Mach, min rho, min T).
+// ext[(k*gridDim.x + b)*3] = (max Mach^2, min rho, min T).
+// Only the sum of T is compensated (two-sum): its plane means enter Nu through a one-sided difference divided
+// by eps dz (Eq. 23), which amplifies their rounding error by ~1/(eps dz) (4e4 on C3).  The other sums are
+// plain: a thread adds <= a few hundred terms and the rest is a tree, far inside their 1e-12 / 1e-13 tolerances;
+// their `c` slots are written as 0.  The pass is then HBM-bound instead of fp64-bound.
 template <int ND>
 MC_KERNEL void k_plane_partials(PointArgs P, double *partial, double *ext)
 {
     constexpr int NF = ND + 2, NQ = 6 + NF;
     const int k = blockIdx.y;
     const double TA = 1.0 - P.D * ((double)k * P.dz);          // adiabatic profile, Eq. 19
-    Acc acc[NQ];
+    const double gz = P.g * ((double)k * P.dz);
+    const double igR = 1.0 / (P.gamma * P.R);
+    Acc accT; accT.s = 0.0; accT.c = 0.0;
+    double acc[NQ];
 #pragma unroll
-    for (int q = 0; q < NQ; ++q) { acc[q].s = 0.0; acc[q].c = 0.0; }
-    double mach = 0.0, rmin = INFINITY, tmin = INFINITY;
+    for (int q = 0; q < NQ; ++q) acc[q] = 0.0;
+    double mach2 = 0.0, rmin = INFINITY, tmin = INFINITY;
+    const double *base = P.X + (long long)k * P.plane;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < P.plane;
          i += (long long)gridDim.x * blockDim.x) {
-        long long n = (long long)k * P.plane + i;
-        double X[NF], u[ND], T;
-        node_primitives<ND>(P, n, k, X, u, T);
+        double X[NF], u[ND];
+#pragma unroll
+        for (int f = 0; f < NF; ++f) X[f] = base[(long long)f * P.N + i];
+        const double rho = X[0], inv = rcp(rho);
         double u2 = 0.0;
 #pragma unroll
-        for (int c = 0; c < ND; ++c) u2 += u[c] * u[c];
-        double uz = u[ND - 1], rho = X[0];
-        acc[DQ_T].add(T);
-        acc[DQ_RHO].add(rho);
-        acc[DQ_P].add(P.R * rho * T);
-        acc[DQ_CONV].add(rho * uz * (T - TA));                  // rho u_z T_sa, Eq. 22
-        acc[DQ_K].add(rho * uz * u2);                           // rho u_z u^2, Eq. 22
-        acc[DQ_U2].add(u2);                                     // Eq. 26
+        for (int c = 0; c < ND; ++c) { u[c] = X[1 + c] * inv; u2 = fma(u[c], u[c], u2); }
+        const double T = (X[NF - 1] * inv - 0.5 * u2 - gz) * P.icv;          // Eq. 17
+        const double muz = X[NF - 2];                                        // rho u_z
+        accT.add(T);
+        acc[DQ_RHO] += rho;
+        acc[DQ_P] += P.R * rho * T;
+        acc[DQ_CONV] += muz * (T - TA);                                      // rho u_z T_sa, Eq. 22
+        acc[DQ_K] += muz * u2;                                               // rho u_z u^2, Eq. 22
+        acc[DQ_U2] += u2;                                                    // Eq. 26
 #pragma unroll
-        for (int f = 0; f < NF; ++f) acc[DQ_X0 + f].add(X[f]);
-        mach = fmax(mach, sqrt(u2) / sqrt(P.gamma * P.R * T));
+        for (int f = 0; f < NF; ++f) acc[DQ_X0 + f] += X[f];
+        mach2 = fmax(mach2, (u2 * igR) * rcp(T));                            // Mach^2 = u^2 / (gamma R T)
         rmin = fmin(rmin, rho);
         tmin = fmin(tmin, T);
     }
     // warp stage
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
+        const double s2 = __shfl_xor_sync(0xffffffffu, accT.s, o);
+        const double c2 = __shfl_xor_sync(0xffffffffu, accT.c, o);
+        accT.merge(s2, c2);
 #pragma unroll
-        for (int q = 0; q < NQ; ++q) {
-            double s2 = __shfl_xor_sync(0xffffffffu, acc[q].s, o);
-            double c2 = __shfl_xor_sync(0xffffffffu, acc[q].c, o);
-            acc[q].merge(s2, c2);
-        }
-        mach = fmax(mach, __shfl_xor_sync(0xffffffffu, mach, o));
+        for (int q = 1; q < NQ; ++q) acc[q] += __shfl_xor_sync(0xffffffffu, acc[q], o);
+        mach2 = fmax(mach2, __shfl_xor_sync(0xffffffffu, mach2, o));
         rmin = fmin(rmin, __shfl_xor_sync(0xffffffffu, rmin, o));
         tmin = fmin(tmin, __shfl_xor_sync(0xffffffffu, tmin, o));
     }
     // block stage
-    __shared__ double sh[DIAG_THREADS / 32][2 * DQ_MAXQ + 3];
+    __shared__ double sh[DIAG_THREADS / 32][DQ_MAXQ + 4];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarp = blockDim.x >> 5;
     if (lane == 0) {
+        sh[warp][0] = accT.s; sh[warp][DQ_MAXQ] = accT.c;
 #pragma unroll
-        for (int q = 0; q < NQ; ++q) { sh[warp][2 * q] = acc[q].s; sh[warp][2 * q + 1] = acc[q].c; }
-        sh[warp][2 * DQ_MAXQ] = mach; sh[warp][2 * DQ_MAXQ + 1] = rmin; sh[warp][2 * DQ_MAXQ + 2] = tmin;
+        for (int q = 1; q < NQ; ++q) sh[warp][q] = acc[q];
+        sh[warp][DQ_MAXQ + 1] = mach2; sh[warp][DQ_MAXQ + 2] = rmin; sh[warp][DQ_MAXQ + 3] = tmin;
     }
     __syncthreads();
     if (threadIdx.x == 0) {
         const long long slot = (long long)k * gridDim.x + blockIdx.x;
-        for (int q = 0; q < NQ; ++q) {
-            Acc a; a.s = 0.0; a.c = 0.0;
-            for (int w = 0; w < nwarp; ++w) a.merge(sh[w][2 * q], sh[w][2 * q + 1]);
-            partial[slot * 2 * DQ_MAXQ + 2 * q] = a.s;
-            partial[slot * 2 * DQ_MAXQ + 2 * q + 1] = a.c;
+        Acc a; a.s = 0.0; a.c = 0.0;
+        for (int w = 0; w < nwarp; ++w) a.merge(sh[w][0], sh[w][DQ_MAXQ]);
+        partial[slot * 2 * DQ_MAXQ] = a.s;
+        partial[slot * 2 * DQ_MAXQ + 1] = a.c;
+        for (int q = 1; q < NQ; ++q) {
+            double t = 0.0;
+            for (int w = 0; w < nwarp; ++w) t += sh[w][q];
+            partial[slot * 2 * DQ_MAXQ + 2 * q] = t;
+            partial[slot * 2 * DQ_MAXQ + 2 * q + 1] = 0.0;
         }
         for (int w = 1; w < nwarp; ++w) {
-            mach = fmax(mach, sh[w][2 * DQ_MAXQ]);
-            rmin = fmin(rmin, sh[w][2 * DQ_MAXQ + 1]);
-            tmin = fmin(tmin, sh[w][2 * DQ_MAXQ + 2]);
+            mach2 = fmax(mach2, sh[w][DQ_MAXQ + 1]);
+            rmin = fmin(rmin, sh[w][DQ_MAXQ + 2]);
+            tmin = fmin(tmin, sh[w][DQ_MAXQ + 3]);
         }
-        ext[slot * 3] = mach; ext[slot * 3 + 1] = rmin; ext[slot * 3 + 2] = tmin;
+        ext[slot * 3] = mach2; ext[slot * 3 + 1] = rmin; ext[slot * 3 + 2] = tmin;
     }
 }
 
@@ -170,44 +184,72 @@ struct DiagArgs {
     double nplane, dz, dxdy, eps, D, Ra, Pr;
 };
 
-// Plane sums -> means, trapezoid rule in z (R16), one-sided plate gradients, Eqs. 22-26.
-MC_KERNEL void k_diag_finish(DiagArgs G)
+// Stage 2: the partial sums of one z plane -> plane_sums[k][q] (one warp per plane, lane q walks the plane's
+// blocks in order) and the plane's extrema -> plane_ext[k][3].
+MC_KERNEL void k_diag_planes(DiagArgs G, double *plane_ext)
 {
-    __shared__ double sh_ext[3][DIAG_THREADS];
-    double mach = 0.0, rmin = INFINITY, tmin = INFINITY;
-    for (int k = threadIdx.x; k < G.nz; k += blockDim.x) {
-        for (int q = 0; q < G.nq; ++q) {
-            Acc a; a.s = 0.0; a.c = 0.0;
-            for (int b = 0; b < G.nblk; ++b) {
-                const double *p = G.partial + ((long long)k * G.nblk + b) * 2 * DQ_MAXQ + 2 * q;
-                a.merge(p[0], p[1]);
-            }
-            G.plane_sums[(long long)k * DQ_MAXQ + q] = a.s + a.c;
-        }
+    const int k = (int)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+    if (k >= G.nz) return;
+    if (lane < G.nq) {
+        Acc a; a.s = 0.0; a.c = 0.0;
         for (int b = 0; b < G.nblk; ++b) {
-            const double *e = G.ext + ((long long)k * G.nblk + b) * 3;
-            mach = fmax(mach, e[0]); rmin = fmin(rmin, e[1]); tmin = fmin(tmin, e[2]);
+            const double *p = G.partial + ((long long)k * G.nblk + b) * 2 * DQ_MAXQ + 2 * lane;
+            a.merge(p[0], p[1]);
         }
+        G.plane_sums[(long long)k * DQ_MAXQ + lane] = a.s + a.c;
+    } else if (lane < G.nq + 3) {
+        const int e = lane - G.nq;                       // 0: max Mach^2, 1: min rho, 2: min T
+        double v = (e == 0) ? 0.0 : INFINITY;
+        for (int b = 0; b < G.nblk; ++b) {
+            const double x = G.ext[((long long)k * G.nblk + b) * 3 + e];
+            v = (e == 0) ? fmax(v, x) : fmin(v, x);
+        }
+        plane_ext[(long long)k * 3 + e] = v;
     }
-    sh_ext[0][threadIdx.x] = mach; sh_ext[1][threadIdx.x] = rmin; sh_ext[2][threadIdx.x] = tmin;
-    __syncthreads();
-    if (threadIdx.x != 0) return;
-    for (int t = 1; t < (int)blockDim.x; ++t) {
-        mach = fmax(mach, sh_ext[0][t]); rmin = fmin(rmin, sh_ext[1][t]); tmin = fmin(tmin, sh_ext[2][t]);
-    }
+}
+
+// Stage 3: plane sums -> means, trapezoid rule in z (R16), one-sided plate gradients,
+// Eqs. 22-26.  One block; the z sums are a strided per-thread sum followed by a shared-memory tree.
+MC_KERNEL void k_diag_finish(DiagArgs G, const double *plane_ext)
+{
+    constexpr int NV = 9;                                // vol_w, conv, K, u2, totals[5]
+    __shared__ double sh[NV + 3][DIAG_THREADS];
     const int nz = G.nz, nf = G.nq - 6;
     double *Tp = G.out + 19, *rp = Tp + nz, *pp = rp + nz;
-    double vol_w = 0.0, v_conv = 0.0, v_K = 0.0, v_u2 = 0.0, tot[5] = {0, 0, 0, 0, 0};
-    for (int k = 0; k < nz; ++k) {
+    double v[NV], mach2 = 0.0, rmin = INFINITY, tmin = INFINITY;
+#pragma unroll
+    for (int i = 0; i < NV; ++i) v[i] = 0.0;
+    for (int k = threadIdx.x; k < nz; k += blockDim.x) {
         const double *ps = G.plane_sums + (long long)k * DQ_MAXQ;
-        double wk = G.dz * ((G.walls && (k == 0 || k == nz - 1)) ? 0.5 : 1.0);
+        const double wk = G.dz * ((G.walls && (k == 0 || k == nz - 1)) ? 0.5 : 1.0);
         Tp[k] = ps[DQ_T] / G.nplane; rp[k] = ps[DQ_RHO] / G.nplane; pp[k] = ps[DQ_P] / G.nplane;
-        vol_w += wk;
-        v_conv += wk * (ps[DQ_CONV] / G.nplane);
-        v_K += wk * (ps[DQ_K] / G.nplane);
-        v_u2 += wk * (ps[DQ_U2] / G.nplane);
-        for (int f = 0; f < nf; ++f) tot[f] += wk * G.dxdy * ps[DQ_X0 + f];
+        v[0] += wk;
+        v[1] += wk * (ps[DQ_CONV] / G.nplane);
+        v[2] += wk * (ps[DQ_K] / G.nplane);
+        v[3] += wk * (ps[DQ_U2] / G.nplane);
+        for (int f = 0; f < nf; ++f) v[4 + f] += wk * G.dxdy * ps[DQ_X0 + f];
+        mach2 = fmax(mach2, plane_ext[(long long)k * 3]);
+        rmin = fmin(rmin, plane_ext[(long long)k * 3 + 1]);
+        tmin = fmin(tmin, plane_ext[(long long)k * 3 + 2]);
     }
+#pragma unroll
+    for (int i = 0; i < NV; ++i) sh[i][threadIdx.x] = v[i];
+    sh[NV][threadIdx.x] = mach2; sh[NV + 1][threadIdx.x] = rmin; sh[NV + 2][threadIdx.x] = tmin;
+    __syncthreads();
+    for (int o = blockDim.x >> 1; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) {
+#pragma unroll
+            for (int i = 0; i < NV; ++i) sh[i][threadIdx.x] += sh[i][threadIdx.x + o];
+            sh[NV][threadIdx.x] = fmax(sh[NV][threadIdx.x], sh[NV][threadIdx.x + o]);
+            sh[NV + 1][threadIdx.x] = fmin(sh[NV + 1][threadIdx.x], sh[NV + 1][threadIdx.x + o]);
+            sh[NV + 2][threadIdx.x] = fmin(sh[NV + 2][threadIdx.x], sh[NV + 2][threadIdx.x + o]);
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x != 0) return;
+    const double vol_w = sh[0][0], v_conv = sh[1][0], v_K = sh[2][0], v_u2 = sh[3][0];
+    double tot[5];
+    for (int f = 0; f < 5; ++f) tot[f] = sh[4 + f][0];
     double *o = G.out;
     const double sRaPr = sqrt(G.Ra * G.Pr);
     o[0] = G.S->time; o[1] = G.S->dt; o[2] = __longlong_as_double(G.S->step);
@@ -215,6 +257,7 @@ MC_KERNEL void k_diag_finish(DiagArgs G)
     double nu_K = G.D * sRaPr / 2.0 * (v_K / vol_w);
     double nu0 = 0.0, nu1 = 0.0;
     if (nz >= 3) {                                                     // Eq. 23 with PAPER.md:309
+        // (Tp[0..2] and Tp[nz-3..nz-1] were written by other threads of this block before the barriers above)
         auto tsa = [&](int k) { return Tp[k] - (1.0 - G.D * ((double)k * G.dz)); };
         double g0 = (-3.0 * tsa(0) + 4.0 * tsa(1) - tsa(2)) / (2.0 * G.dz);
         double g1 = (3.0 * tsa(nz - 1) - 4.0 * tsa(nz - 2) + tsa(nz - 3)) / (2.0 * G.dz);
@@ -227,7 +270,7 @@ MC_KERNEL void k_diag_finish(DiagArgs G)
     o[11] = tot[0]; o[12] = tot[1];
     o[13] = (nf == 5) ? tot[2] : 0.0;
     o[14] = tot[nf - 2]; o[15] = tot[nf - 1];
-    o[16] = mach; o[17] = rmin; o[18] = tmin;
+    o[16] = sqrt(sh[NV][0]); o[17] = sh[NV + 1][0]; o[18] = sh[NV + 2][0];   // the partials carry Mach^2
 }
 
 }  // namespace mc
