@@ -14,6 +14,7 @@
 #include "mc_common.cuh"
 #include "reduce_kernels.cuh"
 #include "sweep_lane.cuh"
+#include "sweep_lane2.cuh"
 #include "sweep_lane3.cuh"
 #include "sweep_march.cuh"
 #include "sweep_march3.cuh"
@@ -45,6 +46,15 @@ size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 #endif
 #ifndef MC_LANE3_WB
 #define MC_LANE3_WB 12
+#endif
+#ifndef MC_LANE2_WARPS
+#define MC_LANE2_WARPS 4
+#endif
+#ifndef MC_LANE2_MINB
+#define MC_LANE2_MINB 2
+#endif
+#ifndef MC_LANE2
+#define MC_LANE2 1
 #endif
 #ifndef MC_LANE_WARPS_2D
 #define MC_LANE_WARPS_2D 4
@@ -266,6 +276,18 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
             with_walls(wl, [&](auto W) { with_tvd(s, [&](auto T) {
                 launch_kernel(mc::k_march<2, 1, -1, WX, 1, decltype(W)::value, false, decltype(T)::value, MARCH_MINB_2D>, grid, block, smem, st, A);
             }); });
+        } else if (alpha == 0 && MC_LANE2 && nx % 2 == 0) {   // x-sweep, even nx: two nodes per lane, march z
+            constexpr int LW = MC_LANE2_WARPS;
+            A.n_b = 1; A.s_b = 0; A.n_m = nz; A.s_m = nx;
+            long long xt = (nx + mc::LANE2_OUT - 1) / mc::LANE2_OUT;
+            long long tiles = (xt + LW - 1) / LW;
+            A.chunk = pick_chunk(s, nz, tiles, MC_LANE2_MINB);
+            dim3 block(32, LW, 1), grid((unsigned)tiles, 1, (unsigned)((nz + A.chunk - 1) / A.chunk));
+            with_walls(wl, [&](auto W) { with_tvd(s, [&](auto T) { with_bool(reduce, [&](auto Rd) {
+                with_bool(dir > 0, [&](auto Fw) {
+                    launch_kernel(mc::k_lane2<LW, decltype(W)::value, decltype(T)::value, decltype(Rd)::value, MC_LANE2_MINB, decltype(Fw)::value>, grid, block, 0, st, A);
+                });
+            }); }); });
         } else if (alpha == 0) {     // x-sweep: lanes x, march z
             constexpr int LW = LANE_WARPS_2D;
             A.n_b = 1; A.s_b = 0; A.n_m = nz; A.s_m = nx;
