@@ -40,9 +40,10 @@ def test_single_rank_passthrough():
     import bench
     assert bench.max_over_ranks(3.5, 1, "cpu") == 3.5
     assert bench.job_value(1, 100, 2, 10.0) == pytest.approx(100 * 2 / 10.0e-3)
-    names3, names2 = bench.kernel_names(3), bench.kernel_names(2)
+    names3, names2, names2odd = bench.kernel_names(3, 1024), bench.kernel_names(2, 16384), bench.kernel_names(2, 29)
     assert names3["Lz+"].startswith("k_march3") and names3["Lx-"].startswith("k_lane3")
-    assert names2["Lz+"].startswith("k_march ") and names2["Lx-"].startswith("k_lane ")
+    assert names2["Lz+"].startswith("k_march ") and names2["Lx-"].startswith("k_lane2 ")
+    assert names2odd["Lx+"].startswith("k_lane ")
 
 
 def test_reference_arm_prints_one_json_line():
