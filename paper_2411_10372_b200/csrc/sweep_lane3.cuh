@@ -27,7 +27,7 @@ namespace mc {
 // direction m (z); WB: warps (rows) per block; WALL_M: m is z with plates; TVD: -1 / 0 / 1 as in
 // k_march; REDUCE: fold the CFL max-reduction of the output into the epilogue (R12).  alpha is x.
 template <int CB, int CM, int WB, bool WALL_M, int TVD, bool REDUCE>
-MC_KERNEL void __maxnreg__((65536 / (32 * WB)) / 8 * 8) k_lane3(SweepArgs A)
+MC_KERNEL void __maxnreg__(((65536 / (32 * WB)) / 8 * 8) > 248 ? 248 : ((65536 / (32 * WB)) / 8 * 8)) k_lane3(SweepArgs A)
 {
     constexpr int ND = 3, NF = 5;
     constexpr bool HAS_B = true;

@@ -34,7 +34,7 @@ namespace mc {
 #define MC_MARCH3_L2PF 4
 #endif
 #ifndef MC_MARCH3_REGS
-#define MC_MARCH3_REGS ((65536 / (32 * WB * MINB)) / 8 * 8)
+#define MC_MARCH3_REGS (((65536 / (32 * WB * MINB)) / 8 * 8) > 248 ? 248 : ((65536 / (32 * WB * MINB)) / 8 * 8))
 #endif
 template <int CA, int CB, int WB, bool WALL_M, bool WALL_B, int TVD, int MINB = 1>
 MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
