@@ -34,7 +34,8 @@ def _solver(gpu, grid, params, X0):
 
 # ---- one operator L_alpha(tau) (Eqs. 31-39), every axis, both directions, both z boundaries ------
 SWEEP_GRIDS = [
-    (2, 300, 1, 70),      # 2-D: 3 march tiles (124 outputs) / 11 lane warps (28 outputs), ragged tails
+    (2, 300, 1, 70),      # 2-D, even nx: 3 march tiles (124 outputs) / 5 two-node lane warps (60 outputs), ragged tails
+    (2, 301, 1, 40),      # 2-D, odd nx: the one-node-per-lane x-sweep (11 lane warps of 28 outputs)
     (2, 29, 1, 5),        # smallest plate problem, one ragged tile
     (3, 60, 21, 19),      # 3-D: 3 x-tiles, 3 b-tiles (8 outputs) with ragged tails, walls in b for Ly
     (3, 30, 9, 33),       # ragged the other way
