@@ -281,7 +281,7 @@ MC_KERNEL void __launch_bounds__(32 * WARPS, MINB) k_lane2(SweepArgs A)
     // ---- the march -------------------------------------------------------------------------------
     std::integral_constant<bool, false> slow;
     std::integral_constant<bool, true> fast;
-    int j = l0 - 4;
+    int j = (WALL_M && l0 == 0) ? -2 : l0 - 4;      // below a plate there is nothing to warm up
     if (exists(j + 2)) load_at(off_of(j + 2), Xn);
     // fast levels: every level j-1 .. j+3 exists, none is a plate, none wraps around
     const int jf0 = max(l0, 1);

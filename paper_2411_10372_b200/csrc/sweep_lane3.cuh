@@ -271,7 +271,7 @@ MC_KERNEL void __maxnreg__(((65536 / (32 * WB)) / 8 * 8) > 248 ? 248 : ((65536 /
         integral_constant<bool, false> slow;
         integral_constant<bool, true> fast;
         integral_constant<int, -1> par_any;
-        int j = l0 - 4;
+        int j = (WALL_M && l0 == 0) ? -2 : l0 - 4;      // below a plate there is nothing to warm up
         if (exists(j + 2)) {
             load(j + 2, Xn);
             if (decltype(role_tag)::value == LROLE_R1) load_outer(j + 2, Xon);

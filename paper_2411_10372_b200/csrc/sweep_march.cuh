@@ -344,7 +344,7 @@ MC_KERNEL void __launch_bounds__(WX * WB, MINB) k_march(SweepArgs A)
         integral_constant<bool, false> slow;
         integral_constant<bool, true> fast;
         integral_constant<int, -1> par_any;
-        int j = l0 - 4;
+        int j = (WALL_M && l0 == 0) ? -2 : l0 - 4;      // below a plate there is nothing to warm up
         if (exists(j + 2)) load(j + 2, Xn);
         // fast levels: every level j-1 .. j+3 exists, none is a plate, none wraps around
         const int jf0 = max(l0, 1);

@@ -377,7 +377,7 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
         integral_constant<bool, false> slow;
         integral_constant<bool, true> fast;
         integral_constant<int, -1> par_any;
-        int j = l0 - 4;
+        int j = (WALL_M && l0 == 0) ? -2 : l0 - 4;      // below a plate there is nothing to warm up
         if (exists(j + 2)) {
             load(j + 2, Xn);
             if (ROLE == ROLE_R1 && has_outer) load_outer(off_of(j + 2) - off_base + off_base_o, Xon);
