@@ -100,3 +100,18 @@ def test_no_cpu_fallback_without_cuda():
     params = inputs.make_params()
     with pytest.raises(RuntimeError, match="no CPU fallback"):
         binding.MCTVD(grid, params, inputs.conduction_state(grid, params))
+
+
+def test_build_refuses_kernels_with_a_large_stack_frame():
+    """A sweep kernel whose lambdas were not all inlined keeps its register pipeline in local memory (6x slower,
+    seen once).  build.py parses ptxas -v and refuses such a build; the committed build's log must be clean."""
+    from paper_2411_10372_b200 import build
+    bad = ("ptxas info    : Compiling entry function '_ZN2mc8k_march3ILi2EEEvNS_9SweepArgsE' for 'sm_100a'\n"
+           "    1472 bytes stack frame, 0 bytes spill stores, 0 bytes spill loads\n")
+    with pytest.raises(RuntimeError, match="1472-byte stack frame"):
+        build._check_stack_frames(bad)
+    ok = bad.replace("1472 bytes", "40 bytes")
+    build._check_stack_frames(ok)
+    log = os.path.join(os.path.dirname(build.LIB_PATH), "build.log")
+    if os.path.exists(log):
+        build._check_stack_frames(open(log).read())
