@@ -162,8 +162,7 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
     double Xc[NF];                 // X(j+1)
     double Xon[ND + 1];            // rho, m of the outer (ring-2) row at the level W works on next (ring-1 rows only)
     double F0[NF];                 // F(j)
-    double H0[NF];                 // (X^P + X)/2 + tau S^P/2 - Dh_{j-1/2} + (tau/2dx) F^P(j) of level j (fast levels;
-    double FP0m = 0.0;             //  F^P(j) mass flux, kept apart for the plate closure, R10)
+    double H0[NF];                 // (X^P + X)/2 + tau S^P/2 - Dh_{j-1/2} + (tau/2dx) F^P(j) of level j
     double d0[NF];                 // dX_{j+1/2}
     double uP0[ND], TP0 = 1.0;     // u, T of X^P(j)
     double a0 = 0.0, b0 = 0.0;     // (dX_{j-1/2}, dX_{j+1/2}), |dX_{j+1/2}|^2
@@ -344,16 +343,15 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
             if (FAST || (j >= l0 && exists(j))) {
                 double o[NF];
                 if (!FAST && WALL_M && j == 0) {
-                    plate(j, H0[0] - hcdt * FP0m - cdt * (FP1[0] - FP0m), o); // 0.5 * (2 tau/dz) * dF
+                    plate(j, H0[0] - cdt * FP1[0], o);    // 0.5 (2 tau/dz) (F^P(1) - F^P(0)); the plate's own mass flux is 0
                 } else if (!FAST && WALL_M && j == n - 1) {
-                    plate(j, H0[0] - hcdt * FP0m, o);
+                    plate(j, H0[0], o);
                 } else {
 #pragma unroll
                     for (int f = 0; f < NF; ++f) o[f] = fma(-hcdt, FP1[f], H0[f]);
                 }
                 if (owner) store_at(o0, o);
             }
-            FP0m = FP1[0];
 #pragma unroll
             for (int f = 0; f < NF; ++f) { H1[f] = fma(hcdt, FP1[f], H1[f]); d0[f] = d1[f]; }
             a0 = a1; b0 = b1; hC0 = hC1; hC1 = hC2;
