@@ -95,8 +95,14 @@ int mc_tvd_step(mc_tvd_state *s, int n_steps);
 
 /* One operator L_alpha(tau) (Eqs. 31-39) applied to d_fields in place (through the workspace):
  * alpha = 0,1,2 for x,y,z; dir = +1 backward predictor / forward corrector,
- * -1 the mirrored pair.  Exposed for per-operator parity tests; does not advance time or dt. */
+ * -1 the mirrored pair.  Exposed for per-operator parity tests.  Time and the step count do not advance;
+ * dt is recomputed from the swept state (as mc_tvd_init does), so a following mc_tvd_step is CFL-safe. */
 int mc_tvd_sweep(mc_tvd_state *s, int alpha, int dir, double tau);
+
+/* Test hook: marching levels per thread block of later operator launches (the kernels march along one
+ * axis and cut it into chunks, each repeating a short warm-up).  0 = automatic (default).
+ * Results do not depend on it; the parity tests use it to start blocks in the middle of a column. */
+int mc_tvd_debug_set_chunk(mc_tvd_state *s, int levels);
 
 /* The end-to-end call for callers whose state lives in HOST memory (pinned memory makes the copies
  * asynchronous, pageable memory works too): copies h_in (HOST, nf*N doubles, same layout) into

@@ -17,7 +17,11 @@
  * vs exact Riemann solution, 2nd-order convergence, mirror identity, viscous
  * shear-wave decay, thermal diffusion, viscous heating pattern, acoustic
  * attenuation, hydrostatic conduction state, closed-form diagnostics,
- * axis-permutation identities.  Unpinned readings are listed in DESIGN.md.
+ * axis-permutation identities, stationary contact (Eqs. 34-39 in closed form),
+ * one-operator Taylor expansion with gravity (S^P of Eq. 32), compact viscous
+ * stencil rate (R7), operator sequence of Eq. 30.  Parity unpinned: R11 only
+ * (TVD flux dropped on plate-adjacent interfaces; the paper is silent) -- see
+ * DESIGN.md.
  *
  * Field layout (all calls): nf = 4 (2-D: rho, rho*u_x, rho*u_z, E) or
  * nf = 5 (3-D: rho, rho*u_x, rho*u_y, rho*u_z, E) arrays of N = nx*ny*nz

@@ -47,6 +47,7 @@ SYMBOLS = {
                               C.c_void_p, C.POINTER(C.c_void_p)]),
     "mc_tvd_step": (C.c_int, [C.c_void_p, C.c_int]),
     "mc_tvd_sweep": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_double]),
+    "mc_tvd_debug_set_chunk": (C.c_int, [C.c_void_p, C.c_int]),
     "mc_tvd_step_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]),
     "mc_tvd_dt": (C.c_int, [C.c_void_p, _DP]),
     "mc_tvd_diagnostics": (C.c_int, [C.c_void_p, C.POINTER(Diag), _DP, _DP, _DP]),
@@ -86,8 +87,7 @@ def load_library(path: str | None = None) -> C.CDLL:
     if _lib is not None and path is None:
         return _lib
     if path is None:
-        if os.environ.get("MC_TVD_NO_BUILD") != "1":
-            build_library()
+        build_library()                  # no-op unless a source file changed since the last build
         path = LIB_PATH
     if not os.path.exists(path):
         raise ImportError(f"{path} is missing: run `python -m paper_2411_10372_b200.build` (needs nvcc)")
@@ -165,6 +165,9 @@ class MCTVD:
 
     def sweep(self, alpha: int, direction: int, tau: float):
         self._check(self.lib.mc_tvd_sweep(self._h, int(alpha), int(direction), float(tau)))
+
+    def debug_set_chunk(self, levels: int):
+        self._check(self.lib.mc_tvd_debug_set_chunk(self._h, int(levels)))
 
     def step_host(self, h_in, h_out, n_steps: int):
         """h_in / h_out: CPU float64 torch tensors (pinned for async copies) or numpy arrays."""

@@ -14,19 +14,34 @@ _PKG = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_PKG, "csrc")
 LIB_PATH = os.path.join(_PKG, "libmc_tvd.so")
 _SOURCES = ["mc_tvd.cu"]
-_DEPS = ["mc_tvd.cu", "mc_common.cuh", "sweep_march.cuh", "sweep_lane.cuh", "sweep_march3.cuh", "sweep_lane3.cuh",
-         "reduce_kernels.cuh",
-         os.path.join("..", "..", "include", "mc_tvd.h")]
+_HASH_PATH = LIB_PATH + ".srchash"
+
+
+def _deps() -> list[str]:
+    """Every file the library is compiled from: all of csrc/ plus the public header."""
+    files = sorted(os.path.join(_CSRC, f) for f in os.listdir(_CSRC) if f.endswith((".cu", ".cuh", ".h")))
+    return files + [os.path.join(_PKG, "..", "include", "mc_tvd.h")]
+
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "--shared", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 
 
+def _source_hash() -> str:
+    """Content hash of the sources and flags (mtimes do not survive the copy to the GPU box)."""
+    import hashlib
+    h = hashlib.sha256(" ".join(NVCC_FLAGS).encode())
+    for path in _deps():
+        with open(path, "rb") as f:
+            h.update(os.path.basename(path).encode() + b"\0" + f.read())
+    return h.hexdigest()
+
+
 def _stale() -> bool:
-    if not os.path.exists(LIB_PATH):
+    if not (os.path.exists(LIB_PATH) and os.path.exists(_HASH_PATH)):
         return True
-    t = os.path.getmtime(LIB_PATH)
-    return any(os.path.getmtime(os.path.join(_CSRC, d)) > t for d in _DEPS)
+    with open(_HASH_PATH) as f:
+        return f.read().strip() != _source_hash()
 
 
 MAX_STACK_BYTES = 256
@@ -62,6 +77,8 @@ def build_library(force: bool = False, verbose: bool = False) -> str:
         raise RuntimeError("nvcc failed building libmc_tvd.so")
     _check_stack_frames(log)
     os.replace(tmp, LIB_PATH)
+    with open(_HASH_PATH, "w") as f:
+        f.write(_source_hash() + "\n")
     if verbose:
         print(log)
     return LIB_PATH

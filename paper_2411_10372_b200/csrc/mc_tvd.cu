@@ -239,16 +239,9 @@ template <class F> void with_tvd(const mc_tvd_state *s, F f)
 
 template <class K> int launch_kernel(K kfn, dim3 grid, dim3 block, size_t smem, cudaStream_t st, const mc::SweepArgs &A)
 {
-    if (smem > 48 * 1024) {            // opt in to large dynamic shared memory, once per kernel
-        static K raised[64];
-        static int n_raised = 0;
-        bool seen = false;
-        for (int i = 0; i < n_raised; ++i) seen = seen || (raised[i] == kfn);
-        if (!seen) {
-            cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-            if (n_raised < 64) raised[n_raised++] = kfn;
-        }
-    }
+    // opt in to large dynamic shared memory: a per-function attribute, set before every such launch (no
+    // cache to guard: distinct handles may launch from different threads)
+    if (smem > 48 * 1024) cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     MC_LAUNCH(kfn, grid, block, smem, st, A);
     return 0;
 }
@@ -427,8 +420,7 @@ int mc_tvd_init(const mc_tvd_grid *grid, const mc_tvd_params *params, double *d_
     s->diag_out = (double *)(w + L.diag_out);
     s->diag_blocks = L.diag_blocks;
     s->stream = (cudaStream_t)cuda_stream;
-    const char *ce = getenv("MC_TVD_CHUNK");
-    s->chunk_override = ce ? atoi(ce) : 0;
+    s->chunk_override = 0;
     {
         int dev = 0, sms = 0;
         if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1)
@@ -450,6 +442,10 @@ int mc_tvd_init(const mc_tvd_grid *grid, const mc_tvd_params *params, double *d_
 int mc_tvd_step(mc_tvd_state *s, int n_steps)
 {
     if (!s || n_steps < 0) return fail(MC_TVD_EINVAL, "bad handle or n_steps");
+    {   // a kernel fault of earlier work on this stream is sticky: report it here without waiting
+        const cudaError_t q = cudaStreamQuery(s->stream);
+        if (q != cudaSuccess && q != cudaErrorNotReady) return cuda_check(q, "earlier work on the stream failed");
+    }
     for (int it = 0; it < n_steps; ++it) {
         const double *src = s->X;
         double *dst = s->Y;
@@ -477,9 +473,19 @@ int mc_tvd_sweep(mc_tvd_state *s, int alpha, int dir, double tau)
     if (!s || alpha < 0 || alpha > 2 || (dir != 1 && dir != -1) || !(tau > 0))
         return fail(MC_TVD_EINVAL, "bad handle, alpha, dir or tau");
     int rc = launch_sweep(s, s->X, s->Y, alpha, dir, tau, false, false);
+    s->ev_open = false;                // the copy below separates this launch from the next one
     if (rc != MC_TVD_OK) return rc;
-    return cuda_check(cudaMemcpyAsync(s->X, s->Y, (size_t)s->nf * s->N * sizeof(double), cudaMemcpyDeviceToDevice,
-                                      s->stream), "sweep copy-back");
+    rc = cuda_check(cudaMemcpyAsync(s->X, s->Y, (size_t)s->nf * s->N * sizeof(double), cudaMemcpyDeviceToDevice,
+                                    s->stream), "sweep copy-back");
+    if (rc != MC_TVD_OK) return rc;
+    return enqueue_initial_dt(s);      // dt now belongs to the swept state (time and step count unchanged)
+}
+
+int mc_tvd_debug_set_chunk(mc_tvd_state *s, int levels)
+{
+    if (!s || levels < 0) return fail(MC_TVD_EINVAL, "bad handle or levels");
+    s->chunk_override = levels;
+    return MC_TVD_OK;
 }
 
 int mc_tvd_step_host(mc_tvd_state *s, const double *h_in, double *h_out, int n_steps)

@@ -74,6 +74,7 @@ def test_init_rejects_bad_arguments_before_touching_the_device(lib):
     g.z_nodes = C.cast(z, C.POINTER(C.c_double))
     assert lib.mc_tvd_init(C.byref(g), C.byref(p), None, None, 0, None, C.byref(h)) == -5      # tanh grid: unsupported
     assert lib.mc_tvd_step(None, 1) == -1
+    assert lib.mc_tvd_debug_set_chunk(None, 4) == -1
     assert lib.mc_tvd_sweep(None, 0, 1, 0.1) == -1
     assert lib.mc_tvd_dt(None, None) == -1
     assert lib.mc_tvd_diagnostics(None, None, None, None, None) == -1
@@ -115,3 +116,15 @@ def test_build_refuses_kernels_with_a_large_stack_frame():
     log = os.path.join(os.path.dirname(build.LIB_PATH), "build.log")
     if os.path.exists(log):
         build._check_stack_frames(open(log).read())
+
+
+def test_every_kernel_source_is_a_build_dependency():
+    """An edit to any file under csrc/ (or to the public header) must make load_library() rebuild the .so:
+    the staleness check hashes the contents of exactly these files."""
+    from paper_2411_10372_b200 import build
+    deps = {os.path.basename(d) for d in build._deps()}
+    csrc = os.path.join(ROOT, "paper_2411_10372_b200", "csrc")
+    for f in os.listdir(csrc):
+        assert f in deps, f
+    assert "mc_tvd.h" in deps
+    assert not build._stale()                                    # load_library() above built it from these sources

@@ -65,9 +65,8 @@ def test_sweep_parity(gpu, orc, ndim, nx, ny, nz, bc_z, tvd_form):
 
 @pytest.mark.parametrize("ndim,nx,ny,nz", [(2, 300, 1, 70), (3, 60, 21, 19)])
 @pytest.mark.parametrize("chunk", [7, 16])
-def test_sweep_parity_chunked(gpu, orc, monkeypatch, ndim, nx, ny, nz, chunk):
+def test_sweep_parity_chunked(gpu, orc, ndim, nx, ny, nz, chunk):
     """Blocks that start in the middle of the marching direction (4-level warm-up)."""
-    monkeypatch.setenv("MC_TVD_CHUNK", str(chunk))
     grid = inputs.make_grid(ndim, nx, nz, ny)
     params = inputs.make_params(Ra=1e4)
     X0 = inputs.smooth_random_state(grid, params, seed=5)
@@ -77,6 +76,7 @@ def test_sweep_parity_chunked(gpu, orc, monkeypatch, ndim, nx, ny, nz, chunk):
         for direction in (1, -1):
             ref = orc.sweep(prob, X0, alpha, tau, direction)
             s = _solver(gpu, grid, params, X0)
+            s.debug_set_chunk(chunk)
             s.sweep(alpha, direction, tau)
             err = rel_err(s.state(), ref).max()
             s.close()
@@ -189,18 +189,17 @@ def test_3d_steps(gpu, orc):
 
 
 @pytest.mark.parametrize("ndim,nx,ny,nz,chunk", [(2, 300, 1, 70, 0), (2, 300, 1, 70, 9), (3, 60, 21, 19, 0), (3, 60, 21, 19, 5)])
-def test_cfl_reduction_is_exact_every_step(gpu, orc, monkeypatch, ndim, nx, ny, nz, chunk):
+def test_cfl_reduction_is_exact_every_step(gpu, orc, ndim, nx, ny, nz, chunk):
     """The CFL max-reduction is folded into the last operator behind a division-free filter that skips
     nodes which cannot raise the maximum already recorded (csrc/mc_common.cuh cfl_can_skip).  It must stay
     EXACT: after every step dt equals the oracle's dt of the same (downloaded) state to an ulp or two, on a
     state whose fastest node is in the interior and moves, with several marching chunks per column."""
-    if chunk:
-        monkeypatch.setenv("MC_TVD_CHUNK", str(chunk))
     grid = inputs.make_grid(ndim, nx, nz, ny)
     params = inputs.make_params(Ra=1e4)
     X0 = inputs.smooth_random_state(grid, params, seed=23)
     prob = orc.Problem(grid, params)
     s = _solver(gpu, grid, params, X0)
+    s.debug_set_chunk(chunk)
     assert abs(s.dt() - orc.dt(prob, X0)) <= 4e-16 * s.dt()
     for _ in range(6):
         s.step(1)

@@ -149,7 +149,7 @@ def test_tvd_form_decision(orc):
 
 
 # ----------------------------------------------------------------------------- check 4: convergence
-def _density_wave_error(orc, n, ndim, oblique, tvd_off, t_end=0.4, corrector_literal=False):
+def _density_wave_error(orc, n, ndim, oblique, tvd_off, t_end=0.4):
     gam = 1.4
     ny = n if (ndim == 3) else 1
     nz = n if oblique else 4
@@ -331,6 +331,196 @@ def test_viscous_heating_pattern_pins_work_term(orc):
     c2 = 2 * np.mean(dT * np.cos(2 * k * z + 0 * dT))
     want = nu * A**2 * k**2 * t_end / 2.0                                   # rho = c_v = 1
     assert 0.7 * want < c2 < 1.1 * want, (c2, want)
+
+
+# ----------------------------------------------------------------------------- TVD coefficient (Eqs. 34-39)
+@pytest.mark.parametrize("tvd_form", [0, 1])
+@pytest.mark.parametrize("axis", [0, 2])
+def test_stationary_contact_pins_tvd_coefficient(orc, tvd_form, axis):
+    """A contact at rest: u = 0, uniform p, one isolated density jump (mu = K = g = 0).  The flux F_alpha is
+    then uniform, so every MacCormack difference of Eqs. 31-32 is exactly zero and one operator returns X + T
+    (Eq. 33).  At an isolated jump dX_{k+1/2} = (drho, 0, 0, 0) with zero neighbours, so r+_k = r-_{k+1} = 0
+    (Eq. 37), phi = 0 and Eq. 34 moves exactly
+        +-[G_k + G_{k+1}] drho = +-(1/2)[C(Co_k) + C(Co_{k+1})] drho        (Davis/Yee sum, tvd_form 1)
+        +-(1/2) mean(C_k, C_{k+1}) drho                                     (Eq. 34 as printed, tvd_form 0, R6)
+    of density across the jump and nothing anywhere else, with Co = c_s tau/dx (R5: u = 0 here) and
+    C = Co (1 - Co) for Co <= 0.5, else 0.25 (Eq. 39).  tau is chosen on both branches of
+    Eq. 39 and straddling them.  Pins the 1/2 of Eq. 38, Eq. 39, and R5's tau and c_s."""
+    gam, p0, rl, rr = 1.4, 1.0, 1.0, 0.25
+    n, h = 16, 0.1
+    cl, cr = np.sqrt(gam * p0 / rl), np.sqrt(gam * p0 / rr)          # c_s = sqrt(gamma p / rho) on either side
+    C = lambda Co: Co * (1.0 - Co) if Co <= 0.5 else 0.25            # Eq. 39
+    for tau in (0.01, 0.03, 0.06):                                   # Co = (0.12, 0.24), (0.35, 0.71), (0.71, 1.42)
+        if axis == 0:
+            g = periodic_grid(2, n, 6, lx=n * h, lz=0.6)
+            shape = (1, 1, n)
+        else:
+            g = periodic_grid(2, 6, n, lx=0.6, lz=n * h)
+            shape = (n, 1, 1)
+        p = ideal_gas_params(gamma=gam, tvd_form=tvd_form)
+        i = np.arange(n)
+        heavy = (i >= 4) & (i < 11)                                  # jumps at 3|4 and 10|11
+        X = state_from_primitives(g, p, np.where(heavy, rl, rr).reshape(shape), 0.0, 0.0, 0.0, p0)
+        for direction in (+1, -1):
+            Y = orc.sweep(orc.Problem(g, p), X, axis, tau, direction)
+            d = (Y - X).reshape(4, g["nz"], g["nx"])
+            assert np.all(d[1:] == 0.0)                              # momenta and E untouched, bit for bit
+            line = d[0][:, 2] if axis == 2 else d[0][2, :]
+            Cl, Cr = C(cl * tau / h), C(cr * tau / h)
+            amount = (0.5 * (Cl + Cr) if tvd_form == 1 else 0.25 * (Cl + Cr)) * (rl - rr)
+            want = np.zeros(n)
+            want[3], want[4], want[10], want[11] = +amount, -amount, -amount, +amount
+            np.testing.assert_allclose(line, want, rtol=0, atol=2e-16)
+    # both nodes beyond Co = 0.5: C = 0.25 exactly, so a quarter (an eighth) of the jump crosses
+    assert amount == (0.25 if tvd_form == 1 else 0.125) * (rl - rr)
+
+
+def test_contact_next_to_a_plate_records_R11(orc):
+    """DESIGN.md R11 (the paper is silent): the dissipation flux of Eq. 34 is dropped on the two interfaces
+    that touch a plate node, whose r+- would need a node outside the box.  A contact at rest sitting on the
+    plate-adjacent interface therefore stays put bit for bit, while the same contact one interface further in
+    is smoothed.  This records the reading; nothing in the paper pins it."""
+    gam, p0 = 1.4, 1.0
+    nz = 12
+    for k_jump, moves in ((0, False), (1, True), (nz - 2, False), (nz - 3, True)):
+        rho = np.where(np.arange(nz) <= k_jump, 1.0, 0.25)
+        g = inputs.make_grid(2, 6, nz, lx=0.6, lz=1.1)
+        # plates at the local gas temperature T = p / (R rho), R = gamma - 1 in these units
+        p = ideal_gas_params(gamma=gam, bc_z=0, T_bot=p0 / ((gam - 1) * rho[0]), T_top=p0 / ((gam - 1) * rho[-1]))
+        X = state_from_primitives(g, p, rho[:, None, None], 0.0, 0.0, 0.0, p0)
+        for direction in (+1, -1):
+            Y = orc.sweep(orc.Problem(g, p), X, 2, 0.01, direction)
+            assert np.allclose(Y[1:], X[1:], rtol=0, atol=1e-15)
+            assert np.array_equal(Y[0], X[0]) != moves, (k_jump, direction)
+
+
+# ----------------------------------------------------------------------------- second order in time (Eq. 32's S^P)
+_TAYLOR = {}
+
+
+def _euler_gravity_taylor(gam, g):
+    """X, X_t and X_tt of the 1-D inviscid equations with gravity (Eqs. 13-15 along z, PAPER.md:181-185:
+    rho_t = -(rho w)_z;  (rho w)_t = -(rho w^2 + p)_z - g rho;  E_t = -(w (E + p))_z with
+    E = rho w^2/2 + p/(gamma-1) + rho g z) for the smooth state below, derived symbolically (sympy) from
+    the PDE itself -- nothing of the scheme enters."""
+    if (gam, g) in _TAYLOR:
+        return _TAYLOR[(gam, g)]
+    import sympy as sp
+    z, s = sp.symbols("z s")
+    k = 2 * sp.pi
+    G, gg = sp.Float(gam), sp.Float(g)
+    rho = 1 + sp.Rational(1, 5) * sp.sin(k * z)
+    w = sp.Rational(3, 10) * sp.sin(k * z + 1)
+    pr = 1 + sp.Rational(1, 10) * sp.cos(k * z)
+    X = (rho, rho * w, rho * w * w / 2 + pr / (G - 1) + rho * gg * z)
+
+    def rhs(r, m, E):
+        u = m / r
+        p = (G - 1) * (E - m * u / 2 - r * gg * z)
+        return (-sp.diff(m, z), -sp.diff(m * u + p, z) - gg * r, -sp.diff(u * (E + p), z))
+
+    Xt = rhs(*X)
+    Xtt = [sp.diff(c, s).subs(s, 0) for c in rhs(*[a + s * b for a, b in zip(X, Xt)])]
+    out = tuple([sp.lambdify(z, e, "numpy") for e in grp] for grp in (X, Xt, Xtt))
+    _TAYLOR[(gam, g)] = out
+    return out
+
+
+@pytest.mark.parametrize("direction", [+1, -1])
+def test_one_operator_is_second_order_in_time_with_gravity(orc, direction):
+    """the scheme is second order in space AND time.  One operator L_z(tau) applied to a smooth
+    state with gravity must then reproduce X + tau X_t + tau^2 X_tt / 2 of the PDE up to O(h^3) when tau ~ dz = h,
+    i.e. the local error falls 8x per halving.  The g tau^2 (rho w)_z / 2 part of X_tt only appears if the
+    corrector's source is taken at the predicted state (S^P_k in Eq. 32); with S(X^n) the local
+    error of rho w is O(h^2) and falls 4x.  (z is periodic here; gravity makes the periodic seam inconsistent,
+    so nodes within 4 of it are left out: one operator reaches 2 nodes.)"""
+    gam, g = 1.4, 10.0
+    f0, ft, ftt = _euler_gravity_taylor(gam, g)
+    errs = []
+    for n in (32, 64, 128):
+        grid = periodic_grid(2, 4, n, lx=4.0 / n, lz=1.0)
+        p = ideal_gas_params(gamma=gam, g_override=g, tvd_off=1)
+        zz = np.arange(n) / n
+        tau = 0.2 / n
+        cols = lambda f: np.repeat(np.asarray(f(zz), dtype=float)[:, None], 4, 1).reshape(-1)
+        X0 = np.stack([cols(f0[0]), np.zeros(4 * n), cols(f0[1]), cols(f0[2])])
+        Y = orc.sweep(orc.Problem(grid, p), X0, 2, tau, direction).reshape(4, n, 4)[:, :, 0]
+        sel = slice(4, n - 4)
+        e = []
+        for i, f in ((0, 0), (1, 2)):                                # rho and rho w
+            exact = f0[i](zz) + tau * ft[i](zz) + 0.5 * tau**2 * ftt[i](zz)
+            e.append(np.abs(Y[f][sel] - exact[sel]).max())
+        errs.append(e)
+    errs = np.array(errs)
+    ratios = errs[:-1] / errs[1:]
+    assert np.all(ratios > 7.0) and np.all(ratios < 9.0), (errs, ratios)
+    assert errs[0, 1] < 3e-4
+
+
+# ----------------------------------------------------------------------------- R7: compact viscous stencil
+@pytest.mark.parametrize("a,b", [(0, 2), (2, 0)])
+def test_aligned_shear_wave_decays_at_the_compact_stencil_rate(orc, a, b):
+    """R7: inside F_alpha the derivative along alpha is one-sided, OPPOSITE to the stage's outer difference, so
+    that predictor and corrector each form the compact second difference (f_{k+1} - 2 f_k + f_{k-1})/h^2.  A
+    grid-aligned shear wave u_a = A sin(k x_b) in a gas at rest then decays at exactly nu (2 - 2 cos(k h))/h^2
+    (the symbol of that stencil; time-stepping error ~1e-5 here).  The same-side rule would give the wide
+    stencil (f_{k+2} - 2 f_k + f_{k-2})/(2h)^2-like average, whose rate is smaller by cos(k h): 7.6 % at
+    n = 16."""
+    gam, nu, A, n, t_end = 1.4, 0.02, 1e-3, 16, 1.0
+    dims = {0: 4, 2: 4}
+    dims[b] = n
+    g = periodic_grid(2, dims[0], dims[2], lx=1.0 if b == 0 else 4.0 / n, lz=1.0 if b == 2 else 4.0 / n)
+    p = ideal_gas_params(gamma=gam, mu_override=nu, tvd_off=1, cfl=0.25)
+    x = (np.arange(dims[0]) / dims[0])[None, None, :]
+    z = (np.arange(dims[2]) / dims[2])[:, None, None]
+    s = x if b == 0 else z
+    k, h = 2 * np.pi, 1.0 / n
+    u = [0.0, 0.0, 0.0]
+    u[a] = A * np.sin(k * s)
+    X = state_from_primitives(g, p, 1.0, u[0], 0.0, u[2], 1.0 / gam)
+    X, _ = advance_to(orc, orc.Problem(g, p), X, t_end)
+    ua = primitives_of(g, p, X)[1 + a]
+    rate = -np.log(2 * np.mean(ua * np.sin(k * s + 0 * ua)) / A) / t_end
+    compact = nu * (2 - 2 * np.cos(k * h)) / h**2
+    assert rate == pytest.approx(compact, rel=1e-4), (rate, compact, compact * np.cos(k * h))
+    assert abs(rate / (nu * k * k) - 1) < 0.02                       # and it approximates nu k^2
+
+
+# ----------------------------------------------------------------------------- Eq. 30: the operator sequence
+@pytest.mark.parametrize("ndim", [2, 3])
+def test_step_is_the_operator_sequence_of_eq30(orc, ndim):
+    """Eq. 30: X^(n+1) = L_x L_y L_z L_x L_y L_z X^n, each with dt/2, operators acting right
+    to left (no L_y in 2-D).  With R9's alternation the list, in the order of application, is
+        L_z(+1), [L_y(+1),] L_x(+1), L_z(-1), [L_y(-1),] L_x(-1),  each with tau = dt/2.
+    One step must equal that list of single operators bit for bit, and must differ from the x-first order
+    (R8: the operators do not commute on a generic state)."""
+    g = inputs.make_grid(ndim, 12, 9, 8 if ndim == 3 else 1)
+    p = inputs.make_params(Ra=1e3)
+    X = inputs.smooth_random_state(g, p, seed=17)
+    prob = orc.Problem(g, p)
+    dt = 0.8 * orc.dt(prob, X)
+    tau = 0.5 * dt
+    z, y, x = 2, 1, 0
+    sequence = [(z, +1), (y, +1), (x, +1), (z, -1), (y, -1), (x, -1)]
+    if ndim == 2:
+        sequence = [(a, d) for a, d in sequence if a != y]
+    Y = X
+    for alpha, direction in sequence:
+        Y = orc.sweep(prob, Y, alpha, tau, direction)
+    got, dts, t = orc.step(prob, X, 1, dt_in=[dt])
+    assert np.array_equal(got, Y)
+    assert dts[0] == dt and t == dt
+    W = X
+    for alpha, direction in [(a, d) for d in (+1, -1) for a in ((x, z) if ndim == 2 else (x, y, z))]:
+        W = orc.sweep(prob, W, alpha, tau, direction)
+    assert np.max(rel_err(W, Y)) > 1e-9
+    # dir_mode 0 (the paper's fixed backward predictor): both triples with dir = +1
+    p0 = inputs.make_params(Ra=1e3, dir_mode=0)
+    prob0 = orc.Problem(g, p0)
+    Y0 = X
+    for alpha, _ in sequence:
+        Y0 = orc.sweep(prob0, Y0, alpha, tau, +1)
+    assert np.array_equal(orc.step(prob0, X, 1, dt_in=[dt])[0], Y0)
 
 
 # ----------------------------------------------------------------------------- gravity, plates
