@@ -11,6 +11,7 @@
 #include <new>
 #include <type_traits>
 
+#include "mc_async.cuh"
 #include "mc_common.cuh"
 #include "reduce_kernels.cuh"
 #include "sweep_lane.cuh"
@@ -47,6 +48,15 @@ size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 #ifndef MC_LANE3_WB
 #define MC_LANE3_WB 12
 #endif
+#ifndef MC_MARCH3_WB_AS
+#define MC_MARCH3_WB_AS 12
+#endif
+#ifndef MC_ASYNC3
+#define MC_ASYNC3 1
+#endif
+#ifndef MC_TMA_L2PROMO
+#define MC_TMA_L2PROMO CU_TENSOR_MAP_L2_PROMOTION_NONE
+#endif
 #ifndef MC_LANE2_WARPS
 #define MC_LANE2_WARPS 4
 #endif
@@ -66,6 +76,7 @@ constexpr int MARCH_WX_2D = MC_MARCH_WX_2D;      // k_march, 2-D: WX - 4 outputs
 constexpr int MARCH_MINB_2D = MC_MARCH_MINB_2D;  // k_march, 2-D: resident blocks per SM the register budget allows
 constexpr int MARCH3_WB = MC_MARCH3_WB;          // k_march3: 32 x WB threads, 28 x (WB - 2) outputs
 constexpr int LANE3_WB = MC_LANE3_WB;            // k_lane3: 32 x WB threads, 28 x (WB - 2) outputs
+constexpr int MARCH3_WB_AS = MC_MARCH3_WB_AS;    // the same with asynchronous staging (TMA + row mbarriers)
 constexpr int LANE_WARPS_2D = MC_LANE_WARPS_2D;  // k_lane, 2-D: independent warps per block
 constexpr int LANE_MINB_2D = MC_LANE_MINB_2D;
 constexpr int DIAG_MAX_BLOCKS = 16;    // blocks per plane in the diagnostics pass (the finish kernel walks them)
@@ -100,6 +111,10 @@ struct mc_tvd_state {
     int n_ev, n_rec;
     int *rec_kind, *rec_ev;
     bool ev_open;                      // the last recorded event directly precedes the next launch
+    // 3-D, even nx: TMA tensor maps (x, y, z, field) of the two state buffers [0] = X, [1] = Y, with the box
+    // of a z-march tile (32 x rows(y) x 1 x 5) and of a y-march tile (32 x 1 x rows(z) x 5)
+    bool async3;
+    CUtensorMap tm_rows_y[2], tm_rows_z[2];
 };
 
 namespace {
@@ -237,12 +252,39 @@ template <class F> void with_tvd(const mc_tvd_state *s, F f)
     else f(std::integral_constant<int, 1>());
 }
 
-template <class K> int launch_kernel(K kfn, dim3 grid, dim3 block, size_t smem, cudaStream_t st, const mc::SweepArgs &A)
+// Tiled tensor map over a 5-field SoA state (x fastest): box = 32 columns x rows_y x rows_z x 5 fields, fp64,
+// no swizzle (a thread reads its own column: consecutive lanes, consecutive doubles), zero fill outside.
+int make_state_map(CUtensorMap *map, const double *base, int nx, int ny, int nz, int rows_y, int rows_z)
+{
+    typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static encode_fn encode = nullptr;                 // resolved once; the value is the same for every thread
+    if (!encode) {
+        void *fn = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) != cudaSuccess || !fn)
+            return fail(MC_TVD_ECUDA, "cuTensorMapEncodeTiled is not available in this driver");
+        encode = (encode_fn)fn;
+    }
+    const cuuint64_t dims[4] = {(cuuint64_t)nx, (cuuint64_t)ny, (cuuint64_t)nz, 5};
+    const cuuint64_t strides[3] = {(cuuint64_t)nx * 8, (cuuint64_t)nx * ny * 8, (cuuint64_t)nx * ny * nz * 8};
+    const cuuint32_t box[4] = {32, (cuuint32_t)rows_y, (cuuint32_t)rows_z, 5};
+    const cuuint32_t estr[4] = {1, 1, 1, 1};
+    const CUresult r = encode(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, (void *)base, dims, strides, box, estr,
+                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, MC_TMA_L2PROMO,
+                              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(MC_TVD_ECUDA, "cuTensorMapEncodeTiled failed");
+    return MC_TVD_OK;
+}
+
+template <class K, class... Extra>
+int launch_kernel(K kfn, dim3 grid, dim3 block, size_t smem, cudaStream_t st, const mc::SweepArgs &A, const Extra &...extra)
 {
     // opt in to large dynamic shared memory: a per-function attribute, set before every such launch (no
     // cache to guard: distinct handles may launch from different threads)
     if (smem > 48 * 1024) cudaFuncSetAttribute(kfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    MC_LAUNCH(kfn, grid, block, smem, st, A);
+    MC_LAUNCH(kfn, grid, block, smem, st, A, extra...);
     return 0;
 }
 
@@ -296,7 +338,28 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
         }
     } else {
         long long xt = (nx + mc::LANE_OUT - 1) / mc::LANE_OUT;
-        if (alpha == 2) {            // z-sweep: march z, tile (x, y)
+        const int ibuf = (in == s->X) ? 0 : 1;        // which state buffer the operator reads
+        if (alpha == 2 && s->async3) {   // z-sweep, TMA-staged tiles: march z, tile (x, y)
+            constexpr int MW = MARCH3_WB_AS, MO = MW - 2;
+            A.n_b = ny; A.s_b = nx; A.n_m = nz; A.s_m = (long long)nx * ny;
+            long long bt = (ny + MO - 1) / MO;
+            A.chunk = pick_chunk(s, nz, xt * bt, 1);
+            dim3 mblock(32, MW, 1), grid((unsigned)xt, (unsigned)bt, (unsigned)((nz + A.chunk - 1) / A.chunk));
+            size_t smem = mc::tile3_async_bytes(MW) + ((size_t)4 * 3 * 32 * (MW + 2) + 4) * sizeof(double);
+            with_walls(wl, [&](auto W) { with_tvd(s, [&](auto T) {
+                launch_kernel(mc::k_march3<2, 1, MW, decltype(W)::value, false, decltype(T)::value, 1, true>, grid, mblock, smem, st, A, s->tm_rows_y[ibuf]);
+            }); });
+        } else if (alpha == 1 && s->async3) {   // y-sweep, TMA-staged tiles: march y, tile (x, z)
+            constexpr int MW = MARCH3_WB_AS, MO = MW - 2;
+            A.n_b = nz; A.s_b = (long long)nx * ny; A.n_m = ny; A.s_m = nx;
+            long long bt = (nz + MO - 1) / MO;
+            A.chunk = pick_chunk(s, ny, xt * bt, 1);
+            dim3 mblock(32, MW, 1), grid((unsigned)xt, (unsigned)bt, (unsigned)((ny + A.chunk - 1) / A.chunk));
+            size_t smem = mc::tile3_async_bytes(MW) + ((size_t)4 * 3 * 32 * (MW + 2) + 4) * sizeof(double);
+            with_walls(wl, [&](auto W) { with_tvd(s, [&](auto T) {
+                launch_kernel(mc::k_march3<1, 2, MW, false, decltype(W)::value, decltype(T)::value, 1, true>, grid, mblock, smem, st, A, s->tm_rows_z[ibuf]);
+            }); });
+        } else if (alpha == 2) {            // z-sweep: march z, tile (x, y)
             constexpr int MW = MARCH3_WB, MO = MW - 2;
             A.n_b = ny; A.s_b = nx; A.n_m = nz; A.s_m = (long long)nx * ny;
             long long bt = (ny + MO - 1) / MO;
@@ -304,7 +367,7 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
             dim3 mblock(32, MW, 1), grid((unsigned)xt, (unsigned)bt, (unsigned)((nz + A.chunk - 1) / A.chunk));
             size_t smem = ((size_t)4 * 3 * 32 * (MW + 2) + 4) * sizeof(double);
             with_walls(wl, [&](auto W) { with_tvd(s, [&](auto T) {
-                launch_kernel(mc::k_march3<2, 1, MW, decltype(W)::value, false, decltype(T)::value, MC_MARCH3_MINB>, grid, mblock, smem, st, A);
+                launch_kernel(mc::k_march3<2, 1, MW, decltype(W)::value, false, decltype(T)::value, MC_MARCH3_MINB, false>, grid, mblock, smem, st, A, s->tm_rows_y[ibuf]);
             }); });
         } else if (alpha == 1) {     // y-sweep: march y, tile (x, z)
             constexpr int MW = MARCH3_WB, MO = MW - 2;
@@ -314,7 +377,7 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
             dim3 mblock(32, MW, 1), grid((unsigned)xt, (unsigned)bt, (unsigned)((ny + A.chunk - 1) / A.chunk));
             size_t smem = ((size_t)4 * 3 * 32 * (MW + 2) + 4) * sizeof(double);
             with_walls(wl, [&](auto W) { with_tvd(s, [&](auto T) {
-                launch_kernel(mc::k_march3<1, 2, MW, false, decltype(W)::value, decltype(T)::value, MC_MARCH3_MINB>, grid, mblock, smem, st, A);
+                launch_kernel(mc::k_march3<1, 2, MW, false, decltype(W)::value, decltype(T)::value, MC_MARCH3_MINB, false>, grid, mblock, smem, st, A, s->tm_rows_z[ibuf]);
             }); });
         } else {                     // x-sweep: lanes x, tile (x, y), march z
             constexpr int LW = LANE3_WB, LO = LW - 2;
@@ -428,10 +491,22 @@ int mc_tvd_init(const mc_tvd_grid *grid, const mc_tvd_params *params, double *d_
         s->sm_count = sms;
     }
 
+    int rc = MC_TVD_OK;
+    // TMA needs 16-byte row strides: an odd nx keeps the kernels that load through registers
+    s->async3 = MC_ASYNC3 && s->nd == 3 && grid->nx % 2 == 0;
+    if (s->async3) {
+        const double *buf[2] = {s->X, s->Y};
+        for (int b = 0; b < 2 && rc == MC_TVD_OK; ++b) {
+            rc = make_state_map(&s->tm_rows_y[b], buf[b], grid->nx, grid->ny, grid->nz, MARCH3_WB_AS + 2, 1);
+            if (rc == MC_TVD_OK) rc = make_state_map(&s->tm_rows_z[b], buf[b], grid->nx, grid->ny, grid->nz, 1, MARCH3_WB_AS + 2);
+        }
+        if (rc != MC_TVD_OK) { delete s; return rc; }
+    }
+
     mc::Scalars h;
     memset(&h, 0, sizeof(h));
     h.cfl = params->cfl; h.fixed_dt = params->fixed_dt;
-    int rc = cuda_check(cudaMemcpyAsync(s->S, &h, sizeof(h), cudaMemcpyHostToDevice, s->stream), "scalar upload");
+    rc = cuda_check(cudaMemcpyAsync(s->S, &h, sizeof(h), cudaMemcpyHostToDevice, s->stream), "scalar upload");
     if (rc == MC_TVD_OK) rc = cuda_check(cudaStreamSynchronize(s->stream), "scalar upload sync");   // h is on the stack
     if (rc == MC_TVD_OK) rc = enqueue_initial_dt(s);
     if (rc != MC_TVD_OK) { delete s; return rc; }

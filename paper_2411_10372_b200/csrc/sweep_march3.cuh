@@ -16,9 +16,25 @@
 //
 // Pipeline of iteration j (output level j), identical to k_march:
 //   prefetch X(j+3) | W(j+2) -> TVD(j+1/2) -> F(j+1) -> P(j+1) | barrier | F^P(j+1) -> out(j)
+//
+// AS = true (the default path, even nx): ASYNCHRONOUS STAGING.  The X tile of every level -- 32 columns x
+// (WB + 2) rows x 5 fields, ring-2 rows included -- is brought in by ONE cp.async.bulk.tensor (TMA, 4-D tensor
+// map (x, y, z, field)) per level into a ring of MARCH3_STAGES shared-memory stages, MARCH3_STAGES - 1 levels
+// ahead, completing on a "full" mbarrier; a thread reads its own column's X(j+2) from the stage (conflict-free
+// LDS), its warp then arrives on the stage's "empty" mbarrier, and one elected lane refills it.  So no
+// register prefetch (X(j+3) and the ring-2 row: 9 doubles less carried), no L2 prefetch instructions, no
+// per-thread load addresses, and no exposed HBM latency.  Nodes the box cannot deliver -- columns or rows that
+// wrap around the periodic seam -- are zero-filled by the TMA unit and loaded by their thread directly.
+// The per-level __syncthreads is replaced by DATAFLOW between neighbouring rows: each row (warp) owns an
+// mbarrier on which it arrives once it has published u(j+2) and u^P(j+1); before F^P(j+1) it waits only for
+// rows r-1 and r+1.  Neighbouring rows thus stay within one level of each other (which is all the double
+// buffered velocity planes need: see the hazard analysis in DESIGN.md 7), but rows far apart -- and with them
+// the three or four warps sharing an SM sub-partition -- drift by several levels, so one warp's dependent
+// chain overlaps another's instead of all warps draining into the barrier together.
 #pragma once
 #include <type_traits>
 
+#include "mc_async.cuh"
 #include "mc_common.cuh"
 #include "sweep_march.cuh"
 
@@ -36,16 +52,32 @@ namespace mc {
 #ifndef MC_MARCH3_REGS
 #define MC_MARCH3_REGS (((65536 / (32 * WB * MINB)) / 8 * 8) > 248 ? 248 : ((65536 / (32 * WB * MINB)) / 8 * 8))
 #endif
-template <int CA, int CB, int WB, bool WALL_M, bool WALL_B, int TVD, int MINB = 1>
-MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
+#ifndef MC_MARCH3_STAGES
+#define MC_MARCH3_STAGES 4
+#endif
+constexpr int MARCH3_STAGES = MC_MARCH3_STAGES;      // power of two
+// dynamic shared memory of k_march3 / k_lane3 with asynchronous staging: stage ring (128-byte aligned) +
+// mbarriers + velocity planes
+__host__ __device__ constexpr size_t tile3_stage_bytes(int WB) { return (size_t)5 * 32 * (WB + 2) * sizeof(double); }
+__host__ __device__ constexpr size_t tile3_async_bytes(int WB) { return MARCH3_STAGES * tile3_stage_bytes(WB) + 8 * (2 * MARCH3_STAGES + 2 * WB); }
+
+template <int CA, int CB, int WB, bool WALL_M, bool WALL_B, int TVD, int MINB = 1, bool AS = false>
+MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A, const __grid_constant__ CUtensorMap tmap)
 {
     constexpr int ND = 3, NF = 5;
     constexpr bool Z_IS_ALPHA = (CA == ND - 1);
     constexpr int OB = WB - 2;                        // output rows per tile
     static_assert(WB >= 3 && WB % 4 == 0, "the SM allocates warps in fours: other row counts waste registers");
     constexpr int TILE = 32 * (WB + 2);               // shared-memory plane: tile rows plus the ring-2 rows
+    constexpr int S = MARCH3_STAGES;
+    static_assert((S & (S - 1)) == 0, "stage count must be a power of two");
     MC_SHARED_DECL(double, smem_raw);
-    double *const smem = smem_raw + 2;                // two pad doubles in front
+    // AS: [stage ring (the dynamic shared memory is 128-byte aligned)][full[S], empty[S], row[2][WB]][velocity planes]
+    constexpr int RING_DOUBLES = AS ? S * (int)(tile3_stage_bytes(WB) / sizeof(double)) : 0;
+    constexpr int BAR_DOUBLES = AS ? 2 * S + 2 * WB : 0;
+    const double *const ring = smem_raw;
+    double *const bars = smem_raw + RING_DOUBLES;
+    double *const smem = smem_raw + RING_DOUBLES + BAR_DOUBLES + 2;   // two pad doubles in front
     double *const slotU = smem;                       // [2][ND][TILE]  velocities of X     (levels j+1, j+2)
     double *const slotP = smem + 2 * ND * TILE;       // [2][ND][TILE]  velocities of X^P   (level j+1)
 
@@ -80,6 +112,13 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
     if (!row_exists) role = ROLE_NONE;
     else if (wallrow) role = ROLE_WALLROW;
     else if (edge) role = ROLE_R1;
+    // AS: can the TMA box deliver this thread's node (and its ring-2 neighbour)?  Not across the periodic seam.
+    const bool in_box = gx >= 0 && gx < A.nx && gb_raw >= 0 && gb_raw < A.n_b;
+    const bool in_box_o = gx >= 0 && gx < A.nx && go_raw >= 0 && go_raw < A.n_b;
+    // AS: rows (warps) that take part: with plates across b the rows outside the box do nothing and leave
+    const int b_first = (int)blockIdx.y * OB - 1;                      // gb_raw of row 0
+    const int ty_lo = WALL_B ? max(0, -b_first) : 0;                   // first and last existing row
+    const int ty_hi = WALL_B ? min(WB - 1, A.n_b - 1 - b_first) : WB - 1;
 
     // ---- sweep constants ------------------------------------------------------------------
     const double tau = A.dt_ptr ? 0.5 * (*A.dt_ptr) : A.tau_fixed;
@@ -157,6 +196,89 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
     };
 
 
+    // ---- AS: stage ring, barriers ----------------------------------------------------------------
+    const unsigned bar0 = AS ? smem_addr(bars) : 0u;                   // full[S], empty[S], row[WB]
+    const unsigned ring0 = AS ? smem_addr(ring) : 0u;
+    const int j_start = (WALL_M && l0 == 0) ? -2 : l0 - 4;             // below a plate there is nothing to warm up
+    const int n_lev = l1 + 2 - (j_start + 2);                          // levels j_start+2 .. l1+1 are staged, one per iteration
+    const bool prod_warp = AS && ty == ty_lo;                          // the warp whose lane 0 feeds the ring
+    // whole tile inside the box: no thread needs the direct-load path (true for all but the seam tiles)
+    const bool tile_in_box = (int)blockIdx.x * 28 - 2 >= 0 && (int)blockIdx.x * 28 + 30 <= A.nx && b_first - 1 >= 0 &&
+                             b_first + WB + 1 <= A.n_b;
+    // issue the TMA load of staged level number q (march level j_start + 2 + q) into stage q % S (lane 0 only)
+    auto issue = [&](int q) MC_INL {
+        const int l = j_start + 2 + q;
+        const int pk = (WALL_M && (l < 0 || l >= n)) ? -1 : phys_k(l);  // a level beyond a plate: all zero fill
+        const unsigned full = bar0 + 8u * (unsigned)(q & (S - 1));
+        const int x0 = (int)blockIdx.x * 28 - 2, b0 = b_first - 1;
+        tma_issue_4d_if(tx == 0, ring0 + (unsigned)(q & (S - 1)) * (unsigned)tile3_stage_bytes(WB), &tmap, full,
+                        (unsigned)tile3_stage_bytes(WB), x0, CB == 1 ? b0 : pk, CB == 1 ? pk : b0, 0);
+    };
+    if (AS) {
+        if (threadIdx.x == 0 && threadIdx.y == 0) {
+            for (int i = 0; i < S; ++i) { mbar_init(bar0 + 8u * i, 1); mbar_init(bar0 + 8u * (S + i), (unsigned)(ty_hi - ty_lo + 1)); }
+            for (int i = 0; i < 2 * WB; ++i) mbar_init(bar0 + 8u * (2 * S + i), 1);
+            mbar_init_fence();
+        }
+        __syncthreads();
+        if (role == ROLE_NONE) return;
+        if (prod_warp) {
+            if (tx == 0) tma_prefetch_descriptor(&tmap);
+            for (int q = 0; q < S - 1 && q < n_lev; ++q) issue(q);
+        }
+    }
+    int it = 0;                                                         // AS: iteration number = staged level number read
+    // AS: take X(j+2) (and the ring-2 row's rho, m for a ring-1 row) of this iteration out of its stage
+    auto stage_read = [&](auto role_tag, bool want, int l, double (&X)[NF], double (&Xo)[ND + 1]) MC_INL {
+        constexpr int ROLE = decltype(role_tag)::value;
+        const unsigned st = (unsigned)it & (S - 1), ph = ((unsigned)it / S) & 1u;
+        mbar_wait(bar0 + 8u * st, ph);
+        if (want) {
+            const double *sp = ring + (size_t)st * (tile3_stage_bytes(WB) / sizeof(double));
+            if (tile_in_box) {                                           // block uniform
+#pragma unroll
+                for (int f = 0; f < NF; ++f) X[f] = sp[f * TILE + tidx];
+                if (ROLE == ROLE_R1 && has_outer) {
+#pragma unroll
+                    for (int f = 0; f <= ND; ++f) Xo[f] = sp[f * TILE + tidx_o];
+                }
+            } else {
+                if (in_box) {
+#pragma unroll
+                    for (int f = 0; f < NF; ++f) X[f] = sp[f * TILE + tidx];
+                } else {
+                    load_at(off_of(l), X);
+                }
+                if (ROLE == ROLE_R1 && has_outer) {
+                    if (in_box_o) {
+#pragma unroll
+                        for (int f = 0; f <= ND; ++f) Xo[f] = sp[f * TILE + tidx_o];
+                    } else {
+                        load_outer(off_of(l) - off_base + off_base_o, Xo);
+                    }
+                }
+            }
+        }
+        __syncwarp();
+        mbar_arrive_if(bar0 + 8u * (S + st), tx == 0);                   // this warp is done with the stage
+        if (prod_warp && it + S - 1 < n_lev) {                           // warp uniform: refill the stage of the PREVIOUS iteration
+            if (it > 0) mbar_wait(bar0 + 8u * (S + (((unsigned)it - 1) & (S - 1))), (((unsigned)it - 1) / S) & 1u);
+            issue(it + S - 1);
+        }
+    };
+    // AS: the row has published u(j+2), u^P(j+1); wait for the two neighbouring rows to have done the same
+    const bool wait_lo = ty > ty_lo, wait_hi = ty < ty_hi;
+    // two barriers per row, used alternately: a neighbour may complete iteration it + 1 on its OTHER barrier
+    // before this row has observed iteration it, but it + 2 needs this row's arrival for it + 1
+    auto level_sync = [&]() MC_INL {
+        if (!AS) { __syncthreads(); return; }
+        const unsigned rb = bar0 + 8u * (2 * S + ((unsigned)it & 1u) * WB + ty), ph = ((unsigned)it >> 1) & 1u;
+        __syncwarp();
+        mbar_arrive_if(rb, tx == 0);
+        if (wait_lo) mbar_wait(rb - 8u, ph);
+        if (wait_hi) mbar_wait(rb + 8u, ph);
+    };
+
     // ---- carried state (levels relative to the current output level j) -------------------------
     double Xn[NF];                 // X(j+2)
     double Xc[NF];                 // X(j+1)
@@ -215,24 +337,25 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
         const bool start_wall1 = !FAST && WALL_M && (j + 1 == 0);     // level j+1 is the plate the march starts on
         const bool end_wall1 = !FAST && WALL_M && (j + 1 == n - 1);   // level j+1 is the plate the march ends on
 
-        if (ROLE == ROLE_NONE) { __syncthreads(); return; }
+        if (ROLE == ROLE_NONE) { level_sync(); return; }          // (AS: such rows have left already)
 
-        // (0) prefetch X(j+3) into registers and X(j+3+MC_MARCH3_L2PF) into L2
+        // (0) not AS: prefetch X(j+3) into registers and X(j+3+MC_MARCH3_L2PF) into L2;  AS: take X(j+2) out of its stage
         const bool ld3 = FAST || (ex3 && j + 3 <= l1 + 1);
-#if MC_MARCH3_L2PF > 0
-        if (FAST) { if (j + 3 <= pf_last) prefetch_l2(o3 + (unsigned)MC_MARCH3_L2PF * sms); }
-        else if (j + 3 + MC_MARCH3_L2PF <= l1 + 1 && exists(j + 3 + MC_MARCH3_L2PF)) prefetch_l2(off_of(j + 3 + MC_MARCH3_L2PF));
-#endif
         double Xq[NF], Xoq[ND + 1];
-        auto fetch = [&]() MC_INL {
+        if (AS) {
+            stage_read(role_tag, ex2, j + 2, Xn, Xon);
+        } else {
+#if MC_MARCH3_L2PF > 0
+            if (FAST) { if (j + 3 <= pf_last) prefetch_l2(o3 + (unsigned)MC_MARCH3_L2PF * sms); }
+            else if (j + 3 + MC_MARCH3_L2PF <= l1 + 1 && exists(j + 3 + MC_MARCH3_L2PF)) prefetch_l2(off_of(j + 3 + MC_MARCH3_L2PF));
+#endif
 #pragma unroll
             for (int f = 0; f < NF; ++f) Xq[f] = Xn[f];
             if (ld3) load_at(o3, Xq);
 #pragma unroll
             for (int f = 0; f <= ND; ++f) Xoq[f] = Xon[f];
             if (ROLE == ROLE_R1 && ld3 && has_outer) load_outer(o3 - off_base + off_base_o, Xoq);
-        };
-        fetch();
+        }
 
         // (1) W(j+2)
         Prim<ND> w2 = w1;
@@ -245,12 +368,13 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
         if (ROLE == ROLE_WALLROW) {
             // a plate row of b (y-sweep): X^P = X and the output is X (R10); publish u^P = u of level j+1
             if (ld1) publish(slotP, p1, tidx, w1.u);
-            __syncthreads();
+            level_sync();
             if (j >= l0 && owner) store_at(o0, H0);
 #pragma unroll
-            for (int f = 0; f < NF; ++f) { H0[f] = Xc[f]; Xc[f] = Xn[f]; Xn[f] = Xq[f]; }
+            for (int f = 0; f < NF; ++f) { H0[f] = Xc[f]; Xc[f] = Xn[f]; if (!AS) Xn[f] = Xq[f]; }
             w1 = w2;
             if (FAST) { o3c += sms; o0c += sms; kd2c += dsgn; }
+            it += 1;
             return;
         }
 
@@ -258,18 +382,16 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
         double d1[NF], Dh[NF], a1 = 0.0, b1 = 0.0;
 #pragma unroll
         for (int f = 0; f < NF; ++f) { Dh[f] = 0.0; d1[f] = 0.0; }
-        {
-            if (ROLE == ROLE_IN && TVD >= 0) {
+        if (ROLE == ROLE_IN && TVD >= 0) {
 #pragma unroll
-                for (int f = 0; f < NF; ++f) d1[f] = (ld1 && ld2) ? Xn[f] - Xc[f] : 0.0;
+            for (int f = 0; f < NF; ++f) d1[f] = (ld1 && ld2) ? Xn[f] - Xc[f] : 0.0;
 #pragma unroll
-                for (int f = 0; f < NF; ++f) { b1 = fma(d1[f], d1[f], b1); a1 = fma(d0[f], d1[f], a1); }
-                const bool have = FAST || ((j >= l0 - 1) && exists(j - 1) && exists(j) && ex1 && ex2);   // R11 at plates
-                if (have) {
-                    const double coef = tvd_coef<(TVD >= 0 ? TVD : 0)>(a0, a1, b0, hC0, hC1);
+            for (int f = 0; f < NF; ++f) { b1 = fma(d1[f], d1[f], b1); a1 = fma(d0[f], d1[f], a1); }
+            const bool have = FAST || ((j >= l0 - 1) && exists(j - 1) && exists(j) && ex1 && ex2);   // R11 at plates
+            if (have) {
+                const double coef = tvd_coef<(TVD >= 0 ? TVD : 0)>(a0, a1, b0, hC0, hC1);
 #pragma unroll
-                    for (int f = 0; f < NF; ++f) { Dh[f] = coef * d0[f]; H0[f] += Dh[f]; }
-                }
+                for (int f = 0; f < NF; ++f) { Dh[f] = coef * d0[f]; H0[f] += Dh[f]; }
             }
         }
 
@@ -319,7 +441,7 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
         }
         if (ld1) publish(slotP, p1, tidx, wP1.u);
 
-        __syncthreads();
+        level_sync();
 
         if (ROLE == ROLE_IN) {
             // (5) F^P(j+1): flux of X^P at level j+1 (inner derivative backward in marching coordinates)
@@ -361,11 +483,14 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
         }
         // (7) rotate the pipeline
 #pragma unroll
-        for (int f = 0; f < NF; ++f) { Xc[f] = Xn[f]; Xn[f] = Xq[f]; F0[f] = F1[f]; H0[f] = H1[f]; }
+        for (int f = 0; f < NF; ++f) { Xc[f] = Xn[f]; if (!AS) Xn[f] = Xq[f]; F0[f] = F1[f]; H0[f] = H1[f]; }
+        if (!AS) {
 #pragma unroll
-        for (int f = 0; f <= ND; ++f) Xon[f] = Xoq[f];
+            for (int f = 0; f <= ND; ++f) Xon[f] = Xoq[f];
+        }
         w1 = w2; gz1 = gz2;
         if (FAST) { o3c += sms; o0c += sms; kd2c += dsgn; }
+        it += 1;
     };
 
     // ---- the march -------------------------------------------------------------------------------
@@ -375,8 +500,8 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A)
         integral_constant<bool, false> slow;
         integral_constant<bool, true> fast;
         integral_constant<int, -1> par_any;
-        int j = (WALL_M && l0 == 0) ? -2 : l0 - 4;      // below a plate there is nothing to warm up
-        if (exists(j + 2)) {
+        int j = j_start;
+        if (!AS && exists(j + 2)) {
             load(j + 2, Xn);
             if (ROLE == ROLE_R1 && has_outer) load_outer(off_of(j + 2) - off_base + off_base_o, Xon);
         }
