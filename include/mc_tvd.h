@@ -104,6 +104,12 @@ int mc_tvd_sweep(mc_tvd_state *s, int alpha, int dir, double tau);
  * Results do not depend on it; the parity tests use it to start blocks in the middle of a column. */
 int mc_tvd_debug_set_chunk(mc_tvd_state *s, int levels);
 
+/* Test hook: the tiling of operator alpha's most recent launch on this handle (all 0 before the first one):
+ * output nodes per thread-block tile along x (*tile_x) and along the tile's second direction (*tile_b; 1 in
+ * 2-D; y for L_z and L_x, z for L_y) and marching levels per block (*chunk).  The full-size parity tests place
+ * their sample windows across these boundaries. */
+int mc_tvd_debug_geometry(const mc_tvd_state *s, int alpha, int *tile_x, int *tile_b, int *chunk);
+
 /* The end-to-end call for callers whose state lives in HOST memory (pinned memory makes the copies
  * asynchronous, pageable memory works too): copies h_in (HOST, nf*N doubles, same layout) into
  * d_fields, recomputes dt from it (as mc_tvd_init does) and resets time and step count to zero, runs

@@ -48,6 +48,7 @@ SYMBOLS = {
     "mc_tvd_step": (C.c_int, [C.c_void_p, C.c_int]),
     "mc_tvd_sweep": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_double]),
     "mc_tvd_debug_set_chunk": (C.c_int, [C.c_void_p, C.c_int]),
+    "mc_tvd_debug_geometry": (C.c_int, [C.c_void_p, C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int)]),
     "mc_tvd_step_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]),
     "mc_tvd_dt": (C.c_int, [C.c_void_p, _DP]),
     "mc_tvd_diagnostics": (C.c_int, [C.c_void_p, C.POINTER(Diag), _DP, _DP, _DP]),
@@ -168,6 +169,12 @@ class MCTVD:
 
     def debug_set_chunk(self, levels: int):
         self._check(self.lib.mc_tvd_debug_set_chunk(self._h, int(levels)))
+
+    def debug_geometry(self, alpha: int):
+        """(outputs per tile along x, along the second tile direction, levels per chunk) of L_alpha's last launch."""
+        tx, tb, ch = C.c_int(), C.c_int(), C.c_int()
+        self._check(self.lib.mc_tvd_debug_geometry(self._h, int(alpha), C.byref(tx), C.byref(tb), C.byref(ch)))
+        return tx.value, tb.value, ch.value
 
     def step_host(self, h_in, h_out, n_steps: int):
         """h_in / h_out: CPU float64 torch tensors (pinned for async copies) or numpy arrays."""

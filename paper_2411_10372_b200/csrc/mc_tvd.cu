@@ -115,6 +115,7 @@ struct mc_tvd_state {
     // of a z-march tile (32 x rows(y) x 1 x 5) and of a y-march tile (32 x 1 x rows(z) x 5)
     bool async3;
     CUtensorMap tm_rows_y[2], tm_rows_z[2];
+    int geom[3][3];                    // per operator alpha, of its last launch: outputs per tile along x, along b, levels per chunk
 };
 
 namespace {
@@ -300,9 +301,11 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
     s->ev_open = timed;                // the closing event of this launch opens the next one
     const bool wl = s->walls;
     cudaStream_t st = s->stream;
+    int geo_x = 0, geo_b = 1;          // outputs per tile along x and along the second tile direction (test hook)
     if (s->nd == 2) {
         if (alpha == 2) {            // z-sweep: march z, tile x
             constexpr int WX = MARCH_WX_2D;
+            geo_x = WX - 4;
             A.n_b = 1; A.s_b = 0; A.n_m = nz; A.s_m = nx;
             long long tiles = (nx + WX - 5) / (WX - 4);
             A.chunk = pick_chunk(s, nz, tiles, MARCH_MINB_2D);
@@ -313,6 +316,7 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
             }); });
         } else if (alpha == 0 && MC_LANE2 && nx % 2 == 0) {   // x-sweep, even nx: two nodes per lane, march z
             constexpr int LW = MC_LANE2_WARPS;
+            geo_x = mc::LANE2_OUT;
             A.n_b = 1; A.s_b = 0; A.n_m = nz; A.s_m = nx;
             long long xt = (nx + mc::LANE2_OUT - 1) / mc::LANE2_OUT;
             long long tiles = (xt + LW - 1) / LW;
@@ -325,6 +329,7 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
             }); }); });
         } else if (alpha == 0) {     // x-sweep: lanes x, march z
             constexpr int LW = LANE_WARPS_2D;
+            geo_x = mc::LANE_OUT;
             A.n_b = 1; A.s_b = 0; A.n_m = nz; A.s_m = nx;
             long long xt = (nx + mc::LANE_OUT - 1) / mc::LANE_OUT;
             long long tiles = (xt + LW - 1) / LW;
@@ -339,10 +344,12 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
     } else {
         long long xt = (nx + mc::LANE_OUT - 1) / mc::LANE_OUT;
         const int ibuf = (in == s->X) ? 0 : 1;        // which state buffer the operator reads
+        geo_x = mc::LANE_OUT;
         if (alpha == 2 && s->async3) {   // z-sweep, TMA-staged tiles: march z, tile (x, y)
             constexpr int MW = MARCH3_WB_AS, MO = MW - 2;
             A.n_b = ny; A.s_b = nx; A.n_m = nz; A.s_m = (long long)nx * ny;
             long long bt = (ny + MO - 1) / MO;
+            geo_b = MO;
             A.chunk = pick_chunk(s, nz, xt * bt, 1);
             dim3 mblock(32, MW, 1), grid((unsigned)xt, (unsigned)bt, (unsigned)((nz + A.chunk - 1) / A.chunk));
             size_t smem = mc::tile3_async_bytes(MW) + ((size_t)4 * 3 * 32 * (MW + 2) + 4) * sizeof(double);
@@ -353,6 +360,7 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
             constexpr int MW = MARCH3_WB_AS, MO = MW - 2;
             A.n_b = nz; A.s_b = (long long)nx * ny; A.n_m = ny; A.s_m = nx;
             long long bt = (nz + MO - 1) / MO;
+            geo_b = MO;
             A.chunk = pick_chunk(s, ny, xt * bt, 1);
             dim3 mblock(32, MW, 1), grid((unsigned)xt, (unsigned)bt, (unsigned)((ny + A.chunk - 1) / A.chunk));
             size_t smem = mc::tile3_async_bytes(MW) + ((size_t)4 * 3 * 32 * (MW + 2) + 4) * sizeof(double);
@@ -363,6 +371,7 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
             constexpr int MW = MARCH3_WB, MO = MW - 2;
             A.n_b = ny; A.s_b = nx; A.n_m = nz; A.s_m = (long long)nx * ny;
             long long bt = (ny + MO - 1) / MO;
+            geo_b = MO;
             A.chunk = pick_chunk(s, nz, xt * bt, 1);
             dim3 mblock(32, MW, 1), grid((unsigned)xt, (unsigned)bt, (unsigned)((nz + A.chunk - 1) / A.chunk));
             size_t smem = ((size_t)4 * 3 * 32 * (MW + 2) + 4) * sizeof(double);
@@ -373,6 +382,7 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
             constexpr int MW = MARCH3_WB, MO = MW - 2;
             A.n_b = nz; A.s_b = (long long)nx * ny; A.n_m = ny; A.s_m = nx;
             long long bt = (nz + MO - 1) / MO;
+            geo_b = MO;
             A.chunk = pick_chunk(s, ny, xt * bt, 1);
             dim3 mblock(32, MW, 1), grid((unsigned)xt, (unsigned)bt, (unsigned)((ny + A.chunk - 1) / A.chunk));
             size_t smem = ((size_t)4 * 3 * 32 * (MW + 2) + 4) * sizeof(double);
@@ -383,6 +393,7 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
             constexpr int LW = LANE3_WB, LO = LW - 2;
             A.n_b = ny; A.s_b = nx; A.n_m = nz; A.s_m = (long long)nx * ny;
             long long bt = (ny + LO - 1) / LO;
+            geo_b = LO;
             A.chunk = pick_chunk(s, nz, xt * bt, 1);
             dim3 lblock(32, LW, 1), grid((unsigned)xt, (unsigned)bt, (unsigned)((nz + A.chunk - 1) / A.chunk));
             size_t smem = (size_t)4 * 2 * 32 * (LW + 2) * sizeof(double);
@@ -391,6 +402,7 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
             }); }); });
         }
     }
+    s->geom[alpha][0] = geo_x; s->geom[alpha][1] = geo_b; s->geom[alpha][2] = A.chunk;
     s->launches += 1;
     int rc = cuda_check(cudaGetLastError(), "sweep launch");
     if (rc == MC_TVD_OK && timed) {
@@ -554,6 +566,13 @@ int mc_tvd_sweep(mc_tvd_state *s, int alpha, int dir, double tau)
                                     s->stream), "sweep copy-back");
     if (rc != MC_TVD_OK) return rc;
     return enqueue_initial_dt(s);      // dt now belongs to the swept state (time and step count unchanged)
+}
+
+int mc_tvd_debug_geometry(const mc_tvd_state *s, int alpha, int *tile_x, int *tile_b, int *chunk)
+{
+    if (!s || alpha < 0 || alpha > 2 || !tile_x || !tile_b || !chunk) return fail(MC_TVD_EINVAL, "bad handle, alpha or output pointer");
+    *tile_x = s->geom[alpha][0]; *tile_b = s->geom[alpha][1]; *chunk = s->geom[alpha][2];
+    return MC_TVD_OK;
 }
 
 int mc_tvd_debug_set_chunk(mc_tvd_state *s, int levels)

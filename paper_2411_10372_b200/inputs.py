@@ -171,6 +171,61 @@ def smooth_random_state(grid: dict, params: dict, seed: int = SEED, u_amp: float
     return pack(grid, rho, ux, uy, uz, T, params)
 
 
+def rough_random_state(grid: dict, params: dict, seed: int = SEED, rough: float = 0.05) -> np.ndarray:
+    """`smooth_random_state` with seeded node-to-node noise of relative amplitude `rough` on rho, u and T of
+    the interior nodes: adjacent differences change sign from node to node, so the limiter ratios r+- of
+    Eq. 37 leave [1/2, infinity) on most nodes and the TVD term of Eqs. 34-39 is non-zero along every axis
+    (the smooth states keep phi = 1 almost everywhere).  Plate nodes keep u = 0 and T = T_w."""
+    nf = num_fields(grid)
+    nx, ny, nz = grid["nx"], grid["ny"], grid["nz"]
+    X = smooth_random_state(grid, params, seed=seed).reshape(nf, nz, ny, nx)
+    c = closure_constants(params)
+    z = z_nodes(grid, params)[:, None, None]
+    rho = X[0]
+    u = [X[1 + k] / rho for k in range(nf - 2)]
+    T = (X[nf - 1] / rho - 0.5 * sum(v * v for v in u) - c["g"] * z) / c["cv"]
+    idx = np.arange(nx * ny * nz, dtype=np.int64).reshape(nz, ny, nx)
+    noise = lambda k: 2.0 * hash_uniform(seed + 1000 * (k + 1), idx) - 1.0
+    interior = np.ones((nz, 1, 1))
+    if params["bc_z"] == 0:
+        interior[0] = interior[-1] = 0.0
+    rho = rho * (1.0 + rough * noise(0))
+    T = T * (1.0 + rough * noise(1) * interior)
+    u = [v + rough * noise(2 + k) * interior for k, v in enumerate(u)]
+    ux, uz = u[0], u[-1]
+    uy = u[1] if nf == 5 else np.zeros_like(rho)
+    return pack(grid, rho, ux, uy, uz, T, params)
+
+
+def moving_state(grid: dict, params: dict, seed: int = SEED, amplitude: float = 1e-3, u_amp: float = 0.05) -> np.ndarray:
+    """The conduction-plus-noise state of `conduction_state` set in motion: a smooth, plate-compatible
+    velocity field of amplitude u_amp (a few per cent of the sound speed) is added plane by plane, so the
+    full-size parity tests also sample a state that moves.  Host memory stays bounded by one z-plane."""
+    assert params["bc_z"] == 0
+    nf = num_fields(grid)
+    nx, ny, nz = grid["nx"], grid["ny"], grid["nz"]
+    X = conduction_state(grid, params, seed=seed, amplitude=amplitude).reshape(nf, nz, ny * nx)
+    zn = z_nodes(grid, params) / grid["lz"]
+    x = (np.arange(nx) / nx)[None, :]
+    y = (np.arange(ny) / ny)[:, None]
+    sx, cx = np.sin(2 * np.pi * 3 * x), np.cos(2 * np.pi * 3 * x)
+    sy, cy = np.sin(2 * np.pi * 2 * y), np.cos(2 * np.pi * 2 * y)
+    for k in range(1, nz - 1):
+        env = np.sin(np.pi * zn[k])
+        rho = X[0, k]
+        ux = (u_amp * env * (cy + 0 * x) * (1.0 + 0.3 * sx)).reshape(-1)
+        uy = (0.6 * u_amp * env * (sx + 0 * y)).reshape(-1)
+        uz = (0.8 * u_amp * env * (sx * cy if ny > 1 else sx + 0 * y)).reshape(-1) * np.cos(np.pi * zn[k])
+        if nf == 4:
+            uy = 0.0 * ux
+        X[1, k] = rho * ux
+        if nf == 5:
+            X[2, k] = rho * uy
+        X[nf - 2, k] = rho * uz
+        X[nf - 1, k] += 0.5 * rho * (ux * ux + uy * uy + uz * uz)
+    return X.reshape(nf, -1)
+
+
 def window_x(X: np.ndarray, grid: dict, i0: int, width: int):
     """Columns [i0, i0 + width) (periodic in x) of every field; returns (X_window, grid_window).
 

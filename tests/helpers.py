@@ -154,3 +154,20 @@ def ulp_perturbed(X, seed=1):
     rng = np.random.default_rng(seed)
     k = rng.integers(-1, 2, size=X.shape)
     return np.where(k > 0, np.nextafter(X, np.inf), np.where(k < 0, np.nextafter(X, -np.inf), X))
+
+
+def plate_nusselt_exact(grid, params, X):
+    """(nu_bottom, nu_top, nu_bar) of Eqs. 23-24 with the plane means of T summed in extended
+    precision: the reference for the Nu tolerance on large grids, where a plain serial fp64 sum of 1e4-1e6 plane
+    values (the oracle's) carries more rounding noise than the tolerance once the one-sided plate difference has
+    amplified it by 1/(eps dz).  Independent numpy restatement; second-order one-sided differences."""
+    T = primitives_of(grid, params, X)[4]
+    z = inputs.z_nodes(grid, params)
+    dz = z[1] - z[0]
+    k = [0, 1, 2, grid["nz"] - 3, grid["nz"] - 2, grid["nz"] - 1]
+    m = {j: float(np.sum(T[j].astype(np.longdouble)) / T[j].size) for j in k}
+    tsa = {j: m[j] - (1.0 - params["D"] * z[j]) for j in k}                      # T_sa = T - T_A, T_A = 1 - D z (Eq. 19)
+    g0 = (-3.0 * tsa[k[0]] + 4.0 * tsa[k[1]] - tsa[k[2]]) / (2.0 * dz)
+    g1 = (3.0 * tsa[k[5]] - 4.0 * tsa[k[4]] + tsa[k[3]]) / (2.0 * dz)
+    nb, nt = -g0 / params["eps"], -g1 / params["eps"]
+    return nb, nt, 0.5 * (nb + nt)

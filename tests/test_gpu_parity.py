@@ -16,7 +16,8 @@ TOL_SWEEP = 2e-13      # one operator L_alpha: a handful of roundings on O(1) fi
 TOL_1STEP = 1e-12      # parity_err norm
 TOL_100STEP = 1e-9
 TOL_NU = 1e-10
-COND_FACTOR = 10.0     # field-max norm: at most this many times the oracle's own response to 1-ulp input noise
+COND_FACTOR = 2.0      # field-max norm: at most twice the oracle's own response to 1-ulp input noise (measured on
+                       # B200: 0.6-1.0 times it after 1 step, 0.8 after 100; the values are printed by the C1 tests)
 
 
 @pytest.fixture(scope="module")
@@ -39,42 +40,66 @@ SWEEP_GRIDS = [
     (2, 29, 1, 5),        # smallest plate problem, one ragged tile
     (3, 60, 21, 19),      # 3-D: 3 x-tiles, 3 b-tiles (8 outputs) with ragged tails, walls in b for Ly
     (3, 30, 9, 33),       # ragged the other way
+    (3, 45, 17, 14),      # 3-D, odd nx: no TMA (16-byte row strides), the register-prefetch k_march3
     (2, 4, 1, 5),         # the smallest boxes the ABI accepts: a tile wraps the periodic seam several times
     (3, 6, 4, 6),
 ]
 
 
+def _state(kind, grid, params, seed):
+    """smooth: a few Fourier modes (the limiter stays at phi = 1 almost everywhere, the TVD term is ~0);
+    rough: the same plus node-to-node noise, which switches the TVD term on along every axis."""
+    if kind == "rough":
+        return inputs.rough_random_state(grid, params, seed=seed)
+    return inputs.smooth_random_state(grid, params, seed=seed)
+
+
+def _tvd_active_fraction(orc, grid, params, X0, alpha, tau, direction, ref):
+    """Fraction of nodes on which the TVD term of Eqs. 34-39 changes the operator's result (oracle, tvd on vs off)."""
+    off = orc.sweep(orc.Problem(grid, dict(params, tvd_off=1)), X0, alpha, tau, direction)
+    return float((np.abs(ref - off).max(axis=0) > 1e-9).mean())
+
+
 @pytest.mark.parametrize("ndim,nx,ny,nz", SWEEP_GRIDS)
 @pytest.mark.parametrize("bc_z", [0, 1])
 @pytest.mark.parametrize("tvd_form", [0, 1])
-def test_sweep_parity(gpu, orc, ndim, nx, ny, nz, bc_z, tvd_form):
+@pytest.mark.parametrize("kind", ["smooth", "rough"])
+def test_sweep_parity(gpu, orc, ndim, nx, ny, nz, bc_z, tvd_form, kind):
     grid = inputs.make_grid(ndim, nx, nz, ny)
     params = inputs.make_params(Ra=1e4, bc_z=bc_z, tvd_form=tvd_form)
-    X0 = inputs.smooth_random_state(grid, params, seed=11 + nx + bc_z)
+    X0 = _state(kind, grid, params, 11 + nx + bc_z)
     prob = orc.Problem(grid, params)
     tau = 0.25 * orc.dt(prob, X0)
     for alpha in ((0, 2) if ndim == 2 else (0, 1, 2)):
         for direction in (1, -1):
             ref = orc.sweep(prob, X0, alpha, tau, direction)
+            if kind == "rough":
+                # the limiter must really be exercised: along every axis, both directions, both forms of Eq. 34
+                # (between plates only the interior interfaces carry a dissipation flux, R11)
+                frac = _tvd_active_fraction(orc, grid, params, X0, alpha, tau, direction, ref)
+                assert frac >= (0.2 if bc_z == 0 and nz <= 6 else 0.5), (alpha, direction, frac)
             s = _solver(gpu, grid, params, X0)
             s.sweep(alpha, direction, tau)
             err = rel_err(s.state(), ref).max()
             s.close()
-            assert err <= TOL_SWEEP, (alpha, direction, err)
+            assert err <= TOL_SWEEP, (kind, alpha, direction, err)
 
 
 @pytest.mark.parametrize("ndim,nx,ny,nz", [(2, 300, 1, 70), (3, 60, 21, 19)])
 @pytest.mark.parametrize("chunk", [7, 16])
-def test_sweep_parity_chunked(gpu, orc, ndim, nx, ny, nz, chunk):
-    """Blocks that start in the middle of the marching direction (4-level warm-up)."""
+@pytest.mark.parametrize("tvd_form", [0, 1])
+def test_sweep_parity_chunked(gpu, orc, ndim, nx, ny, nz, chunk, tvd_form):
+    """Blocks that start in the middle of the marching direction (4-level warm-up), on a rough state so that the
+    TVD stencil of the warm-up levels (dX of the levels below the chunk) matters."""
     grid = inputs.make_grid(ndim, nx, nz, ny)
-    params = inputs.make_params(Ra=1e4)
-    X0 = inputs.smooth_random_state(grid, params, seed=5)
+    params = inputs.make_params(Ra=1e4, tvd_form=tvd_form)
+    X0 = inputs.rough_random_state(grid, params, seed=5)
     prob = orc.Problem(grid, params)
     tau = 0.25 * orc.dt(prob, X0)
     for alpha in ((0, 2) if ndim == 2 else (0, 1, 2)):
         for direction in (1, -1):
             ref = orc.sweep(prob, X0, alpha, tau, direction)
+            assert _tvd_active_fraction(orc, grid, params, X0, alpha, tau, direction, ref) >= 0.5
             s = _solver(gpu, grid, params, X0)
             s.debug_set_chunk(chunk)
             s.sweep(alpha, direction, tau)
@@ -123,6 +148,8 @@ def test_c1_one_step(gpu, orc, c1):
     # field-max norm: rho and E meet the tolerance outright; the momenta (max ~8e-4 here) are bounded by
     # the conditioning of the step, measured on the oracle itself
     fm = rel_err(X, c1["ref1"])
+    print("C1, 1 step: parity_err", parity_err(c1["grid"], c1["params"], X, c1["ref1"]), "field-max", fm,
+          "oracle 1-ulp conditioning", c1["cond1"])
     assert fm[0] <= TOL_1STEP and fm[-1] <= TOL_1STEP
     assert np.all(fm <= np.maximum(TOL_1STEP, COND_FACTOR * c1["cond1"])), (fm, c1["cond1"])
 
@@ -133,6 +160,8 @@ def test_c1_100_steps_and_diagnostics(gpu, orc, c1):
     X = s.state()
     assert parity_err(c1["grid"], c1["params"], X, c1["ref100"]).max() <= TOL_100STEP
     fm = rel_err(X, c1["ref100"])
+    print("C1, 100 steps: parity_err", parity_err(c1["grid"], c1["params"], X, c1["ref100"]), "field-max", fm,
+          "oracle 1-ulp conditioning", c1["cond100"])
     assert np.all(fm <= np.maximum(TOL_100STEP, COND_FACTOR * c1["cond100"])), (fm, c1["cond100"])
     d, Tp, rp, pp = s.diagnostics()
     assert d["step"] == c1["steps"]
