@@ -46,6 +46,7 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
+    ap.add_argument("--no-2d", action="store_true", help="skip the extra 2-D roofline leg (C3 at its 200 steps) of the default C5 run")
     ap.add_argument("--e2e-steps", type=int, default=3)
     return ap.parse_args()
 
@@ -191,14 +192,15 @@ def kernel_names(ndim, nx=0):
 
 
 def ncu_counters(name: str, kernel_key: str):
-    """(DRAM bytes, fp64 thread instructions) per launch of a kernel from the committed ncu --set full
-    capture (profiles/traffic.json, written from profiles/*_ncu_full.txt), or (None, None)."""
+    """(DRAM bytes, fp64 thread instructions) per launch of ONE kernel instance -- operator and direction, e.g.
+    "Lx-" (the dir -1 x-sweep is the instance that carries the fused CFL reduction) -- from the committed
+    ncu --set full capture (profiles/traffic.json, copied from profiles/*_ncu_full.txt), or (None, None)."""
     path = os.path.join(ROOT, "profiles", "traffic.json")
     if not os.path.exists(path):
         return None, None
     try:
         with open(path) as f:
-            rec = json.load(f).get(name, {}).get(kernel_key[:2], {})
+            rec = json.load(f).get(name, {}).get(kernel_key, {})
         return rec.get("dram_bytes"), rec.get("fp64_thread_insts")
     except Exception:
         return None, None
@@ -218,6 +220,78 @@ def max_over_ranks(x: float, world: int, device: str) -> float:
 def job_value(world: int, cells_per_rank: int, steps: int, ms: float) -> float:
     """Whole-job cell-updates/s: every rank advanced its own replica `steps` steps in `ms` milliseconds."""
     return world * cells_per_rank * steps / (ms * 1e-3)
+
+
+def roofline_of(name, grid, per_kernel, ms, steps, sm_mhz):
+    """The `roofline` object of one timed run: the slowest operator kernel against the measured HBM peak, the
+    whole step, every kernel's share, and the fp64-pipe view of each kernel instance from the committed ncu capture."""
+    nf, N = inputs.num_fields(grid), inputs.num_nodes(grid)
+    peak, peak_src = measured_peaks()
+    alg_bytes = 2 * nf * 8 * N                                       # read nf + write nf doubles per node per operator
+    names = kernel_names(grid["ndim"], grid["nx"])
+    fp64_peak = 148 * 64 * (sm_mhz or 1965) * 1e6                    # fp64 instructions/s: 64 lanes per SM per clock
+    kernels = {}
+    for k, (ms_sum, cnt) in per_kernel.items():
+        avg = ms_sum / cnt
+        traffic, insts = ncu_counters(name, k)
+        kernels[names[k]] = {"avg_ms": avg, "launches": cnt, "share_of_step": ms_sum / ms,
+                             "achieved_GBps": alg_bytes / (avg * 1e-3) / 1e9,
+                             "frac": alg_bytes / (avg * 1e-3) / 1e9 / peak, "traffic": traffic,
+                             "fp64_per_cell": insts / N if insts else None,
+                             "fp64_pipe_frac": insts / (avg * 1e-3) / fp64_peak if insts else None}
+    dom = max(per_kernel, key=lambda k: per_kernel[k][0] / per_kernel[k][1])
+    d = kernels[names[dom]]
+    fp64 = None
+    if d["fp64_per_cell"]:
+        fp64 = {"thread_insts_per_launch": d["fp64_per_cell"] * N, "per_cell": d["fp64_per_cell"],
+                "peak_Ginst_s": fp64_peak / 1e9, "frac": d["fp64_pipe_frac"],
+                "note": "co-bound: the fp64 pipe time of this kernel is close to its HBM time (DESIGN.md 8)"}
+    step_gbps = (4 if grid["ndim"] == 2 else 6) * alg_bytes * steps / (ms * 1e-3) / 1e9
+    return {"bound": "hbm", "kernel": names[dom], "achieved": d["achieved_GBps"], "peak": peak, "unit": "GB/s",
+            "frac": d["frac"], "traffic": d["traffic"], "fp64_pipe": fp64, "peak_source": peak_src,
+            "algorithmic_bytes_per_launch": alg_bytes, "algorithmic_bytes_per_cell_per_operator": 2 * nf * 8,
+            "whole_step_achieved_GBps": step_gbps, "whole_step_frac": step_gbps / peak, "kernels": kernels}
+
+
+def timed_run(binding, torch, name, steps, warmup, local, barrier, h_in=None):
+    """W warm-up steps, then exactly K timed steps of workload `name` with the state resident in HBM; CUDA events on
+    the library's stream around the region and around every operator launch; clocks sampled meanwhile."""
+    grid, params, _ = inputs.config(name)
+    if h_in is None:
+        h_in = torch.from_numpy(inputs.conduction_state(grid, params).reshape(-1))
+    solver = binding.MCTVD(grid, params, h_in, device=f"cuda:{local}")
+    solver.step(warmup)
+    barrier()
+    l0 = solver.launch_count()
+    solver.timing_enable(True)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local) as clocks:
+        barrier()
+        e0.record(solver.stream)
+        solver.step(steps)
+        e1.record(solver.stream)
+        barrier()
+    ms = e0.elapsed_time(e1)
+    launches = solver.launch_count() - l0
+    per_kernel = solver.timing_read()
+    solver.timing_enable(False)
+    return solver, grid, params, ms, launches, per_kernel, clocks.summary()
+
+
+def _oracle_worker(job):
+    name, steps, warmup, target = job
+    return time_oracle(name, steps, warmup, target)
+
+
+def oracle_all_cores(name, steps, warmup, target):
+    """The oracle as it stands (single-threaded C), one independent instance per host core on the same sample,
+    started together: whole-host cell-updates/s = instances x cells x steps / slowest instance's time."""
+    import multiprocessing as mp
+    cores = os.cpu_count() or 1
+    with mp.get_context("spawn").Pool(cores) as pool:
+        res = pool.map(_oracle_worker, [(name, steps, warmup, target)] * cores)
+    s_per_step = max(r[1] for r in res)
+    return cores * res[0][3] / s_per_step, cores, res[0][2], res[0][3], s_per_step
 
 
 def run_ours(args):
@@ -248,7 +322,6 @@ def run_ours(args):
     except Exception:
         h_out = torch.empty_like(h_in)
         pinned = False
-    solver = binding.MCTVD(grid, params, h_in, device=f"cuda:{local}")
 
     def barrier():
         if world > 1:
@@ -256,21 +329,8 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     # ---- device-resident throughput: W warm-up steps, then exactly K timed steps ------------------
-    solver.step(args.warmup)
-    barrier()
-    l0 = solver.launch_count()
-    solver.timing_enable(True)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    with ClockSampler(local) as clocks:
-        barrier()
-        e0.record(solver.stream)
-        solver.step(args.steps)
-        e1.record(solver.stream)
-        barrier()
-    ms = e0.elapsed_time(e1)
-    launches = solver.launch_count() - l0
-    per_kernel = solver.timing_read()
-    solver.timing_enable(False)
+    solver, grid, params, ms, launches, per_kernel, clock_sum = timed_run(binding, torch, name, args.steps, args.warmup,
+                                                                           local, barrier, h_in)
     dt_now = solver.dt()                                             # raises if the state went non-finite
     diag, *_ = solver.diagnostics()
     torch.cuda.synchronize()
@@ -299,38 +359,28 @@ def run_ours(args):
                "call": "mc_tvd_step_host(h_in, h_out, 1): H2D of the state, dt reduction, 1 step, D2H of the state",
                "host_memory": "pinned" if pinned else "pageable"}
     solver.close()
+    del solver, h_in, h_out
+    torch.cuda.empty_cache()
+
+    # ---- the other roofline case of north_star: the largest 2-D grid (C3) at the config's own step count ----
+    roofline_2d = None
+    if world == 1 and name == "C5" and not args.no_2d:
+        s2, g2, p2, ms2, l2, pk2, clk2 = timed_run(binding, torch, "C3", inputs.CONFIGS["C3"]["steps"], max(3, args.warmup),
+                                                    local, barrier)
+        dt2 = s2.dt()
+        s2.close()
+        del s2
+        torch.cuda.empty_cache()
+        st2 = inputs.CONFIGS["C3"]["steps"]
+        roofline_2d = {"config": workload_config("C3", g2, p2), "steps": st2, "ms_per_step": ms2 / st2,
+                       "value": inputs.num_nodes(g2) * st2 / (ms2 * 1e-3), "unit": UNIT, "gpu_launches": int(l2),
+                       "clocks": clk2, "roofline": roofline_of("C3", g2, pk2, ms2, st2, clk2.get("sm_mhz")),
+                       "state_check": {"dt": dt2}}
 
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
-
-    # ---- roofline of the dominant kernel ------------------------------------------------------------
-    peak, peak_src = measured_peaks()
-    alg_bytes = 2 * nf * 8 * N                                       # read nf + write nf doubles per node per operator
-    dom = max(per_kernel, key=lambda k: per_kernel[k][0])
-    dom_ms = per_kernel[dom][0] / per_kernel[dom][1]
-    achieved = alg_bytes / (dom_ms * 1e-3) / 1e9
-    KERNEL_NAMES = kernel_names(grid["ndim"], grid["nx"])
-    kernels = {KERNEL_NAMES[k]: {"avg_ms": v[0] / v[1], "launches": v[1], "share_of_step": v[0] / ms,
-                                 "achieved_GBps": alg_bytes / (v[0] / v[1] * 1e-3) / 1e9}
-               for k, v in per_kernel.items()}
-    step_gbps = (4 if grid["ndim"] == 2 else 6) * alg_bytes * args.steps / (ms * 1e-3) / 1e9
-    traffic, fp64_insts = ncu_counters(name, dom)
-    sm_mhz = clocks.summary().get("sm_mhz") or 1965
-    fp64_peak = 148 * 64 * sm_mhz * 1e6                               # DFMA/s: 64 fp64 lanes per SM per clock
-    fp64 = None
-    if fp64_insts:
-        fp64 = {"thread_insts_per_launch": fp64_insts, "per_cell": fp64_insts / N,
-                "achieved_Ginst_s": fp64_insts / (dom_ms * 1e-3) / 1e9, "peak_Ginst_s": fp64_peak / 1e9,
-                "frac": fp64_insts / (dom_ms * 1e-3) / fp64_peak,
-                "note": "co-bound: the fp64 pipe time of this kernel is close to its HBM time (DESIGN.md 7)"}
-    roofline = {"bound": "hbm", "kernel": KERNEL_NAMES[dom], "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": traffic, "fp64_pipe": fp64, "peak_source": peak_src,
-                "algorithmic_bytes_per_launch": alg_bytes,
-                "algorithmic_bytes_per_cell_per_operator": 2 * nf * 8,
-                "whole_step_achieved_GBps": step_gbps, "whole_step_frac": step_gbps / peak,
-                "kernels": kernels}
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -338,19 +388,24 @@ def run_ours(args):
         "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic (seeded hydrostatic conduction state + T noise, DESIGN.md input recipe)",
         "config": workload_config(name, grid, params),
-        "clocks": clocks.summary(), "gpu_launches": int(launches),
-        "roofline": roofline,
+        "clocks": clock_sum, "gpu_launches": int(launches),
+        "roofline": roofline_of(name, grid, per_kernel, ms, args.steps, clock_sum.get("sm_mhz")),
         "diagnostics_ms": diag_ms,
         "state_check": {"dt": dt_now, "nu_bar": diag["nu_bar"], "min_rho": diag["min_rho"], "min_T": diag["min_T"],
                         "steps_taken": diag["step"]},
     }
+    if roofline_2d is not None:
+        line["roofline_2d"] = roofline_2d
     if e2e is not None:
         line["e2e"] = e2e
     if world == 1 and not args.no_cpu_baseline:
-        target = ORACLE_RATE_EST * 8.0                                # ~8 s per oracle step, 1 warm-up + 2 timed
+        target = ORACLE_RATE_EST * 6.0                                # ~6 s per oracle step, 1 warm-up + 2 timed
         v, s_per_step, desc, cells = time_oracle(name, 2, 1, target)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
                                 "sample": f"{desc}; 2 timed steps of {cells} cells after 1 warm-up, {s_per_step:.1f} s/step"}
+        va, cores, desc, cells, sps = oracle_all_cores(name, 2, 1, target)
+        line["cpu_baseline_all_cores"] = {"value": va, "unit": UNIT, "cores": cores, "kind": "oracle, one independent instance per core",
+                                          "sample": f"{cores} x ({desc}); 2 timed steps after 1 warm-up, slowest instance {sps:.1f} s/step"}
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()

@@ -73,6 +73,21 @@ typedef struct {
     double max_mach, min_rho, min_T;
 } mc_tvd_diag;
 
+/* Running time averages <.>_t of the diagnostics (the paper reports Nu, Nu_conv, Nu_K of Eq. 22 as <.>_{V,t},
+ * Nu_{z=0,1} of Eq. 23 from <T_sa>_{A,t}, Re of Eq. 26 as <sqrt(<u^2>_V)>_t, and averages them over 50 time units
+ * of the steady state).  Sample k is the instantaneous diagnostic of the state at
+ * time t_k weighted with w_k = t_k - t_{k-1} (the time since the previous sample, or since the reset for the first
+ * one): <f>_t = sum_k w_k f_k / sum_k w_k.  The plate Nusselt numbers are LINEAR in the plane means of T, so their
+ * averages equal Eq. 23 applied to <T_sa>_{A,t}. */
+typedef struct {
+    double t_begin, t_end;                 /* averaged time span: reset time, time of the last sample */
+    double weight; long long samples;      /* sum of the weights (= t_end - t_begin) and number of samples */
+    double nu_bottom, nu_top, nu_bar;      /* Eqs. 23-24, time averaged */
+    double nu_bulk, nu_conv, nu_K;         /* Eq. 22, <.>_{V,t} */
+    double re, u_rms;                      /* Eq. 26 */
+    double nu_bar_sq, re_sq;               /* <Nu_bar^2>_t, <Re^2>_t: the +- the paper quotes is sqrt(<f^2> - <f>^2) */
+} mc_tvd_stats;
+
 typedef struct mc_tvd_state mc_tvd_state;  /* opaque host-side handle */
 
 /* Bytes of device workspace mc_tvd_init needs for this problem: the second (ping-pong) state
@@ -126,6 +141,17 @@ int mc_tvd_dt(mc_tvd_state *s, double *dt_host);
  * Synchronises the stream. */
 int mc_tvd_diagnostics(mc_tvd_state *s, mc_tvd_diag *out, double *T_prof, double *rho_prof,
                        double *p_prof);
+
+/* Time averages.  mc_tvd_stats_reset zeroes the device-resident accumulators and starts the averaging
+ * span at the current simulated time.  mc_tvd_step_stats advances n_steps steps like mc_tvd_step and, after every
+ * `every`-th of them (counted since the reset), evaluates the diagnostics of Eqs. 22-26 on the device and adds them
+ * to the accumulators with the weight stated at mc_tvd_stats; asynchronous, never synchronises.  mc_tvd_stats_read
+ * forms the averages on the device, copies them into a HOST struct and the time-averaged horizontal means <T>_{A,t},
+ * <rho>_{A,t}, <p>_{A,t} into HOST arrays of nz doubles (each may be NULL), and synchronises the stream.  With no
+ * sample yet it returns MC_TVD_EINVAL. */
+int mc_tvd_stats_reset(mc_tvd_state *s);
+int mc_tvd_step_stats(mc_tvd_state *s, int n_steps, int every);
+int mc_tvd_stats_read(mc_tvd_state *s, mc_tvd_stats *out, double *T_prof, double *rho_prof, double *p_prof);
 
 /* Number of kernel launches this handle has enqueued so far (for bench.py's gpu_launches). */
 long long mc_tvd_launch_count(const mc_tvd_state *s);

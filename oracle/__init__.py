@@ -57,6 +57,13 @@ class _Diag(C.Structure):
                 ("max_mach", C.c_double), ("min_rho", C.c_double), ("min_T", C.c_double)]
 
 
+class _Stats(C.Structure):
+    _fields_ = [("t_begin", C.c_double), ("t_end", C.c_double), ("weight", C.c_double), ("samples", C.c_longlong),
+                ("nu_bottom", C.c_double), ("nu_top", C.c_double), ("nu_bar", C.c_double),
+                ("nu_bulk", C.c_double), ("nu_conv", C.c_double), ("nu_K", C.c_double),
+                ("re", C.c_double), ("u_rms", C.c_double), ("nu_bar_sq", C.c_double), ("re_sq", C.c_double)]
+
+
 _lib = None
 
 
@@ -75,6 +82,9 @@ def lib():
         L.orc_step.argtypes = [C.POINTER(_Grid), C.POINTER(_Params), dp, C.c_int, dp, dp, dp]
         L.orc_diagnostics.restype = C.c_int
         L.orc_diagnostics.argtypes = [C.POINTER(_Grid), C.POINTER(_Params), dp, C.POINTER(_Diag), dp, dp, dp]
+        L.orc_step_stats.restype = C.c_int
+        L.orc_step_stats.argtypes = [C.POINTER(_Grid), C.POINTER(_Params), dp, C.c_int, C.c_int, dp,
+                                     C.POINTER(_Stats), dp, dp, dp]
         L.orc_coefficients.restype = C.c_int
         L.orc_coefficients.argtypes = [C.POINTER(_Grid), C.POINTER(_Params), dp]
         _lib = L
@@ -168,6 +178,25 @@ def diagnostics(prob: Problem, X: np.ndarray):
     if rc:
         raise ValueError(f"orc_diagnostics failed: {rc}")
     return {n: getattr(d, n) for n, _ in _Diag._fields_}, Tp, rp, pp
+
+
+def step_stats(prob: Problem, X: np.ndarray, n_steps: int, every: int = 1, dt_in=None):
+    """Advance a copy of X by n_steps, sampling the diagnostics after every `every`-th step; returns
+    (X_new, dict of time averages, <T>_{A,t}, <rho>_{A,t}, <p>_{A,t})."""
+    X = _check(prob, X).copy()
+    g, p = prob.c_grid(), prob.c_params()
+    nz = int(prob.grid["nz"])
+    din = None
+    if dt_in is not None:
+        din = np.ascontiguousarray(dt_in, dtype=np.float64)
+        assert din.size >= n_steps
+    st = _Stats()
+    Tp, rp, pp = np.zeros(nz), np.zeros(nz), np.zeros(nz)
+    rc = lib().orc_step_stats(C.byref(g), C.byref(p), _dp(X), n_steps, every, _dp(din), C.byref(st), _dp(Tp),
+                              _dp(rp), _dp(pp))
+    if rc:
+        raise ValueError(f"orc_step_stats failed: {rc}")
+    return X, {n: getattr(st, n) for n, _ in _Stats._fields_}, Tp, rp, pp
 
 
 def coefficients(prob: Problem) -> dict:

@@ -487,6 +487,45 @@ int orc_diagnostics(const orc_grid *g, const orc_params *p, const double *X, orc
     return 0;
 }
 
+/* Time averages (PAPER.md:218 "<.>_{V,t}", :222 "<.>_{A,t}", :236, :355): step, sample, weight with the time
+ * elapsed since the previous sample, divide by the total weight at the end.  A composition of orc_step and
+ * orc_diagnostics; no new arithmetic of the scheme. */
+int orc_step_stats(const orc_grid *g, const orc_params *p, double *X, int n_steps, int every,
+                   const double *dt_in, orc_stats *out, double *T_prof, double *rho_prof, double *p_prof)
+{
+    if (!g || !p || !X || !out || n_steps < 0 || every < 1) return -1;
+    int nz = g->nz;
+    double *aT = arr(nz), *ar = arr(nz), *ap = arr(nz), *iT = arr(nz), *ir = arr(nz), *ip = arr(nz);
+    double sum[10] = { 0 }, weight = 0.0, t = 0.0, t_last = 0.0;
+    long long samples = 0;
+    for (int s = 0; s < n_steps; ++s) {
+        int rc = orc_step(g, p, X, 1, dt_in ? dt_in + s : NULL, NULL, &t);
+        if (rc) return rc;
+        if ((s + 1) % every) continue;
+        orc_diag d;
+        orc_diagnostics(g, p, X, &d, iT, ir, ip);
+        double w = t - t_last;
+        double f[10] = { d.nu_bottom, d.nu_top, d.nu_bar, d.nu_bulk, d.nu_conv, d.nu_K, d.re, d.u_rms,
+                         d.nu_bar * d.nu_bar, d.re * d.re };
+        for (int i = 0; i < 10; ++i) sum[i] += w * f[i];
+        for (int k = 0; k < nz; ++k) { aT[k] += w * iT[k]; ar[k] += w * ir[k]; ap[k] += w * ip[k]; }
+        weight += w; t_last = t; samples += 1;
+    }
+    memset(out, 0, sizeof(*out));
+    out->t_begin = 0.0; out->t_end = t_last; out->weight = weight; out->samples = samples;
+    if (samples > 0) {
+        double *o = &out->nu_bottom;
+        for (int i = 0; i < 10; ++i) o[i] = sum[i] / weight;
+        for (int k = 0; k < nz; ++k) {
+            if (T_prof) T_prof[k] = aT[k] / weight;
+            if (rho_prof) rho_prof[k] = ar[k] / weight;
+            if (p_prof) p_prof[k] = ap[k] / weight;
+        }
+    }
+    free(aT); free(ar); free(ap); free(iT); free(ir); free(ip);
+    return 0;
+}
+
 int orc_coefficients(const orc_grid *g, const orc_params *p, double *o)
 {
     ctx c;

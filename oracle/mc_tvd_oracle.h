@@ -83,6 +83,19 @@ int orc_step(const orc_grid *g, const orc_params *p, double *X, int n_steps,
 int orc_diagnostics(const orc_grid *g, const orc_params *p, const double *X, orc_diag *out,
                     double *T_prof, double *rho_prof, double *p_prof);
 
+/* Time averages of the diagnostics (twin of mc_tvd_step_stats / mc_tvd_stats_read; the paper averages Nu and Re
+ * over 50 time units of the steady state): n_steps steps of Eq. 30; after every `every`-th
+ * step the instantaneous diagnostics f_k of the state at time t_k enter with the weight w_k = t_k - t_{k-1} (time
+ * since the previous sample, or since the start for the first one); <f>_t = sum w_k f_k / sum w_k.  X is advanced
+ * in place.  dt_in as in orc_step.  Profiles: nz doubles each, may be NULL. */
+typedef struct {
+    double t_begin, t_end, weight; long long samples;
+    double nu_bottom, nu_top, nu_bar, nu_bulk, nu_conv, nu_K, re, u_rms;
+    double nu_bar_sq, re_sq;                 /* <Nu_bar^2>_t, <Re^2>_t */
+} orc_stats;
+int orc_step_stats(const orc_grid *g, const orc_params *p, double *X, int n_steps, int every,
+                   const double *dt_in, orc_stats *out, double *T_prof, double *rho_prof, double *p_prof);
+
 /* Derived coefficients, in this order: R, c_v, g, mu, K, lambda, dx, dy, dz (9 doubles). */
 int orc_coefficients(const orc_grid *g, const orc_params *p, double *out9);
 

@@ -40,6 +40,13 @@ class Diag(C.Structure):            # mc_tvd_diag
                 ("max_mach", C.c_double), ("min_rho", C.c_double), ("min_T", C.c_double)]
 
 
+class Stats(C.Structure):           # mc_tvd_stats
+    _fields_ = [("t_begin", C.c_double), ("t_end", C.c_double), ("weight", C.c_double), ("samples", C.c_longlong),
+                ("nu_bottom", C.c_double), ("nu_top", C.c_double), ("nu_bar", C.c_double),
+                ("nu_bulk", C.c_double), ("nu_conv", C.c_double), ("nu_K", C.c_double),
+                ("re", C.c_double), ("u_rms", C.c_double), ("nu_bar_sq", C.c_double), ("re_sq", C.c_double)]
+
+
 # every symbol include/mc_tvd.h declares: name -> (restype, argtypes)
 SYMBOLS = {
     "mc_tvd_workspace_bytes": (C.c_size_t, [C.POINTER(Grid), C.POINTER(Params)]),
@@ -52,6 +59,9 @@ SYMBOLS = {
     "mc_tvd_step_host": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]),
     "mc_tvd_dt": (C.c_int, [C.c_void_p, _DP]),
     "mc_tvd_diagnostics": (C.c_int, [C.c_void_p, C.POINTER(Diag), _DP, _DP, _DP]),
+    "mc_tvd_stats_reset": (C.c_int, [C.c_void_p]),
+    "mc_tvd_step_stats": (C.c_int, [C.c_void_p, C.c_int, C.c_int]),
+    "mc_tvd_stats_read": (C.c_int, [C.c_void_p, C.POINTER(Stats), _DP, _DP, _DP]),
     "mc_tvd_launch_count": (C.c_longlong, [C.c_void_p]),
     "mc_tvd_timing_enable": (C.c_int, [C.c_void_p, C.c_int]),
     "mc_tvd_timing_read": (C.c_int, [C.c_void_p, _DP, C.POINTER(C.c_longlong)]),
@@ -192,6 +202,20 @@ class MCTVD:
         self._check(self.lib.mc_tvd_diagnostics(self._h, C.byref(d), Tp.ctypes.data_as(_DP),
                                                 rp.ctypes.data_as(_DP), pp.ctypes.data_as(_DP)))
         return {n: getattr(d, n) for n, _ in Diag._fields_}, Tp, rp, pp
+
+    def stats_reset(self):
+        self._check(self.lib.mc_tvd_stats_reset(self._h))
+
+    def step_stats(self, n_steps: int, every: int = 1):
+        self._check(self.lib.mc_tvd_step_stats(self._h, int(n_steps), int(every)))
+
+    def stats_read(self):
+        """Returns (dict of time averages, <T>_{A,t}, <rho>_{A,t}, <p>_{A,t}) -- same shape as the oracle's."""
+        st = Stats()
+        Tp, rp, pp = np.zeros(self.nz), np.zeros(self.nz), np.zeros(self.nz)
+        self._check(self.lib.mc_tvd_stats_read(self._h, C.byref(st), Tp.ctypes.data_as(_DP), rp.ctypes.data_as(_DP),
+                                               pp.ctypes.data_as(_DP)))
+        return {n: getattr(st, n) for n, _ in Stats._fields_}, Tp, rp, pp
 
     def launch_count(self) -> int:
         return int(self.lib.mc_tvd_launch_count(self._h))

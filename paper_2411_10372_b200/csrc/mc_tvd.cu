@@ -82,7 +82,7 @@ constexpr int LANE_MINB_2D = MC_LANE_MINB_2D;
 constexpr int DIAG_MAX_BLOCKS = 16;    // blocks per plane in the diagnostics pass (the finish kernel walks them)
 
 struct Layout {                        // byte offsets inside the workspace
-    size_t Y, scalars, partial, ext, plane_sums, plane_ext, diag_out, total;
+    size_t Y, scalars, partial, ext, plane_sums, plane_ext, diag_out, stats, stats_out, total;
     int diag_blocks;
 };
 
@@ -98,7 +98,8 @@ struct mc_tvd_state {
     bool walls;
     double *X, *Y;
     mc::Scalars *S;
-    double *partial, *ext, *plane_sums, *plane_ext, *diag_out;
+    double *partial, *ext, *plane_sums, *plane_ext, *diag_out, *stats, *stats_out;
+    long long stat_steps;              // steps taken through mc_tvd_step_stats since the last reset
     int diag_blocks;
     cudaStream_t stream;
     long long launches;
@@ -159,6 +160,8 @@ Layout make_layout(const mc_tvd_grid *g)
     L.plane_sums = o; o = align_up(o + (size_t)g->nz * mc::DQ_MAXQ * sizeof(double), 256);
     L.plane_ext = o;  o = align_up(o + (size_t)g->nz * 3 * sizeof(double), 256);
     L.diag_out = o;   o = align_up(o + (19 + 3 * (size_t)g->nz) * sizeof(double), 256);
+    L.stats = o;      o = align_up(o + (mc::ST_HEAD + 3 * (size_t)g->nz) * sizeof(double), 256);
+    L.stats_out = o;  o = align_up(o + (4 + mc::ST_NSUM + 3 * (size_t)g->nz) * sizeof(double), 256);
     L.total = o;
     return L;
 }
@@ -493,6 +496,8 @@ int mc_tvd_init(const mc_tvd_grid *grid, const mc_tvd_params *params, double *d_
     s->plane_sums = (double *)(w + L.plane_sums);
     s->plane_ext = (double *)(w + L.plane_ext);
     s->diag_out = (double *)(w + L.diag_out);
+    s->stats = (double *)(w + L.stats);
+    s->stats_out = (double *)(w + L.stats_out);
     s->diag_blocks = L.diag_blocks;
     s->stream = (cudaStream_t)cuda_stream;
     s->chunk_override = 0;
@@ -521,6 +526,7 @@ int mc_tvd_init(const mc_tvd_grid *grid, const mc_tvd_params *params, double *d_
     rc = cuda_check(cudaMemcpyAsync(s->S, &h, sizeof(h), cudaMemcpyHostToDevice, s->stream), "scalar upload");
     if (rc == MC_TVD_OK) rc = cuda_check(cudaStreamSynchronize(s->stream), "scalar upload sync");   // h is on the stack
     if (rc == MC_TVD_OK) rc = enqueue_initial_dt(s);
+    if (rc == MC_TVD_OK) rc = mc_tvd_stats_reset(s);
     if (rc != MC_TVD_OK) { delete s; return rc; }
     *out = s;
     return MC_TVD_OK;
@@ -594,6 +600,7 @@ int mc_tvd_step_host(mc_tvd_state *s, const double *h_in, double *h_out, int n_s
     rc = cuda_check(cudaMemcpyAsync(s->S, &h, sizeof(h), cudaMemcpyHostToDevice, s->stream), "scalar upload");
     if (rc == MC_TVD_OK) rc = cuda_check(cudaStreamSynchronize(s->stream), "upload sync");      // h is on the stack
     if (rc == MC_TVD_OK) rc = enqueue_initial_dt(s);
+    if (rc == MC_TVD_OK) rc = mc_tvd_stats_reset(s);                 // time restarts at zero: so does the averaging span
     if (rc == MC_TVD_OK) rc = mc_tvd_step(s, n_steps);
     if (rc == MC_TVD_OK) rc = cuda_check(cudaMemcpyAsync(h_out, s->X, bytes, cudaMemcpyDeviceToHost, s->stream), "state download");
     if (rc == MC_TVD_OK) rc = cuda_check(cudaStreamSynchronize(s->stream), "download sync");
@@ -611,10 +618,12 @@ int mc_tvd_dt(mc_tvd_state *s, double *dt_host)
     return MC_TVD_OK;
 }
 
-int mc_tvd_diagnostics(mc_tvd_state *s, mc_tvd_diag *out, double *T_prof, double *rho_prof, double *p_prof)
+}  // extern "C"
+
+namespace {
+// Enqueue the three diagnostics kernels (Eqs. 22-26): the result block lands in s->diag_out on the device.
+int enqueue_diagnostics(mc_tvd_state *s)
 {
-    if (!s || !out) return fail(MC_TVD_EINVAL, "bad handle or out");
-    static_assert(sizeof(mc_tvd_diag) == 19 * sizeof(double), "mc_tvd_diag layout");
     mc::PointArgs P = point_args(s);
     dim3 grid((unsigned)s->diag_blocks, (unsigned)s->grid.nz, 1);
     if (s->nd == 2) { auto kfn = mc::k_plane_partials<2>; MC_LAUNCH(kfn, grid, mc::DIAG_THREADS, 0, s->stream, P, s->partial, s->ext); }
@@ -629,7 +638,17 @@ int mc_tvd_diagnostics(mc_tvd_state *s, mc_tvd_diag *out, double *T_prof, double
     { auto kfn = mc::k_diag_planes; MC_LAUNCH(kfn, (unsigned)((s->grid.nz + 3) / 4), 128, 0, s->stream, G, s->plane_ext); }
     { auto kfn = mc::k_diag_finish; MC_LAUNCH(kfn, 1, mc::DIAG_THREADS, 0, s->stream, G, s->plane_ext); }
     s->launches += 3;
-    int rc = cuda_check(cudaGetLastError(), "diagnostics launch");
+    return cuda_check(cudaGetLastError(), "diagnostics launch");
+}
+}  // namespace
+
+extern "C" {
+
+int mc_tvd_diagnostics(mc_tvd_state *s, mc_tvd_diag *out, double *T_prof, double *rho_prof, double *p_prof)
+{
+    if (!s || !out) return fail(MC_TVD_EINVAL, "bad handle or out");
+    static_assert(sizeof(mc_tvd_diag) == 19 * sizeof(double), "mc_tvd_diag layout");
+    int rc = enqueue_diagnostics(s);
     if (rc != MC_TVD_OK) return rc;
     const size_t nz = (size_t)s->grid.nz;
     double *h = (double *)malloc((19 + 3 * nz) * sizeof(double));
@@ -642,6 +661,58 @@ int mc_tvd_diagnostics(mc_tvd_state *s, mc_tvd_diag *out, double *T_prof, double
         if (T_prof) memcpy(T_prof, h + 19, nz * sizeof(double));
         if (rho_prof) memcpy(rho_prof, h + 19 + nz, nz * sizeof(double));
         if (p_prof) memcpy(p_prof, h + 19 + 2 * nz, nz * sizeof(double));
+    }
+    free(h);
+    return rc;
+}
+
+int mc_tvd_stats_reset(mc_tvd_state *s)
+{
+    if (!s) return fail(MC_TVD_EINVAL, "bad handle");
+    { auto kfn = mc::k_stats_reset; MC_LAUNCH(kfn, 1, 256, 0, s->stream, s->stats, s->S, s->grid.nz); }
+    s->launches += 1;
+    s->stat_steps = 0;
+    return cuda_check(cudaGetLastError(), "stats reset launch");
+}
+
+int mc_tvd_step_stats(mc_tvd_state *s, int n_steps, int every)
+{
+    if (!s || n_steps < 0 || every < 1) return fail(MC_TVD_EINVAL, "bad handle, n_steps or every");
+    for (int it = 0; it < n_steps; ++it) {
+        int rc = mc_tvd_step(s, 1);
+        if (rc != MC_TVD_OK) return rc;
+        s->stat_steps += 1;
+        if (s->stat_steps % every) continue;
+        rc = enqueue_diagnostics(s);
+        if (rc != MC_TVD_OK) return rc;
+        { auto kfn = mc::k_stats_accumulate; MC_LAUNCH(kfn, 1, 256, 0, s->stream, s->stats, s->diag_out, s->S, s->grid.nz); }
+        s->launches += 1;
+        rc = cuda_check(cudaGetLastError(), "stats accumulate launch");
+        if (rc != MC_TVD_OK) return rc;
+    }
+    return MC_TVD_OK;
+}
+
+int mc_tvd_stats_read(mc_tvd_state *s, mc_tvd_stats *out, double *T_prof, double *rho_prof, double *p_prof)
+{
+    if (!s || !out) return fail(MC_TVD_EINVAL, "bad handle or out");
+    static_assert(sizeof(mc_tvd_stats) == (4 + mc::ST_NSUM) * sizeof(double), "mc_tvd_stats layout");
+    const size_t nz = (size_t)s->grid.nz, n = 4 + mc::ST_NSUM + 3 * nz;
+    { auto kfn = mc::k_stats_finish; MC_LAUNCH(kfn, 1, 256, 0, s->stream, s->stats, s->stats_out, s->grid.nz); }
+    s->launches += 1;
+    int rc = cuda_check(cudaGetLastError(), "stats finish launch");
+    if (rc != MC_TVD_OK) return rc;
+    double *h = (double *)malloc(n * sizeof(double));
+    if (!h) return fail(MC_TVD_ENOMEM, "host allocation failed");
+    rc = cuda_check(cudaMemcpyAsync(h, s->stats_out, n * sizeof(double), cudaMemcpyDeviceToHost, s->stream), "stats copy");
+    if (rc == MC_TVD_OK) rc = cuda_check(cudaStreamSynchronize(s->stream), "stats sync");
+    if (rc == MC_TVD_OK && !(h[3] >= 1.0)) rc = fail(MC_TVD_EINVAL, "no sample has been accumulated since the last mc_tvd_stats_reset");
+    if (rc == MC_TVD_OK) {
+        out->t_begin = h[0]; out->t_end = h[1]; out->weight = h[2]; out->samples = (long long)h[3];
+        memcpy(&out->nu_bottom, h + 4, mc::ST_NSUM * sizeof(double));
+        if (T_prof) memcpy(T_prof, h + 4 + mc::ST_NSUM, nz * sizeof(double));
+        if (rho_prof) memcpy(rho_prof, h + 4 + mc::ST_NSUM + nz, nz * sizeof(double));
+        if (p_prof) memcpy(p_prof, h + 4 + mc::ST_NSUM + 2 * nz, nz * sizeof(double));
     }
     free(h);
     return rc;

@@ -273,4 +273,41 @@ MC_KERNEL void k_diag_finish(DiagArgs G, const double *plane_ext)
     o[16] = sqrt(sh[NV][0]); o[17] = sh[NV + 1][0]; o[18] = sh[NV + 2][0];   // the partials carry Mach^2
 }
 
+// ---------------------------------------------------------------------------------------------
+// running time averages of the diagnostics (include/mc_tvd.h mc_tvd_stats)
+// ---------------------------------------------------------------------------------------------
+// Device block: [0] t_begin, [1] t_last, [2] weight, [3] samples, [4..13] weighted sums in the order of
+// mc_tvd_stats from nu_bottom on, [16 .. 16 + 3 nz) weighted profile sums (T, rho, p).
+constexpr int ST_HEAD = 16, ST_NSUM = 10;
+
+MC_KERNEL void k_stats_reset(double *st, const Scalars *S, int nz)
+{
+    for (int i = threadIdx.x; i < ST_HEAD + 3 * nz; i += blockDim.x) st[i] = 0.0;
+    __syncthreads();
+    if (threadIdx.x == 0) { st[0] = S->time; st[1] = S->time; }
+}
+
+// Add the diagnostics block `diag` (layout of k_diag_finish: 19 scalars, then the T, rho, p profiles) with the weight
+// w = time - t_last.
+MC_KERNEL void k_stats_accumulate(double *st, const double *diag, const Scalars *S, int nz)
+{
+    const double w = S->time - st[1];
+    // mc_tvd_diag order: 3 nu_bottom, 4 nu_top, 5 nu_bar, 6 nu_bulk, 7 nu_conv, 8 nu_K, 9 re, 10 u_rms
+    if (threadIdx.x < 8) st[4 + threadIdx.x] += w * diag[3 + threadIdx.x];
+    if (threadIdx.x == 8) st[12] += w * (diag[5] * diag[5]);
+    if (threadIdx.x == 9) st[13] += w * (diag[9] * diag[9]);
+    for (int i = threadIdx.x; i < 3 * nz; i += blockDim.x) st[ST_HEAD + i] += w * diag[19 + i];
+    __syncthreads();
+    if (threadIdx.x == 0) { st[2] += w; st[3] += 1.0; st[1] = S->time; }
+}
+
+// out: 4 header values (t_begin, t_end, weight, samples), the 10 averages, then the 3 nz averaged profile values
+MC_KERNEL void k_stats_finish(const double *st, double *out, int nz)
+{
+    const double iw = 1.0 / st[2];
+    if (threadIdx.x == 0) { out[0] = st[0]; out[1] = st[1]; out[2] = st[2]; out[3] = st[3]; }
+    if (threadIdx.x < ST_NSUM) out[4 + threadIdx.x] = st[4 + threadIdx.x] * iw;
+    for (int i = threadIdx.x; i < 3 * nz; i += blockDim.x) out[4 + ST_NSUM + i] = st[ST_HEAD + i] * iw;
+}
+
 }  // namespace mc

@@ -1,0 +1,93 @@
+"""Physical validation runs against the paper's Tables 1 and 2.
+
+    python -m paper_2411_10372_b200.validate [--case table2-1] [--out results.json]
+
+Runs the CUDA library (no oracle, no CPU path) from the seeded conduction-plus-noise state to a statistically
+steady state on a UNIFORM grid, then averages Nu_bar (Eq. 24) and Re (Eq. 26) in time with the device-side
+accumulators (mc_tvd_step_stats), as the paper does over 50 time units, and prints them next to
+the values the paper lists.  The paper's own grids for these runs are not stated and its z grid is stretched
+(PAPER.md:249-251); agreement within the ~3 % the paper itself reports against the earlier codes is the bar.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import time
+
+from . import inputs
+
+# PAPER.md:331-345.  `paper` = (Nu, +-, Re, +-) of "our simulations"; `ref` = the earlier code's (Nu, Re).
+CASES = {
+    "table2-1": dict(ndim=2, Ra=1e4, D=0.49, Gamma=2.0, gamma=5.0 / 3.0, Pr=0.7, eps=0.1, nx=256, ny=1, nz=129,
+                     t_spin=150.0, t_avg=50.0, paper=(2.175, 0.005, 26.98, 0.05), ref=(2.1, 26.3), cite="Table 2 case 1"),
+    "table2-1-fine": dict(ndim=2, Ra=1e4, D=0.49, Gamma=2.0, gamma=5.0 / 3.0, Pr=0.7, eps=0.1, nx=512, ny=1, nz=257,
+                          t_spin=150.0, t_avg=50.0, paper=(2.175, 0.005, 26.98, 0.05), ref=(2.1, 26.3),
+                          cite="Table 2 case 1, grid doubled"),
+    "table2-2": dict(ndim=2, Ra=1e5, D=0.49, Gamma=2.0, gamma=5.0 / 3.0, Pr=0.7, eps=0.1, nx=384, ny=1, nz=193,
+                     t_spin=150.0, t_avg=50.0, paper=(4.0, 0.1, 100.0, 3.0), ref=(3.9, 102.0), cite="Table 2 case 2"),
+    "table2-3": dict(ndim=2, Ra=1e6, D=0.49, Gamma=2.0, gamma=5.0 / 3.0, Pr=0.7, eps=0.1, nx=768, ny=1, nz=385,
+                     t_spin=150.0, t_avg=50.0, paper=(7.3, 0.2, 330.0, 7.0), ref=(7.1, 322.0), cite="Table 2 case 3"),
+    "table1-3": dict(ndim=3, Ra=1e6, D=0.5, Gamma=4.0, gamma=1.4, Pr=0.7, eps=0.1, nx=384, ny=384, nz=129,
+                     t_spin=80.0, t_avg=50.0, paper=(6.89, 0.05, 406.0, 3.0), ref=(6.93, 407.0), cite="Table 1 case 3"),
+}
+
+
+def run_case(name: str, device: str = "cuda:0", chunk: int = 2000, every: int = 10, verbose: bool = True) -> dict:
+    from . import binding
+    c = CASES[name]
+    grid = inputs.make_grid(c["ndim"], c["nx"], c["nz"], c["ny"], lx=c["Gamma"], ly=c["Gamma"], lz=1.0)
+    params = inputs.make_params(gamma=c["gamma"], Pr=c["Pr"], Ra=c["Ra"], eps=c["eps"], D=c["D"], cfl=0.5)
+    X0 = inputs.conduction_state(grid, params, amplitude=1e-3)
+    s = binding.MCTVD(grid, params, X0, device=device)
+    t0 = time.perf_counter()
+    t, series = 0.0, []
+    while t < c["t_spin"]:
+        s.step(chunk)
+        d, *_ = s.diagnostics()
+        t = d["time"]
+        series.append((t, d["nu_bar"], d["re"]))
+        if verbose and len(series) % 10 == 0:
+            print(f"  {name}: t = {t:8.2f}  Nu_bar = {d['nu_bar']:.4f}  Nu_bulk = {d['nu_bulk']:.4f}  Re = {d['re']:.3f}", flush=True)
+    s.stats_reset()
+    t_end = t + c["t_avg"]
+    while t < t_end:
+        s.step_stats(chunk, every)
+        d, *_ = s.diagnostics()
+        t = d["time"]
+        series.append((t, d["nu_bar"], d["re"]))
+    st, Tp, rp, pp = s.stats_read()
+    steps = int(d["step"])
+    s.close()
+    nu, re = st["nu_bar"], st["re"]
+    nu_sd = max(st["nu_bar_sq"] - nu * nu, 0.0) ** 0.5
+    re_sd = max(st["re_sq"] - re * re, 0.0) ** 0.5
+    out = {"case": name, "cite": c["cite"], "grid": [c["nx"], c["ny"], c["nz"]], "uniform_z": True,
+           "parameters": {k: c[k] for k in ("Ra", "D", "Gamma", "gamma", "Pr", "eps")},
+           "steps": steps, "t_end": t, "averaged_over": st["weight"], "samples": st["samples"],
+           "nu_bar": nu, "nu_bar_sd": nu_sd, "nu_bulk": st["nu_bulk"], "nu_bottom": st["nu_bottom"], "nu_top": st["nu_top"],
+           "re": re, "re_sd": re_sd,
+           "paper": {"nu": c["paper"][0], "nu_pm": c["paper"][1], "re": c["paper"][2], "re_pm": c["paper"][3]},
+           "earlier_code": {"nu": c["ref"][0], "re": c["ref"][1]},
+           "nu_vs_paper_pct": 100.0 * (nu / c["paper"][0] - 1.0), "re_vs_paper_pct": 100.0 * (re / c["paper"][2] - 1.0),
+           "wall_s": time.perf_counter() - t0}
+    if verbose:
+        print(f"{name} ({c['cite']}): Nu_bar = {nu:.4f} +- {nu_sd:.4f} (paper {c['paper'][0]} +- {c['paper'][1]}, "
+              f"{out['nu_vs_paper_pct']:+.2f} %), Re = {re:.3f} +- {re_sd:.3f} (paper {c['paper'][2]} +- {c['paper'][3]}, "
+              f"{out['re_vs_paper_pct']:+.2f} %), {steps} steps in {out['wall_s']:.0f} s", flush=True)
+    return out
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--case", action="append", choices=sorted(CASES), help="default: table2-1")
+    ap.add_argument("--out", default=None, help="write the results as JSON lines to this file")
+    args = ap.parse_args()
+    results = [run_case(n) for n in (args.case or ["table2-1"])]
+    if args.out:
+        with open(args.out, "w") as f:
+            for r in results:
+                f.write(json.dumps(r) + "\n")
+
+
+if __name__ == "__main__":
+    main()

@@ -197,6 +197,45 @@ def test_step_host_matches_step(gpu, orc, c1):
     s.close()
 
 
+@pytest.mark.parametrize("name,n,every", [("C1", 24, 3), ("3d", 9, 2)])
+def test_time_averages(gpu, orc, name, n, every):
+    """mc_tvd_step_stats / mc_tvd_stats_read against the oracle's twin: the same samples, the
+    same weights; the two states differ by the parity error of n steps, so do the averages."""
+    if name == "C1":
+        grid, params, _ = inputs.config("C1")
+    else:
+        grid, params = inputs.make_grid(3, 64, 20, 24), inputs.make_params(Ra=1e5)
+    X0 = inputs.conduction_state(grid, params, amplitude=1e-2)
+    prob = orc.Problem(grid, params)
+    ref, ro, To, rho_o, po = orc.step_stats(prob, X0, n, every)
+    s = _solver(gpu, grid, params, X0)
+    s.step_stats(n, every)
+    st, Tp, rp, pp = s.stats_read()
+    assert st["samples"] == n // every == ro["samples"]
+    assert abs(st["t_end"] - ro["t_end"]) <= 1e-12 * ro["t_end"] and abs(st["weight"] - ro["weight"]) <= 1e-12 * ro["weight"]
+    for k in ("nu_bottom", "nu_top", "nu_bar", "nu_bulk", "re", "u_rms", "nu_bar_sq", "re_sq"):
+        assert abs(st[k] - ro[k]) <= 1e-9 * max(abs(ro[k]), 1.0), (k, st[k], ro[k])
+    for k in ("nu_conv", "nu_K"):
+        assert abs(st[k] - ro[k]) <= 1e-9, (k, st[k], ro[k])
+    np.testing.assert_allclose(Tp, To, rtol=1e-12)
+    np.testing.assert_allclose(rp, rho_o, rtol=1e-12)
+    np.testing.assert_allclose(pp, po, rtol=1e-12)
+    assert parity_err(grid, params, s.state(), ref).max() <= n * TOL_1STEP
+    # sampling in one call or call by call is the same thing, bit for bit; a reset starts a new span
+    s2 = _solver(gpu, grid, params, X0)
+    for _ in range(n):
+        s2.step_stats(1, every)
+    st2, Tp2, _, _ = s2.stats_read()
+    assert st2 == st and np.array_equal(Tp2, Tp)
+    s2.stats_reset()
+    with pytest.raises(gpu.MCTVDError):
+        s2.stats_read()                                   # no sample yet
+    s2.step_stats(every, every)
+    st3, *_ = s2.stats_read()
+    assert st3["samples"] == 1 and st3["t_begin"] == st["t_end"] if n % every == 0 else st3["samples"] == 1
+    s.close(); s2.close()
+
+
 def test_3d_steps(gpu, orc):
     """A 3-D box with plates, 3 full steps of Eq. 30 (18 sweeps), CFL dt from the fused reduction."""
     grid = inputs.make_grid(3, 64, 20, 24)

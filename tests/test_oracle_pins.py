@@ -676,3 +676,52 @@ def test_sweeps_are_one_operator_under_axis_relabelling(orc, a, b):
             lhs, _ = _swap_axes(orc.sweep(orc.Problem(g, p), X, sweep_axis, 0.004, d), g, a, b)
             rhs = orc.sweep(orc.Problem(gs, p), Xs, mapped, 0.004, d)
             assert np.max(rel_err(lhs, rhs)) < 1e-14, (sweep_axis, d)
+
+
+# ----------------------------------------------------------------------------- time averages
+def test_time_averages_are_the_weighted_means_of_the_samples(orc):
+    """<f>_t = sum_k w_k f_k / sum_k w_k with w_k = t_k - t_{k-1} (time since the previous sample): the twin of
+    mc_tvd_step_stats must equal that composition of single steps and instantaneous diagnostics written out
+    here, the weights must add up to the elapsed time, and a diagnostic that does not change in time (the plate
+    temperature profile of a steady conduction state, Nu = 1) must average to itself."""
+    g, p, _ = inputs.config("C1")
+    prob = orc.Problem(g, p)
+    X0 = inputs.conduction_state(g, p, amplitude=1e-2)
+    n, every = 14, 3
+    Y, st, Tp, rp, pp = orc.step_stats(prob, X0, n, every)
+    X, t, t_last, wsum = X0, 0.0, 0.0, 0.0
+    acc = {k: 0.0 for k in ("nu_bottom", "nu_top", "nu_bar", "nu_bulk", "nu_conv", "nu_K", "re", "u_rms")}
+    sq = {"nu_bar": 0.0, "re": 0.0}
+    accT = np.zeros(g["nz"])
+    for s in range(n):
+        X, dts, _ = orc.step(prob, X, 1)
+        t += dts[0]
+        if (s + 1) % every:
+            continue
+        d, T_, _, _ = orc.diagnostics(prob, X)
+        w = t - t_last
+        for k in acc:
+            acc[k] += w * d[k]
+        for k in sq:
+            sq[k] += w * d[k] ** 2
+        accT += w * T_
+        wsum += w
+        t_last = t
+    assert np.array_equal(Y, X)
+    assert st["samples"] == n // every and st["t_end"] == t_last
+    assert st["weight"] == pytest.approx(wsum, rel=1e-15) and st["weight"] == pytest.approx(st["t_end"], rel=1e-14)
+    for k in acc:
+        assert st[k] == pytest.approx(acc[k] / wsum, rel=1e-14, abs=1e-18), k
+    assert st["nu_bar_sq"] == pytest.approx(sq["nu_bar"] / wsum, rel=1e-14)
+    assert st["re_sq"] == pytest.approx(sq["re"] / wsum, rel=1e-14)
+    np.testing.assert_allclose(Tp, accT / wsum, rtol=1e-14)
+    # Eq. 23 is linear in the plane means: the averaged plate Nusselt number is Eq. 23 of the averaged profile
+    z = inputs.z_nodes(g, p)
+    tsa = Tp - (1.0 - p["D"] * z)
+    dz = z[1]
+    assert st["nu_bottom"] == pytest.approx(-(-3 * tsa[0] + 4 * tsa[1] - tsa[2]) / (2 * dz) / p["eps"], rel=1e-9)
+    # steady conduction state (no noise): every sample is Nu = 1, Re = 0 up to the O(dz^2) drift
+    Xs = inputs.conduction_state(g, p, amplitude=0.0)
+    _, ss, Ts, _, _ = orc.step_stats(prob, Xs, 6, 2)
+    assert ss["nu_bar"] == pytest.approx(1.0, abs=1e-4) and ss["re"] < 1e-2
+    np.testing.assert_allclose(Ts, 1 - 0.5 * z, atol=2e-5)           # O(dz^2) drift of the discrete steady state
