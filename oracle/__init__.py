@@ -36,7 +36,7 @@ def build(force: bool = False) -> str:
 
 class _Grid(C.Structure):
     _fields_ = [("ndim", C.c_int), ("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int),
-                ("lx", C.c_double), ("ly", C.c_double), ("lz", C.c_double)]
+                ("lx", C.c_double), ("ly", C.c_double), ("lz", C.c_double), ("z_nodes", C.POINTER(C.c_double))]
 
 
 class _Params(C.Structure):
@@ -99,8 +99,13 @@ class Problem:
 
     def c_grid(self) -> _Grid:
         g = self.grid
+        zp = None
+        if g.get("z_nodes") is not None:             # non-uniform z (R19): keep the array alive next to the struct
+            self._z = np.ascontiguousarray(g["z_nodes"], dtype=np.float64)
+            assert self._z.size == int(g["nz"])
+            zp = self._z.ctypes.data_as(C.POINTER(C.c_double))
         return _Grid(int(g["ndim"]), int(g["nx"]), int(g.get("ny", 1)), int(g["nz"]),
-                     float(g["lx"]), float(g.get("ly", 1.0)), float(g["lz"]))
+                     float(g["lx"]), float(g.get("ly", 1.0)), float(g["lz"]), zp)
 
     def c_params(self) -> _Params:
         p = self.params

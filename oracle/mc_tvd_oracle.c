@@ -24,6 +24,7 @@ typedef struct {
     int ndim, nx, ny, nz, nf;
     size_t N;
     double d[3];                 /* dx, dy, dz */
+    const double *z;             /* NULL: uniform z; else the nz node heights z_k (R19) */
     double gamma, R, cv, icv, g, mu, K, lam;
     double Tw[2];                /* T at the bottom (k = 0) and top (k = nz-1) plates */
     int walls;                   /* 1: no-slip isothermal plates at k = 0, nz-1; 0: periodic in z */
@@ -52,6 +53,11 @@ static int ctx_init(ctx *c, const orc_grid *g, const orc_params *p)
     c->d[0] = g->lx / g->nx;
     c->d[1] = (g->ndim == 3) ? g->ly / g->ny : 1.0;
     c->d[2] = c->walls ? g->lz / (g->nz - 1) : g->lz / g->nz;
+    c->z = g->z_nodes;
+    if (c->z) {                                      /* R19: plates at the first and last node, strictly increasing */
+        if (!c->walls || g->nz < 5) return -1;
+        for (int k = 0; k + 1 < g->nz; ++k) if (!(c->z[k + 1] > c->z[k])) return -1;
+    }
     c->gamma = p->gamma;
     c->icv = p->gamma * p->eps * p->D;               /* gamma eps D: T = icv*(E/rho - u^2/2 - z/eps), Eq. 17 */
     c->cv = 1.0 / c->icv;
@@ -86,7 +92,23 @@ static long nb(const ctx *c, int i, int j, int k, int axis, int off)
     return (long)at(c, i, j, k);
 }
 
-static double z_of(const ctx *c, int k) { return (double)k * c->d[2]; }
+static double z_of(const ctx *c, int k) { return c->z ? c->z[k] : (double)k * c->d[2]; }
+
+/* Non-uniform z grid ("non-uniform tangent-hyperbolic grid in the z-direction"; the paper
+ * gives no formulas for it: reading R19).  The scheme is written in the computational
+ * coordinate zeta = k with the metric taken from the node heights themselves:
+ *   h_{k+1/2} = z_{k+1} - z_k                         spacing across a face (inner one-sided differences);
+ *   dzc_k = (z_{k+1} - z_{k-1})/2, half of the adjacent spacing at a plate node (the height of the cell
+ *           a node owns: outer MacCormack differences, central differences, Co, trapezoid weights);
+ * so that sum_k dzc_k X_k telescopes exactly as on the uniform grid.  Both reduce to dz when z_k = k dz. */
+static double hface(const ctx *c, int k) { return c->z ? c->z[k + 1] - c->z[k] : c->d[2]; }
+static double dzc(const ctx *c, int k)
+{
+    if (!c->z) return c->d[2];
+    if (k == 0) return 0.5 * (c->z[1] - c->z[0]);
+    if (k == c->nz - 1) return 0.5 * (c->z[k] - c->z[k - 1]);
+    return 0.5 * (c->z[k + 1] - c->z[k - 1]);
+}
 
 /* Primitive variables from X (Eqs. 16-17):
  * u = (rho u)/rho;  T = gamma eps D (E/rho - u^2/2 - z/eps);  p = (gamma-1)/(gamma eps D) rho T. */
@@ -113,6 +135,12 @@ static double deriv(const ctx *c, const double *f, int i, int j, int k, int axis
 {
     long n0 = (long)at(c, i, j, k);
     long np = nb(c, i, j, k, axis, +1), nm = nb(c, i, j, k, axis, -1);
+    if (axis == 2 && c->z) {                         /* R19: divide by the distance between the nodes differenced */
+        if (mode == 0) { if (np < 0 || nm < 0) return NAN; return (f[np] - f[nm]) / (c->z[k + 1] - c->z[k - 1]); }
+        if (mode > 0)  { if (np < 0) return NAN; return (f[np] - f[n0]) / hface(c, k); }
+        if (nm < 0) return NAN;
+        return (f[n0] - f[nm]) / hface(c, k - 1);
+    }
     if (mode == 0) { if (np < 0 || nm < 0) return NAN; return (f[np] - f[nm]) / (2.0 * c->d[axis]); }
     if (mode > 0)  { if (np < 0) return NAN; return (f[np] - f[n0]) / c->d[axis]; }
     if (nm < 0) return NAN;
@@ -181,10 +209,10 @@ static void wall_node(const ctx *c, double *const X[5], double *const Fl[5], dou
     double rho = X[Q_RHO][n];
     if (kw == 0 && o > 0) {
         size_t n1 = at(c, i, j, 1);
-        rho = rho - (2.0 * tau / c->d[2]) * (Fl[Q_RHO][n1] - Fl[Q_RHO][n]);
+        rho = rho - (c->z ? tau / dzc(c, kw) : 2.0 * tau / c->d[2]) * (Fl[Q_RHO][n1] - Fl[Q_RHO][n]);
     } else if (kw == c->nz - 1 && o < 0) {
         size_t n1 = at(c, i, j, c->nz - 2);
-        rho = rho - (2.0 * tau / c->d[2]) * (Fl[Q_RHO][n] - Fl[Q_RHO][n1]);
+        rho = rho - (c->z ? tau / dzc(c, kw) : 2.0 * tau / c->d[2]) * (Fl[Q_RHO][n] - Fl[Q_RHO][n1]);
     }
     double Tw = c->Tw[kw == 0 ? 0 : 1];
     Xs[Q_RHO][n] = rho;
@@ -205,6 +233,7 @@ static void stage(const ctx *c, int a, int o, double tau, double *const X[5], do
         for (int j = 0; j < c->ny; ++j)
             for (int i = 0; i < c->nx; ++i) {
                 size_t n = at(c, i, j, k);
+                if (a == 2 && c->z) cdt = tau / dzc(c, k);       /* R19: the cell height of node k */
                 if (is_wall_row(c, k)) {
                     if (a == 2) wall_node(c, X, Fl, Xs, i, j, k, o, tau);
                     else for (int f = 0; f < 5; ++f) Xs[f][n] = X[f][n];
@@ -240,7 +269,7 @@ static void tvd_interface_flux(const ctx *c, int a, double tau, double *const X[
             for (int i = 0; i < c->nx; ++i) {
                 size_t n = at(c, i, j, k);
                 double cs = sqrt(c->gamma * c->R * w[W_T][n]);
-                double Co = (fabs(w[a][n]) + cs) * tau / c->d[a];
+                double Co = (fabs(w[a][n]) + cs) * tau / ((a == 2) ? dzc(c, k) : c->d[a]);
                 Cn[n] = (Co <= 0.5) ? Co * (1.0 - Co) : 0.25;
             }
     for (int k = 0; k < c->nz; ++k)
@@ -265,7 +294,11 @@ static void tvd_interface_flux(const ctx *c, int a, double tau, double *const X[
                 else
                     coef = 0.5 * Cn[n] * (1.0 - phi_minmod(rplus_k))
                          + 0.5 * Cn[np] * (1.0 - phi_minmod(rminus_kp));
-                for (int f = 0; f < 5; ++f) Dh[f][n] = coef * d0[f];
+                /* R20 (non-uniform z only): in the computational coordinate the dissipation acts on dzc_k X_k, so the
+                 * interface flux carries the face spacing h_{k+1/2} and sweep5 divides the difference by dzc_k; the sum
+                 * of dzc_k T_k over a column then telescopes (conservation) and a uniform grid gives Eq. 34 back. */
+                double hw = (a == 2 && c->z) ? hface(c, k) : 1.0;
+                for (int f = 0; f < 5; ++f) Dh[f][n] = hw * (coef * d0[f]);
             }
     free(Cn);
 }
@@ -307,6 +340,7 @@ static void sweep5(const ctx *c, int a, double tau, int dir, double *const X[5],
                 long nm = nb(c, i, j, k, a, -1);
                 for (int f = 0; f < 5; ++f) {
                     double T = Dh[f][n] - Dh[f][nm];               /* Eq. 34 */
+                    if (a == 2 && c->z) T = T / dzc(c, k);         /* R20 */
                     Xo[f][n] = 0.5 * (XP[f][n] + XC[f][n]) + T;    /* Eq. 33 */
                 }
             }
@@ -357,7 +391,11 @@ double orc_max_speed(const orc_grid *g, const orc_params *p, const double *X)
                 double cs = sqrt(c.gamma * c.R * T);
                 for (int a = 0; a < 3; ++a) {
                     if (c.ndim == 2 && a == 1) continue;
-                    double v = (fabs(u[a]) + cs) / c.d[a];
+                    /* z: the height of the node's cell (R19); a plate node, whose cell is a half cell, takes the
+                     * full adjacent spacing, as on the uniform grid */
+                    double da = c.d[a];
+                    if (a == 2 && c.z) da = (k == 0 || k == c.nz - 1) ? 2.0 * dzc(&c, k) : dzc(&c, k);
+                    double v = (fabs(u[a]) + cs) / da;
                     if (!isfinite(v)) bad = 1;
                     if (v > s) s = v;
                 }
@@ -453,7 +491,7 @@ int orc_diagnostics(const orc_grid *g, const orc_params *p, const double *X, orc
             pT += rT; prho += rrho; pp += rp; pconv += rconv; pK += rK; pu2 += ru2;
             for (int f = 0; f < 5; ++f) pq[f] += rq[f];
         }
-        double wk = c.d[2] * ((c.walls && (k == 0 || k == nz - 1)) ? 0.5 : 1.0);
+        double wk = c.z ? dzc(&c, k) : c.d[2] * ((c.walls && (k == 0 || k == nz - 1)) ? 0.5 : 1.0);
         sT[k] = pT / nplane;
         sTsa[k] = sT[k] - TA;
         if (T_prof) T_prof[k] = sT[k];
@@ -475,6 +513,16 @@ int orc_diagnostics(const orc_grid *g, const orc_params *p, const double *X, orc
         double dz = c.d[2];
         double g0 = (-3.0 * sTsa[0] + 4.0 * sTsa[1] - sTsa[2]) / (2.0 * dz);
         double g1 = (3.0 * sTsa[nz - 1] - 4.0 * sTsa[nz - 2] + sTsa[nz - 3]) / (2.0 * dz);
+        if (c.z) {
+            /* second-order one-sided differences through the plate node and its two neighbours at distances h1 < h2
+             * (the derivative of the quadratic through the three points; (-3, 4, -1)/(2 dz) when h2 = 2 h1) */
+            double h1 = c.z[1] - c.z[0], h2 = c.z[2] - c.z[0];
+            double b = h2 / (h1 * (h2 - h1)), cc = -h1 / (h2 * (h2 - h1));
+            g0 = -(b + cc) * sTsa[0] + b * sTsa[1] + cc * sTsa[2];
+            h1 = c.z[nz - 1] - c.z[nz - 2]; h2 = c.z[nz - 1] - c.z[nz - 3];
+            b = h2 / (h1 * (h2 - h1)); cc = -h1 / (h2 * (h2 - h1));
+            g1 = (b + cc) * sTsa[nz - 1] - b * sTsa[nz - 2] - cc * sTsa[nz - 3];
+        }
         out->nu_bottom = -g0 / p->eps;
         out->nu_top = -g1 / p->eps;
         out->nu_bar = 0.5 * (out->nu_bottom + out->nu_top);

@@ -38,6 +38,8 @@ typedef struct {
     int ndim;            /* 2 or 3 */
     int nx, ny, nz;      /* ny = 1 in 2-D; nz counts both wall nodes */
     double lx, ly, lz;   /* box size; 4,4,1 for the paper's aspect ratio 4 */
+    const double *z_nodes; /* NULL: uniform z.  Else nz strictly increasing node heights, plates at the first and
+                              last (bc_z = 0 only): the paper's non-uniform z grid, readings R19-R20 */
 } orc_grid;
 
 typedef struct {

@@ -29,13 +29,30 @@ CONFIGS = {
 }
 
 
+TANH_STRETCH = 1.5      # default stretching of `tanh_nodes` (the paper names the grid but gives no parameter)
+
+
+def tanh_nodes(nz: int, lz: float = 1.0, stretch: float = TANH_STRETCH) -> np.ndarray:
+    """Node heights of a "non-uniform tangent-hyperbolic grid in the z-direction" with nodes on
+    both plates: z_k = lz/2 (1 + tanh(s (2k/(nz-1) - 1)) / tanh(s)), finest at the plates.  The paper does not
+    state its stretching parameter; s = 1.5 makes the plate spacing about 0.3 of the uniform one."""
+    xi = 2.0 * np.arange(nz, dtype=np.float64) / (nz - 1) - 1.0
+    z = 0.5 * lz * (1.0 + np.tanh(stretch * xi) / np.tanh(stretch))
+    z[0], z[-1] = 0.0, lz
+    return z
+
+
 def make_grid(ndim: int, nx: int, nz: int, ny: int = 1, lx: float = 4.0, ly: float = 4.0,
-              lz: float = 1.0) -> dict:
-    """Box of aspect ratio 4 by default."""
+              lz: float = 1.0, z_stretch: float | None = None) -> dict:
+    """Box of aspect ratio 4 by default.  z_stretch: tanh-stretched z nodes (`tanh_nodes`),
+    stored under "z_nodes"; None = uniform z."""
     if ndim == 2:
         ny, ly = 1, 1.0
-    return dict(ndim=int(ndim), nx=int(nx), ny=int(ny), nz=int(nz), lx=float(lx), ly=float(ly),
-                lz=float(lz))
+    g = dict(ndim=int(ndim), nx=int(nx), ny=int(ny), nz=int(nz), lx=float(lx), ly=float(ly),
+             lz=float(lz))
+    if z_stretch is not None:
+        g["z_nodes"] = tanh_nodes(nz, lz, z_stretch)
+    return g
 
 
 def make_params(**over) -> dict:
@@ -73,6 +90,8 @@ def closure_constants(params: dict) -> dict:
 
 
 def z_nodes(grid: dict, params: dict) -> np.ndarray:
+    if grid.get("z_nodes") is not None:
+        return np.asarray(grid["z_nodes"], dtype=np.float64)
     nz = grid["nz"]
     dz = grid["lz"] / (nz - 1) if params["bc_z"] == 0 else grid["lz"] / nz
     return np.arange(nz, dtype=np.float64) * dz
@@ -110,11 +129,12 @@ def conduction_state(grid: dict, params: dict, seed: int = SEED, amplitude: floa
     nxg = nx if nx_global is None else nx_global
     c = closure_constants(params)
     z = z_nodes(grid, params)
-    dz = z[1] - z[0]
+    uniform = grid.get("z_nodes") is None
     Tbar = params["T_bot"] + (params["T_top"] - params["T_bot"]) * z / grid["lz"]
     rho = np.empty(nz)
     rho[0] = 1.0
     for k in range(nz - 1):   # p_{k+1} - p_k = -(dz/2) g (rho_k + rho_{k+1}),  p = R rho Tbar
+        dz = (z[1] - z[0]) if uniform else (z[k + 1] - z[k])
         rho[k + 1] = rho[k] * (c["R"] * Tbar[k] - c["g"] * dz / 2) / (c["R"] * Tbar[k + 1] + c["g"] * dz / 2)
     nf = num_fields(grid)
     X = np.zeros((nf, nz, ny * nx), dtype=np.float64)     # momenta stay zero (u = 0)
