@@ -39,7 +39,7 @@ typedef enum {
     MC_TVD_ECUDA = -2,        /* a CUDA runtime call or kernel launch failed */
     MC_TVD_ENOMEM = -3,       /* workspace too small / host allocation failed */
     MC_TVD_ENONFINITE = -4,   /* state holds a non-finite value or non-positive rho or T */
-    MC_TVD_EUNSUPPORTED = -5  /* valid request this build does not implement (e.g. z_nodes != NULL) */
+    MC_TVD_EUNSUPPORTED = -5  /* valid request this build does not implement (e.g. 2^32 or more nodes per field) */
 } mc_tvd_status;
 
 /* The box (Sec. 2; aspect ratio 4). */
@@ -47,7 +47,15 @@ typedef struct {
     int ndim;                 /* 2 or 3 */
     int nx, ny, nz;           /* ny = 1 in 2-D; nx, ny = distinct periodic nodes; nz counts both plate nodes */
     double lx, ly, lz;        /* box size: 4, 4, 1 for the paper's runs */
-    const double *z_nodes;    /* NULL = uniform z.  Non-NULL (tanh grid) -> MC_TVD_EUNSUPPORTED */
+    const double *z_nodes;    /* NULL = uniform z, z_k = k lz / (nz - 1).  Else HOST array of nz strictly increasing node
+                                 heights, plates at the first and last (bc_z = 0 only): the paper's "non-uniform
+                                 tangent-hyperbolic grid in the z-direction".  The paper prints no formula
+                                 for it; R19 / R20: outer differences, central differences, Co and trapezoid weights
+                                 use the height of the cell a node owns, (z_{k+1} - z_{k-1})/2 (half the adjacent spacing
+                                 at a plate), inner one-sided differences the spacing across the face, the TVD interface
+                                 flux carries the face spacing.  Read during mc_tvd_init only; any node spacing is
+                                 accepted, so no stretching parameter appears in this interface.  MC_TVD_EINVAL if not
+                                 increasing or bc_z != 0. */
 } mc_tvd_grid;
 
 /* The paper's dimensionless numbers and the switches of DESIGN.md's readings. */

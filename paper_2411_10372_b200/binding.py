@@ -109,8 +109,17 @@ def load_library(path: str | None = None) -> C.CDLL:
 
 
 def make_grid(grid: dict) -> Grid:
-    return Grid(int(grid["ndim"]), int(grid["nx"]), int(grid.get("ny", 1)), int(grid["nz"]),
-                float(grid["lx"]), float(grid.get("ly", 1.0)), float(grid["lz"]), None)
+    """grid["z_nodes"] (optional): nz node heights of the non-uniform z grid; the library copies what it
+    needs during mc_tvd_init, the array only has to live until then (it is kept on the returned struct)."""
+    g = Grid(int(grid["ndim"]), int(grid["nx"]), int(grid.get("ny", 1)), int(grid["nz"]),
+             float(grid["lx"]), float(grid.get("ly", 1.0)), float(grid["lz"]), None)
+    if grid.get("z_nodes") is not None:
+        z = np.ascontiguousarray(grid["z_nodes"], dtype=np.float64)
+        if z.size != g.nz:
+            raise ValueError("z_nodes must hold nz values")
+        g._z_keepalive = z
+        g.z_nodes = z.ctypes.data_as(_DP)
+    return g
 
 
 def make_params(p: dict) -> Params:

@@ -82,7 +82,7 @@ constexpr int LANE_MINB_2D = MC_LANE_MINB_2D;
 constexpr int DIAG_MAX_BLOCKS = 16;    // blocks per plane in the diagnostics pass (the finish kernel walks them)
 
 struct Layout {                        // byte offsets inside the workspace
-    size_t Y, scalars, partial, ext, plane_sums, plane_ext, diag_out, stats, stats_out, total;
+    size_t Y, scalars, partial, ext, plane_sums, plane_ext, diag_out, stats, stats_out, zt, total;
     int diag_blocks;
 };
 
@@ -99,6 +99,8 @@ struct mc_tvd_state {
     double *X, *Y;
     mc::Scalars *S;
     double *partial, *ext, *plane_sums, *plane_ext, *diag_out, *stats, *stats_out;
+    const double *zt;                  // device z-metric tables of the non-uniform grid (R19 / R20), or null
+    double zt_max_icfl;                // max over levels of the CFL rule's reciprocal z spacing
     long long stat_steps;              // steps taken through mc_tvd_step_stats since the last reset
     int diag_blocks;
     cudaStream_t stream;
@@ -134,12 +136,17 @@ bool valid_problem(const mc_tvd_grid *g, const mc_tvd_params *p, int *code)
         *code = MC_TVD_EUNSUPPORTED;
         return fail(0, "more than 2^32 - 1 nodes per field: the kernels index nodes with 32 bits"), false;
     }
-    if (g->z_nodes) { *code = MC_TVD_EUNSUPPORTED; return fail(0, "non-uniform z grid is not built (SURVEY 8f)"), false; }
     if (!(p->gamma > 1) || !(p->eps > 0) || !(p->D > 0) || !(p->Pr > 0) || !(p->Ra > 0))
         return fail(0, "need gamma > 1 and eps, D, Pr, Ra > 0"), false;
     if (!(p->fixed_dt > 0) && !(p->cfl > 0)) return fail(0, "need cfl > 0 or fixed_dt > 0"), false;
     if ((p->bc_z | 1) != 1 || (p->tvd_form | 1) != 1 || (p->dir_mode | 1) != 1 || (p->tvd_off | 1) != 1)
         return fail(0, "bc_z, tvd_form, dir_mode, tvd_off must be 0 or 1"), false;
+    if (g->z_nodes) {                  // non-uniform z grid (R19): plates at the first and last node
+        if (p->bc_z != 0) return fail(0, "z_nodes needs plates (bc_z = 0)"), false;
+        for (int k = 0; k + 1 < g->nz; ++k)
+            if (!(g->z_nodes[k + 1] > g->z_nodes[k]) || !isfinite(g->z_nodes[k + 1]) || !isfinite(g->z_nodes[k]))
+                return fail(0, "z_nodes must be finite and strictly increasing"), false;
+    }
     return true;
 }
 
@@ -162,6 +169,7 @@ Layout make_layout(const mc_tvd_grid *g)
     L.diag_out = o;   o = align_up(o + (19 + 3 * (size_t)g->nz) * sizeof(double), 256);
     L.stats = o;      o = align_up(o + (mc::ST_HEAD + 3 * (size_t)g->nz) * sizeof(double), 256);
     L.stats_out = o;  o = align_up(o + (4 + mc::ST_NSUM + 3 * (size_t)g->nz) * sizeof(double), 256);
+    L.zt = o;         o = align_up(o + 5 * (size_t)g->nz * sizeof(double), 256);       // z-metric tables (SweepArgs::zt)
     L.total = o;
     return L;
 }
@@ -200,6 +208,18 @@ void fill_common(const mc_tvd_state *s, mc::SweepArgs &A, const double *in, doub
         A.lam_mu_2c[c] = lam * mu / (2.0 * s->d[a]);
     }
     A.dz = s->d[2];
+    if (s->zt) {
+        // non-uniform z (R19 / R20): every z spacing folded into a launch constant becomes 1; the kernels (template
+        // switch ZS) multiply by the local metric from the tables instead
+        const int cz = comp_of_axis(s->nd, 2);
+        A.zt = s->zt;
+        A.mu_2c[cz] = mu; A.lam_mu_2c[cz] = lam * mu;        // central z-differences: x 1 / (z_{k+1} - z_{k-1}) in the kernel
+        A.inv_d[cz] = s->zt_max_icfl;                         // only the bound D of the CFL filter uses it
+        if (alpha == 2) {
+            A.d_a = 1.0; A.inv_h = (dir > 0 ? 1.0 : -1.0);
+            A.mu_h = mu * A.inv_h; A.two_mu_h = 2.0 * mu * A.inv_h; A.lam_mu_h = lam * mu * A.inv_h; A.K_h = s->K * A.inv_h;
+        }
+    }
     A.R = s->R; A.cv = s->cv; A.icv = s->icv; A.g = s->g;
     A.gamma = s->par.gamma; A.gammaR = s->par.gamma * s->R;
     A.Tw0 = s->par.T_bot; A.Tw1 = s->par.T_top;
@@ -236,6 +256,12 @@ int pick_chunk(const mc_tvd_state *s, int n_m, long long tiles, int blocks_per_s
 template <class F> void with_bool(bool b, F f)
 {
     if (b) f(std::true_type()); else f(std::false_type());
+}
+// the non-uniform z grid exists between plates only: ZS kernels are instantiated for WALL = true
+template <class W, class F> void with_zs(const mc_tvd_state *s, W, F f)
+{
+    if constexpr (W::value) { if (s->zt) { f(std::true_type()); return; } }
+    f(std::false_type());
 }
 // MC_ONLY_DEFAULT_SWITCHES (tuning builds only): instantiate just the plates + Davis/Yee kernels
 template <class F> void with_walls(bool b, F f)
@@ -314,9 +340,9 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
             A.chunk = pick_chunk(s, nz, tiles, MARCH_MINB_2D);
             dim3 block(WX, 1, 1), grid((unsigned)tiles, 1, (unsigned)((nz + A.chunk - 1) / A.chunk));
             size_t smem = ((size_t)4 * 2 * WX + 4) * sizeof(double);
-            with_walls(wl, [&](auto W) { with_tvd(s, [&](auto T) {
-                launch_kernel(mc::k_march<2, 1, -1, WX, 1, decltype(W)::value, false, decltype(T)::value, MARCH_MINB_2D>, grid, block, smem, st, A);
-            }); });
+            with_walls(wl, [&](auto W) { with_tvd(s, [&](auto T) { with_zs(s, W, [&](auto Z) {
+                launch_kernel(mc::k_march<2, 1, -1, WX, 1, decltype(W)::value, false, decltype(T)::value, MARCH_MINB_2D, decltype(Z)::value>, grid, block, smem, st, A);
+            }); }); });
         } else if (alpha == 0 && MC_LANE2 && nx % 2 == 0) {   // x-sweep, even nx: two nodes per lane, march z
             constexpr int LW = MC_LANE2_WARPS;
             geo_x = mc::LANE2_OUT;
@@ -326,9 +352,9 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
             A.chunk = pick_chunk(s, nz, tiles, MC_LANE2_MINB);
             dim3 block(32, LW, 1), grid((unsigned)tiles, 1, (unsigned)((nz + A.chunk - 1) / A.chunk));
             with_walls(wl, [&](auto W) { with_tvd(s, [&](auto T) { with_bool(reduce, [&](auto Rd) {
-                with_bool(dir > 0, [&](auto Fw) {
-                    launch_kernel(mc::k_lane2<LW, decltype(W)::value, decltype(T)::value, decltype(Rd)::value, MC_LANE2_MINB, decltype(Fw)::value>, grid, block, 0, st, A);
-                });
+                with_bool(dir > 0, [&](auto Fw) { with_zs(s, W, [&](auto Z) {
+                    launch_kernel(mc::k_lane2<LW, decltype(W)::value, decltype(T)::value, decltype(Rd)::value, MC_LANE2_MINB, decltype(Fw)::value, decltype(Z)::value>, grid, block, 0, st, A);
+                }); });
             }); }); });
         } else if (alpha == 0) {     // x-sweep: lanes x, march z
             constexpr int LW = LANE_WARPS_2D;
@@ -338,9 +364,9 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
             long long tiles = (xt + LW - 1) / LW;
             A.chunk = pick_chunk(s, nz, tiles, LANE_MINB_2D);
             dim3 block(32, LW, 1), grid((unsigned)tiles, 1, (unsigned)((nz + A.chunk - 1) / A.chunk));
-            with_walls(wl, [&](auto W) { with_tvd(s, [&](auto T) { with_bool(reduce, [&](auto Rd) {
-                launch_kernel(mc::k_lane<2, -1, 1, LW, decltype(W)::value, decltype(T)::value, decltype(Rd)::value, LANE_MINB_2D>, grid, block, 0, st, A);
-            }); }); });
+            with_walls(wl, [&](auto W) { with_tvd(s, [&](auto T) { with_bool(reduce, [&](auto Rd) { with_zs(s, W, [&](auto Z) {
+                launch_kernel(mc::k_lane<2, -1, 1, LW, decltype(W)::value, decltype(T)::value, decltype(Rd)::value, LANE_MINB_2D, decltype(Z)::value>, grid, block, 0, st, A);
+            }); }); }); });
         } else {
             return fail(MC_TVD_EINVAL, "a 2-D problem has no y-sweep");
         }
@@ -356,9 +382,9 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
             A.chunk = pick_chunk(s, nz, xt * bt, 1);
             dim3 mblock(32, MW, 1), grid((unsigned)xt, (unsigned)bt, (unsigned)((nz + A.chunk - 1) / A.chunk));
             size_t smem = mc::tile3_async_bytes(MW) + ((size_t)4 * 3 * 32 * (MW + 2) + 4) * sizeof(double);
-            with_walls(wl, [&](auto W) { with_tvd(s, [&](auto T) {
-                launch_kernel(mc::k_march3<2, 1, MW, decltype(W)::value, false, decltype(T)::value, 1, true>, grid, mblock, smem, st, A, s->tm_rows_y[ibuf]);
-            }); });
+            with_walls(wl, [&](auto W) { with_tvd(s, [&](auto T) { with_zs(s, W, [&](auto Z) {
+                launch_kernel(mc::k_march3<2, 1, MW, decltype(W)::value, false, decltype(T)::value, 1, true, decltype(Z)::value>, grid, mblock, smem, st, A, s->tm_rows_y[ibuf]);
+            }); }); });
         } else if (alpha == 1 && s->async3) {   // y-sweep, TMA-staged tiles: march y, tile (x, z)
             constexpr int MW = MARCH3_WB_AS, MO = MW - 2;
             A.n_b = nz; A.s_b = (long long)nx * ny; A.n_m = ny; A.s_m = nx;
@@ -367,9 +393,9 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
             A.chunk = pick_chunk(s, ny, xt * bt, 1);
             dim3 mblock(32, MW, 1), grid((unsigned)xt, (unsigned)bt, (unsigned)((ny + A.chunk - 1) / A.chunk));
             size_t smem = mc::tile3_async_bytes(MW) + ((size_t)4 * 3 * 32 * (MW + 2) + 4) * sizeof(double);
-            with_walls(wl, [&](auto W) { with_tvd(s, [&](auto T) {
-                launch_kernel(mc::k_march3<1, 2, MW, false, decltype(W)::value, decltype(T)::value, 1, true>, grid, mblock, smem, st, A, s->tm_rows_z[ibuf]);
-            }); });
+            with_walls(wl, [&](auto W) { with_tvd(s, [&](auto T) { with_zs(s, W, [&](auto Z) {
+                launch_kernel(mc::k_march3<1, 2, MW, false, decltype(W)::value, decltype(T)::value, 1, true, decltype(Z)::value>, grid, mblock, smem, st, A, s->tm_rows_z[ibuf]);
+            }); }); });
         } else if (alpha == 2) {            // z-sweep: march z, tile (x, y)
             constexpr int MW = MARCH3_WB, MO = MW - 2;
             A.n_b = ny; A.s_b = nx; A.n_m = nz; A.s_m = (long long)nx * ny;
@@ -378,9 +404,9 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
             A.chunk = pick_chunk(s, nz, xt * bt, 1);
             dim3 mblock(32, MW, 1), grid((unsigned)xt, (unsigned)bt, (unsigned)((nz + A.chunk - 1) / A.chunk));
             size_t smem = ((size_t)4 * 3 * 32 * (MW + 2) + 4) * sizeof(double);
-            with_walls(wl, [&](auto W) { with_tvd(s, [&](auto T) {
-                launch_kernel(mc::k_march3<2, 1, MW, decltype(W)::value, false, decltype(T)::value, MC_MARCH3_MINB, false>, grid, mblock, smem, st, A, s->tm_rows_y[ibuf]);
-            }); });
+            with_walls(wl, [&](auto W) { with_tvd(s, [&](auto T) { with_zs(s, W, [&](auto Z) {
+                launch_kernel(mc::k_march3<2, 1, MW, decltype(W)::value, false, decltype(T)::value, MC_MARCH3_MINB, false, decltype(Z)::value>, grid, mblock, smem, st, A, s->tm_rows_y[ibuf]);
+            }); }); });
         } else if (alpha == 1) {     // y-sweep: march y, tile (x, z)
             constexpr int MW = MARCH3_WB, MO = MW - 2;
             A.n_b = nz; A.s_b = (long long)nx * ny; A.n_m = ny; A.s_m = nx;
@@ -389,9 +415,9 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
             A.chunk = pick_chunk(s, ny, xt * bt, 1);
             dim3 mblock(32, MW, 1), grid((unsigned)xt, (unsigned)bt, (unsigned)((ny + A.chunk - 1) / A.chunk));
             size_t smem = ((size_t)4 * 3 * 32 * (MW + 2) + 4) * sizeof(double);
-            with_walls(wl, [&](auto W) { with_tvd(s, [&](auto T) {
-                launch_kernel(mc::k_march3<1, 2, MW, false, decltype(W)::value, decltype(T)::value, MC_MARCH3_MINB, false>, grid, mblock, smem, st, A, s->tm_rows_z[ibuf]);
-            }); });
+            with_walls(wl, [&](auto W) { with_tvd(s, [&](auto T) { with_zs(s, W, [&](auto Z) {
+                launch_kernel(mc::k_march3<1, 2, MW, false, decltype(W)::value, decltype(T)::value, MC_MARCH3_MINB, false, decltype(Z)::value>, grid, mblock, smem, st, A, s->tm_rows_z[ibuf]);
+            }); }); });
         } else {                     // x-sweep: lanes x, tile (x, y), march z
             constexpr int LW = LANE3_WB, LO = LW - 2;
             A.n_b = ny; A.s_b = nx; A.n_m = nz; A.s_m = (long long)nx * ny;
@@ -400,9 +426,9 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
             A.chunk = pick_chunk(s, nz, xt * bt, 1);
             dim3 lblock(32, LW, 1), grid((unsigned)xt, (unsigned)bt, (unsigned)((nz + A.chunk - 1) / A.chunk));
             size_t smem = (size_t)4 * 2 * 32 * (LW + 2) * sizeof(double);
-            with_walls(wl, [&](auto W) { with_tvd(s, [&](auto T) { with_bool(reduce, [&](auto Rd) {
-                launch_kernel(mc::k_lane3<1, 2, LW, decltype(W)::value, decltype(T)::value, decltype(Rd)::value>, grid, lblock, smem, st, A);
-            }); }); });
+            with_walls(wl, [&](auto W) { with_tvd(s, [&](auto T) { with_bool(reduce, [&](auto Rd) { with_zs(s, W, [&](auto Z) {
+                launch_kernel(mc::k_lane3<1, 2, LW, decltype(W)::value, decltype(T)::value, decltype(Rd)::value, decltype(Z)::value>, grid, lblock, smem, st, A);
+            }); }); }); });
         }
     }
     s->geom[alpha][0] = geo_x; s->geom[alpha][1] = geo_b; s->geom[alpha][2] = A.chunk;
@@ -427,6 +453,7 @@ mc::PointArgs point_args(const mc_tvd_state *s)
         if (s->nd == 2 && a == 1) continue;
         P.inv_d[comp_of_axis(s->nd, a)] = 1.0 / s->d[a];
     }
+    P.zt = s->zt;
     return P;
 }
 
@@ -498,6 +525,8 @@ int mc_tvd_init(const mc_tvd_grid *grid, const mc_tvd_params *params, double *d_
     s->diag_out = (double *)(w + L.diag_out);
     s->stats = (double *)(w + L.stats);
     s->stats_out = (double *)(w + L.stats_out);
+    s->zt = nullptr; s->zt_max_icfl = 0.0;
+    s->grid.z_nodes = nullptr;         // the caller's array is not kept: its numbers live in the device tables
     s->diag_blocks = L.diag_blocks;
     s->stream = (cudaStream_t)cuda_stream;
     s->chunk_override = 0;
@@ -520,11 +549,37 @@ int mc_tvd_init(const mc_tvd_grid *grid, const mc_tvd_params *params, double *d_
         if (rc != MC_TVD_OK) { delete s; return rc; }
     }
 
+    // Non-uniform z grid (R19 / R20): the metric tables of SweepArgs::zt, built once from the caller's
+    // node heights: z, g z, 1 / cell height, 1 / face spacing, face spacing.
+    double *zt_host = nullptr;
+    if (grid->z_nodes) {
+        const int nz = grid->nz;
+        const double *z = grid->z_nodes;
+        zt_host = (double *)malloc(5 * (size_t)nz * sizeof(double));
+        if (!zt_host) { delete s; return fail(MC_TVD_ENOMEM, "host allocation failed"); }
+        for (int k = 0; k < nz; ++k) {
+            const double dzc = (k == 0) ? 0.5 * (z[1] - z[0]) : (k == nz - 1) ? 0.5 * (z[k] - z[k - 1]) : 0.5 * (z[k + 1] - z[k - 1]);
+            const double hf = (k < nz - 1) ? z[k + 1] - z[k] : z[k] - z[k - 1];
+            zt_host[k] = z[k];
+            zt_host[nz + k] = s->g * z[k];
+            zt_host[2 * nz + k] = 1.0 / dzc;
+            zt_host[3 * nz + k] = 1.0 / hf;
+            zt_host[4 * nz + k] = hf;
+            const double icfl = (k == 0 || k == nz - 1) ? 0.5 / dzc : 1.0 / dzc;
+            if (icfl > s->zt_max_icfl) s->zt_max_icfl = icfl;
+        }
+        double *zt_dev = (double *)(w + L.zt);
+        rc = cuda_check(cudaMemcpyAsync(zt_dev, zt_host, 5 * (size_t)nz * sizeof(double), cudaMemcpyHostToDevice, s->stream),
+                        "z table upload");
+        s->zt = zt_dev;
+    }
+
     mc::Scalars h;
     memset(&h, 0, sizeof(h));
     h.cfl = params->cfl; h.fixed_dt = params->fixed_dt;
-    rc = cuda_check(cudaMemcpyAsync(s->S, &h, sizeof(h), cudaMemcpyHostToDevice, s->stream), "scalar upload");
-    if (rc == MC_TVD_OK) rc = cuda_check(cudaStreamSynchronize(s->stream), "scalar upload sync");   // h is on the stack
+    if (rc == MC_TVD_OK) rc = cuda_check(cudaMemcpyAsync(s->S, &h, sizeof(h), cudaMemcpyHostToDevice, s->stream), "scalar upload");
+    if (rc == MC_TVD_OK) rc = cuda_check(cudaStreamSynchronize(s->stream), "scalar upload sync");   // h and zt_host are host temporaries
+    free(zt_host);
     if (rc == MC_TVD_OK) rc = enqueue_initial_dt(s);
     if (rc == MC_TVD_OK) rc = mc_tvd_stats_reset(s);
     if (rc != MC_TVD_OK) { delete s; return rc; }
@@ -635,6 +690,7 @@ int enqueue_diagnostics(mc_tvd_state *s)
     G.nplane = (double)s->grid.nx * (double)s->grid.ny;
     G.dz = s->d[2]; G.dxdy = s->d[0] * s->d[1];
     G.eps = s->par.eps; G.D = s->par.D; G.Ra = s->par.Ra; G.Pr = s->par.Pr;
+    G.zt = s->zt;
     { auto kfn = mc::k_diag_planes; MC_LAUNCH(kfn, (unsigned)((s->grid.nz + 3) / 4), 128, 0, s->stream, G, s->plane_ext); }
     { auto kfn = mc::k_diag_finish; MC_LAUNCH(kfn, 1, mc::DIAG_THREADS, 0, s->stream, G, s->plane_ext); }
     s->launches += 3;

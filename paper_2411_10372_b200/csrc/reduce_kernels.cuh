@@ -21,7 +21,11 @@ struct PointArgs {                   // what a pointwise pass over the state nee
     int nz;
     double dz, g, icv, R, gamma, D;
     double inv_d[3];
+    const double *zt;                // non-uniform z grid: the tables of SweepArgs::zt, or null
 };
+
+MC_DEV double point_z(const PointArgs &P, int k) { return P.zt ? P.zt[k] : (double)k * P.dz; }
+MC_DEV double point_gz(const PointArgs &P, int k) { return P.zt ? P.zt[P.nz + k] : P.g * ((double)k * P.dz); }
 
 template <int ND>
 MC_DEV void node_primitives(const PointArgs &P, long long n, int k, double (&X)[ND + 2], double (&u)[ND],
@@ -32,7 +36,7 @@ MC_DEV void node_primitives(const PointArgs &P, long long n, int k, double (&X)[
     double inv = rcp(X[0]), ke = 0.0;
 #pragma unroll
     for (int c = 0; c < ND; ++c) { u[c] = X[1 + c] * inv; ke += u[c] * u[c]; }
-    T = (X[ND + 1] * inv - 0.5 * ke - P.g * ((double)k * P.dz)) * P.icv;       // Eq. 17
+    T = (X[ND + 1] * inv - 0.5 * ke - point_gz(P, k)) * P.icv;                 // Eq. 17
 }
 
 // s = max over nodes and directions of (|u_a| + c_s)/dx_a (R12); NaN if rho or T is not positive.
@@ -48,8 +52,10 @@ MC_KERNEL void k_max_speed(PointArgs P, unsigned long long *smax_bits)
         double s = 0.0;
         if (!(X[0] > 0.0) || !(T > 0.0)) s = NAN;
         double cs = sqrt(P.gamma * P.R * T);
+        // non-uniform z (R19): the cell height; a plate node takes the full adjacent spacing
+        const double idz = P.zt ? P.zt[2 * P.nz + k] * ((k == 0 || k == P.nz - 1) ? 0.5 : 1.0) : P.inv_d[ND - 1];
 #pragma unroll
-        for (int c = 0; c < ND; ++c) s = fmax_nan(s, (fabs(u[c]) + cs) * P.inv_d[c]);
+        for (int c = 0; c < ND; ++c) s = fmax_nan(s, (fabs(u[c]) + cs) * (c == ND - 1 ? idz : P.inv_d[c]));
         smax = fmax_nan(smax, s);
     }
 #pragma unroll
@@ -100,8 +106,8 @@ MC_KERNEL void k_plane_partials(PointArgs P, double *partial, double *ext)
 {
     constexpr int NF = ND + 2, NQ = 6 + NF;
     const int k = blockIdx.y;
-    const double TA = 1.0 - P.D * ((double)k * P.dz);          // adiabatic profile, Eq. 19
-    const double gz = P.g * ((double)k * P.dz);
+    const double TA = 1.0 - P.D * point_z(P, k);               // adiabatic profile, Eq. 19
+    const double gz = point_gz(P, k);
     const double igR = 1.0 / (P.gamma * P.R);
     Acc accT; accT.s = 0.0; accT.c = 0.0;
     double acc[NQ];
@@ -182,6 +188,7 @@ struct DiagArgs {
     const Scalars *S;
     int nz, nblk, nq, walls;
     double nplane, dz, dxdy, eps, D, Ra, Pr;
+    const double *zt;                // non-uniform z grid: the tables of SweepArgs::zt, or null
 };
 
 // Stage 2: the partial sums of one z plane -> plane_sums[k][q] (one warp per plane, lane q walks the plane's
@@ -221,7 +228,8 @@ MC_KERNEL void k_diag_finish(DiagArgs G, const double *plane_ext)
     for (int i = 0; i < NV; ++i) v[i] = 0.0;
     for (int k = threadIdx.x; k < nz; k += blockDim.x) {
         const double *ps = G.plane_sums + (long long)k * DQ_MAXQ;
-        const double wk = G.dz * ((G.walls && (k == 0 || k == nz - 1)) ? 0.5 : 1.0);
+        // trapezoid weight = the height of the cell the node owns (R16; R19 on the non-uniform grid)
+        const double wk = G.zt ? 1.0 / G.zt[2 * nz + k] : G.dz * ((G.walls && (k == 0 || k == nz - 1)) ? 0.5 : 1.0);
         Tp[k] = ps[DQ_T] / G.nplane; rp[k] = ps[DQ_RHO] / G.nplane; pp[k] = ps[DQ_P] / G.nplane;
         v[0] += wk;
         v[1] += wk * (ps[DQ_CONV] / G.nplane);
@@ -258,9 +266,20 @@ MC_KERNEL void k_diag_finish(DiagArgs G, const double *plane_ext)
     double nu0 = 0.0, nu1 = 0.0;
     if (nz >= 3) {                                                     // Eq. 23 with PAPER.md:309
         // (Tp[0..2] and Tp[nz-3..nz-1] were written by other threads of this block before the barriers above)
-        auto tsa = [&](int k) { return Tp[k] - (1.0 - G.D * ((double)k * G.dz)); };
+        auto zk = [&](int k) { return G.zt ? G.zt[k] : (double)k * G.dz; };
+        auto tsa = [&](int k) { return Tp[k] - (1.0 - G.D * zk(k)); };
         double g0 = (-3.0 * tsa(0) + 4.0 * tsa(1) - tsa(2)) / (2.0 * G.dz);
         double g1 = (3.0 * tsa(nz - 1) - 4.0 * tsa(nz - 2) + tsa(nz - 3)) / (2.0 * G.dz);
+        if (G.zt) {
+            // derivative at the plate of the quadratic through the plate node and its two neighbours at distances
+            // h1 < h2: weights (-(b + c), b, c), b = h2 / (h1 (h2 - h1)), c = -h1 / (h2 (h2 - h1))
+            double h1 = zk(1) - zk(0), h2 = zk(2) - zk(0);
+            double b = h2 / (h1 * (h2 - h1)), c = -h1 / (h2 * (h2 - h1));
+            g0 = -(b + c) * tsa(0) + b * tsa(1) + c * tsa(2);
+            h1 = zk(nz - 1) - zk(nz - 2); h2 = zk(nz - 1) - zk(nz - 3);
+            b = h2 / (h1 * (h2 - h1)); c = -h1 / (h2 * (h2 - h1));
+            g1 = (b + c) * tsa(nz - 1) - b * tsa(nz - 2) - c * tsa(nz - 3);
+        }
         nu0 = -g0 / G.eps; nu1 = -g1 / G.eps;
     }
     o[3] = nu0; o[4] = nu1; o[5] = 0.5 * (nu0 + nu1);                  // Eq. 24

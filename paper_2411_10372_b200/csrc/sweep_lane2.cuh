@@ -46,10 +46,12 @@ MC_DEV void nbr_left(double vA, double vB, double &lA, double &lB)
 // FWD: dir = +1 (compile time: the pair's halves are swapped for dir = -1).  The fast loop is unrolled by
 // MC_LANE2_UNROLL so that most of the register pipeline's rotation needs no moves (6 = lcm of the rotation
 // periods removes them all, but measured 2 < 3 < 6 in time: 0.83 / 0.87 / 0.88 ms on C3).
-template <int WARPS, bool WALL_M, int TVD, bool REDUCE, int MINB, bool FWD>
+// ZS: non-uniform z grid (R19; SweepArgs::zt): z is the marching direction, i.e. the cross direction of this sweep.
+template <int WARPS, bool WALL_M, int TVD, bool REDUCE, int MINB, bool FWD, bool ZS = false>
 MC_KERNEL void __launch_bounds__(32 * WARPS, MINB) k_lane2(SweepArgs A)
 {
     constexpr int ND = 2, NF = 4, CA = 0, CM = 1;
+    static_assert(!ZS || WALL_M, "the non-uniform z grid lies between plates");
     const int lane = threadIdx.x;
     const int xtile = (int)blockIdx.x * WARPS + (int)threadIdx.y;
     const int gx0 = xtile * LANE2_OUT;
@@ -78,7 +80,7 @@ MC_KERNEL void __launch_bounds__(32 * WARPS, MINB) k_lane2(SweepArgs A)
     auto exists = [&](int l) MC_INL { return WALL_M ? (l >= 0 && l < n) : true; };
     auto is_plate = [&](int l) MC_INL { return WALL_M && (l == 0 || l == n - 1); };
     auto lev = [&](int l) MC_INL { return WALL_M ? l : wrap1(l, n); };
-    auto gz_of = [&](int l) MC_INL { return A.g * ((double)lev(l) * A.dz); };
+    auto gz_of = [&](int l) MC_INL { return ZS ? zt_gz(A, clampk(l, n)) : A.g * ((double)lev(l) * A.dz); };
     auto off_of = [&](int l) MC_INL { return off_base + (unsigned)lev(l) * sm; };
     auto load_at = [&](unsigned o, double (&X)[2][NF]) MC_INL {
 #pragma unroll
@@ -142,7 +144,7 @@ MC_KERNEL void __launch_bounds__(32 * WARPS, MINB) k_lane2(SweepArgs A)
         Prim<ND> w2[2] = {w1[0], w1[1]};
         double hC2[2] = {0.0, 0.0}, gz2 = 0.0;
         if (ex2) {
-            gz2 = FAST ? A.g * (kd2c * A.dz) : gz_of(j + 2);
+            gz2 = (FAST && !ZS) ? A.g * (kd2c * A.dz) : gz_of(j + 2);
 #pragma unroll
             for (int P = 0; P < 2; ++P) {
                 w2[P] = primitives<ND>(Xn[P], gz2, A);
@@ -170,6 +172,7 @@ MC_KERNEL void __launch_bounds__(32 * WARPS, MINB) k_lane2(SweepArgs A)
                 for (int c = 0; c < ND; ++c) { du[c] = uR[P][c] - w1[P].u[c]; dxa[c] = 0.0; dxc[c] = 0.0; }
                 dxa[CM] = w2[P].u[CA] - um0[P][0];
                 dxc[CM] = w2[P].u[CM] - um0[P][1];
+                if (ZS) { const double sz = zt_icz(A, clampk(j + 1, n)); dxa[CM] *= sz; dxc[CM] *= sz; }   // / (z_{k+1} - z_{k-1})
                 flux<ND, CA>(X1[P], w1[P], du, TR[P] - w1[P].T, dxa, dxc, A, F1[P]);
             }
 #pragma unroll
@@ -203,6 +206,7 @@ MC_KERNEL void __launch_bounds__(32 * WARPS, MINB) k_lane2(SweepArgs A)
                     for (int c = 0; c < ND; ++c) { du[c] = wP0[P].u[c] - uL[P][c]; dxa[c] = 0.0; dxc[c] = 0.0; }
                     dxa[CM] = wP1[P].u[CA] - uPm[P][0];
                     dxc[CM] = wP1[P].u[CM] - uPm[P][1];
+                    if (ZS) { const double sz = zt_icz(A, clampk(j, n)); dxa[CM] *= sz; dxc[CM] *= sz; }
                     flux<ND, CA>(XP0[P], wP0[P], du, wP0[P].T - TL[P], dxa, dxc, A, FP0[P]);
                 }
 #pragma unroll
@@ -260,7 +264,8 @@ MC_KERNEL void __launch_bounds__(32 * WARPS, MINB) k_lane2(SweepArgs A)
             if (REDUCE) {                                        // CFL max-reduction of the new state (R12)
                 const bool need = owner && !(cfl_can_skip<ND>(o[0], gz0, smax2, A) && cfl_can_skip<ND>(o[1], gz0, smax2, A));
                 if (__any_sync(0xffffffffu, need)) {             // rare once the running maximum has settled
-                    const double s = fmax_nan(cfl_speed<ND>(o[0], gz0, A), cfl_speed<ND>(o[1], gz0, A));
+                    const double idz = ZS ? zt_icfl(A, clampk(j, n)) : -1.0;
+                    const double s = fmax_nan(cfl_speed<ND>(o[0], gz0, A, idz), cfl_speed<ND>(o[1], gz0, A, idz));
                     if (owner) { smax = fmax_nan(smax, s); smax2 = fmax_nan(smax2, (smax * smax) * (1.0 - 1e-6)); }
                 }
             }

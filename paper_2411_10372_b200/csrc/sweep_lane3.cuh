@@ -26,7 +26,8 @@ namespace mc {
 // CB: velocity component of the tile's second direction b (y); CM: component of the marching
 // direction m (z); WB: warps (rows) per block; WALL_M: m is z with plates; TVD: -1 / 0 / 1 as in
 // k_march; REDUCE: fold the CFL max-reduction of the output into the epilogue (R12).  alpha is x.
-template <int CB, int CM, int WB, bool WALL_M, int TVD, bool REDUCE>
+// ZS: non-uniform z grid (R19; SweepArgs::zt): z is the marching direction, a cross direction of this sweep.
+template <int CB, int CM, int WB, bool WALL_M, int TVD, bool REDUCE, bool ZS = false>
 MC_KERNEL void __maxnreg__(((65536 / (32 * WB)) / 8 * 8) > 248 ? 248 : ((65536 / (32 * WB)) / 8 * 8)) k_lane3(SweepArgs A)
 {
     constexpr int ND = 3, NF = 5;
@@ -74,7 +75,7 @@ MC_KERNEL void __maxnreg__(((65536 / (32 * WB)) / 8 * 8) > 248 ? 248 : ((65536 /
     auto exists = [&](int l) MC_INL { return WALL_M ? (l >= 0 && l < n) : true; };
     auto is_plate = [&](int l) MC_INL { return WALL_M && (l == 0 || l == n - 1); };
     auto lev = [&](int l) MC_INL { return WALL_M ? l : wrap1(l, n); };
-    auto gz_of = [&](int l) MC_INL { return A.g * ((double)lev(l) * A.dz); };       // m is z
+    auto gz_of = [&](int l) MC_INL { return ZS ? zt_gz(A, clampk(l, n)) : A.g * ((double)lev(l) * A.dz); };       // m is z
     auto load_at = [&](unsigned o, double (&X)[NF]) MC_INL {
 #pragma unroll
         for (int f = 0; f < NF; ++f) X[f] = inb[f][o];
@@ -157,7 +158,7 @@ MC_KERNEL void __maxnreg__(((65536 / (32 * WB)) / 8 * 8) > 248 ? 248 : ((65536 /
         Prim<ND> w2 = w1;
         double hC2 = 0.0, gz2 = 0.0;
         if (ex2) {
-            gz2 = FAST ? A.g * (kd2c * A.dz) : gz_of(j + 2);
+            gz2 = (FAST && !ZS) ? A.g * (kd2c * A.dz) : gz_of(j + 2);
             w2 = primitives<ND>(Xn, gz2, A);
             if (ROLE == LROLE_IN && TVD >= 0) hC2 = half_courant_coef(w2.u[CA], w2.T, half_tod, A);
             publish(slotU, p0, w2.u);                   // parity of level j+2
@@ -184,6 +185,7 @@ MC_KERNEL void __maxnreg__(((65536 / (32 * WB)) / 8 * 8) > 248 ? 248 : ((65536 /
             const double dT = __shfl_down_sync(0xffffffffu, w1.T, 1) - w1.T;
             dxa[CM] = w2.u[CA] - um0[0];
             dxc[CM] = w2.u[CM] - um0[1];
+            if (ZS) { const double sz = zt_icz(A, clampk(j + 1, n)); dxa[CM] *= sz; dxc[CM] *= sz; }   // / (z_{k+1} - z_{k-1})
             cross_b(slotU, p1, dxa, dxc);
             flux<ND, CA>(X1, w1, du, dT, dxa, dxc, A, F1);
             shfl_up_vec<NF>(F1, Fm);
@@ -211,6 +213,7 @@ MC_KERNEL void __maxnreg__(((65536 / (32 * WB)) / 8 * 8) > 248 ? 248 : ((65536 /
                     const double dT = wP0.T - __shfl_up_sync(0xffffffffu, wP0.T, 1);
                     dxa[CM] = wP1.u[CA] - uPm[0];
                     dxc[CM] = wP1.u[CM] - uPm[1];
+                    if (ZS) { const double sz = zt_icz(A, clampk(j, n)); dxa[CM] *= sz; dxc[CM] *= sz; }
                     cross_b(slotP, p0, dxa, dxc);
                     flux<ND, CA>(XP0, wP0, du, dT, dxa, dxc, A, FP0);
                     shfl_down_vec<NF>(FP0, FPp);
@@ -250,7 +253,7 @@ MC_KERNEL void __maxnreg__(((65536 / (32 * WB)) / 8 * 8) > 248 ? 248 : ((65536 /
                     const double gzj = gz0;
                     const bool need = owner && !cfl_can_skip<ND>(o, gzj, smax2, A);
                     if (__any_sync(0xffffffffu, need)) {             // rare once the running maximum has settled
-                        const double s = cfl_speed<ND>(o, gzj, A);
+                        const double s = cfl_speed<ND>(o, gzj, A, ZS ? zt_icfl(A, clampk(j, n)) : -1.0);
                         if (owner) { smax = fmax_nan(smax, s); smax2 = fmax_nan(smax2, (smax * smax) * (1.0 - 1e-6)); }
                     }
                 }

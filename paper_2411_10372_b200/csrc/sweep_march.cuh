@@ -38,12 +38,14 @@ enum { ROLE_NONE = 0, ROLE_R2 = 1, ROLE_WALLROW = 2, ROLE_R1 = 3, ROLE_IN = 4 };
 // CA: velocity component of alpha; CB: velocity component of the tile's second direction b (-1 in 2-D);
 // WX x WB: threads of a block (WB = 1 in 2-D); WALL_M / WALL_B: the marching / second direction is z
 // with plates; TVD: -1 no TVD term, 0 Eq. 34 as printed, 1 Davis/Yee (R4).
-template <int ND, int CA, int CB, int WX, int WB, bool WALL_M, bool WALL_B, int TVD, int MINB = 1>
+// ZS: non-uniform z grid (R19 / R20; SweepArgs::zt), z being the sweep axis.
+template <int ND, int CA, int CB, int WX, int WB, bool WALL_M, bool WALL_B, int TVD, int MINB = 1, bool ZS = false>
 MC_KERNEL void __launch_bounds__(WX * WB, MINB) k_march(SweepArgs A)
 {
     constexpr int NF = ND + 2;
     constexpr bool HAS_B = (CB >= 0);
     constexpr bool Z_IS_ALPHA = (CA == ND - 1);      // z is the last velocity component
+    static_assert(!ZS || (Z_IS_ALPHA && WALL_M && !HAS_B), "k_march serves the non-uniform grid as the 2-D z-sweep between plates");
     constexpr int TILE = WX * WB;
     constexpr int cb = HAS_B ? CB : 0;
     MC_SHARED_DECL(double, smem_raw);
@@ -108,8 +110,10 @@ MC_KERNEL void __launch_bounds__(WX * WB, MINB) k_march(SweepArgs A)
     auto lev = [&](int l) MC_INL { return WALL_M ? l : wrap1(l, n); };              // l in [-n, 2n)
     auto off_of = [&](int l) MC_INL { return off_base + (unsigned)lev(l) * sms; };
     auto phys_k = [&](int l) MC_INL { const int w = lev(l); return (A.dir > 0) ? w : n - 1 - w; };
+    auto kz = [&](int l) MC_INL { return clampk((A.dir > 0) ? l : n - 1 - l, n); }; // ZS: z index of level l (clamped: values beyond a plate are unused)
     auto gz_of = [&](int l) MC_INL {                         // g z_k of Eq. 17 for this thread's node at level l
         if (!Z_IS_ALPHA) return gz_fixed;
+        if (ZS) return zt_gz(A, kz(l));
         return A.g * ((double)phys_k(l) * A.dz);
     };
     auto load_at = [&](unsigned o, double (&X)[NF]) MC_INL {
@@ -145,7 +149,7 @@ MC_KERNEL void __launch_bounds__(WX * WB, MINB) k_march(SweepArgs A)
         X[0] = rho;
 #pragma unroll
         for (int c = 0; c < ND; ++c) X[1 + c] = 0.0;
-        X[NF - 1] = rho * (A.cv * Tw + A.g * ((double)k * A.dz));
+        X[NF - 1] = rho * (A.cv * Tw + (ZS ? zt_gz(A, k) : A.g * ((double)k * A.dz)));
     };
 
     // ---- carried state (levels relative to the current output level j) -------------------------
@@ -202,14 +206,28 @@ MC_KERNEL void __launch_bounds__(WX * WB, MINB) k_march(SweepArgs A)
         }
 #endif
         auto advance = [&]() MC_INL { if (FAST) { o3c += sms; o0c += sms; kd2c += dsgn; } };
+        // ZS (R19): the outer differences of levels j and j+1 use the height of the node's cell (a plate's half cell
+        // carries the factor 2 of R10), the inner one-sided differences the spacing across the face, the TVD flux of
+        // face (j, j+1) is weighted by h / dzc (R20).  Uniform grid: the launch constants.
+        double cdt1 = cdt, hcdt1 = hcdt, hcdt0 = hcdt, cw1 = 2.0 * cdt, cw0 = cdt, htod2 = half_tod;
+        double sF = 1.0, sB = 1.0, tw0 = 1.0, tw1 = 1.0;
+        if (ZS) {
+            const int k0 = kz(j), k1 = kz(j + 1), k2 = kz(j + 2);
+            const double idc0 = zt_idc(A, k0), idc1 = zt_idc(A, k1), hf01 = zt_hf(A, min(k0, k1));
+            cdt1 = (tau * dsgn) * idc1; hcdt1 = 0.5 * cdt1; hcdt0 = (0.5 * tau * dsgn) * idc0;
+            cw1 = cdt1; cw0 = hcdt0;
+            htod2 = (0.5 * tau) * zt_idc(A, k2);
+            sF = zt_ihf(A, min(k1, k2)); sB = zt_ihf(A, min(k0, k1));
+            tw0 = hf01 * idc0; tw1 = hf01 * idc1;
+        }
 
         // (1) W(j+2): primitives, Courant coefficient, publish velocities
         Prim<ND> w2 = w1;
         double hC2 = 0.0, gz2 = 0.0;
         if (ld2) {
-            gz2 = (FAST && Z_IS_ALPHA) ? A.g * (kd2c * A.dz) : gz_of(j + 2);
+            gz2 = (FAST && Z_IS_ALPHA && !ZS) ? A.g * (kd2c * A.dz) : gz_of(j + 2);
             w2 = primitives<ND>(Xn, gz2, A);
-            if (ROLE == ROLE_IN && TVD >= 0) hC2 = half_courant_coef(w2.u[CA], w2.T, half_tod, A);
+            if (ROLE == ROLE_IN && TVD >= 0) hC2 = half_courant_coef(w2.u[CA], w2.T, htod2, A);
             publish(slotU, p2, w2.u);
         }
         if (ROLE == ROLE_R2) {
@@ -232,9 +250,9 @@ MC_KERNEL void __launch_bounds__(WX * WB, MINB) k_march(SweepArgs A)
         }
 
         // (2) TVD (Eqs. 34-39): Dh_{j+1/2} from dX_{j-1/2}, dX_{j+1/2}, dX_{j+3/2}
-        double d1[NF], Dh[NF], a1 = 0.0, b1 = 0.0;
+        double d1[NF], Dh[NF], Dh1[NF], a1 = 0.0, b1 = 0.0;       // Dh1: the same flux as level j+1 sees it (ZS: other weight)
 #pragma unroll
-        for (int f = 0; f < NF; ++f) { Dh[f] = 0.0; d1[f] = 0.0; }
+        for (int f = 0; f < NF; ++f) { Dh[f] = 0.0; Dh1[f] = 0.0; d1[f] = 0.0; }
         if (ROLE == ROLE_IN && TVD >= 0) {
 #pragma unroll
             for (int f = 0; f < NF; ++f) d1[f] = (ld1 && ld2) ? Xn[f] - Xc[f] : 0.0;
@@ -244,7 +262,10 @@ MC_KERNEL void __launch_bounds__(WX * WB, MINB) k_march(SweepArgs A)
             if (have) {
                 const double coef = tvd_coef<(TVD >= 0 ? TVD : 0)>(a0, a1, b0, hC0, hC1);
 #pragma unroll
-                for (int f = 0; f < NF; ++f) { Dh[f] = coef * d0[f]; H0[f] += Dh[f]; }
+                for (int f = 0; f < NF; ++f) {
+                    Dh[f] = (ZS ? coef * tw0 : coef) * d0[f]; H0[f] += Dh[f];
+                    Dh1[f] = ZS ? (coef * tw1) * d0[f] : Dh[f];
+                }
             }
         }
 
@@ -260,9 +281,9 @@ MC_KERNEL void __launch_bounds__(WX * WB, MINB) k_march(SweepArgs A)
             } else {
                 double du[ND], dxa[ND], dxc[ND];
 #pragma unroll
-                for (int c = 0; c < ND; ++c) du[c] = w2.u[c] - w1.u[c];
+                for (int c = 0; c < ND; ++c) du[c] = ZS ? (w2.u[c] - w1.u[c]) * sF : w2.u[c] - w1.u[c];
                 cross(slotU, p1, dxa, dxc);
-                flux<ND, CA>(Xc, w1, du, w2.T - w1.T, dxa, dxc, A, F1);
+                flux<ND, CA>(Xc, w1, du, ZS ? (w2.T - w1.T) * sF : w2.T - w1.T, dxa, dxc, A, F1);
             }
         }
         // (4) P(j+1): predictor (Eq. 31), plate values, primitives of X^P, publish
@@ -271,13 +292,13 @@ MC_KERNEL void __launch_bounds__(WX * WB, MINB) k_march(SweepArgs A)
             if (start_wall1) {
                 plate(j + 1, Xc[0], XP);                                      // rho unchanged
             } else if (end_wall1) {
-                plate(j + 1, Xc[0] - 2.0 * cdt * (F1[0] - F0[0]), XP);       // half-cell closure (R10)
+                plate(j + 1, Xc[0] - cw1 * (F1[0] - F0[0]), XP);             // half-cell closure (R10): 2 tau / dz
             } else {
 #pragma unroll
                 for (int f = 0; f < NF; ++f) {
                     const double dF = F1[f] - F0[f];
-                    XP[f] = fma(-cdt, dF, Xc[f]);
-                    H1[f] = fma(-hcdt, dF, Xc[f]) - Dh[f];                    // (X^P + X)/2 - Dh
+                    XP[f] = fma(-cdt1, dF, Xc[f]);
+                    H1[f] = fma(-hcdt1, dF, Xc[f]) - Dh1[f];                  // (X^P + X)/2 - Dh
                 }
                 XP[1 + CA] = fma(tsrc, Xc[0], XP[1 + CA]);
                 H1[1 + CA] = fma(0.5 * tsrc, Xc[0], H1[1 + CA]);
@@ -306,21 +327,21 @@ MC_KERNEL void __launch_bounds__(WX * WB, MINB) k_march(SweepArgs A)
                 } else {
                     double du[ND], dxa[ND], dxc[ND];
 #pragma unroll
-                    for (int c = 0; c < ND; ++c) du[c] = wP1.u[c] - uP0[c];
+                    for (int c = 0; c < ND; ++c) du[c] = ZS ? (wP1.u[c] - uP0[c]) * sB : wP1.u[c] - uP0[c];
                     cross(slotP, p1, dxa, dxc);
-                    flux<ND, CA>(XP, wP1, du, wP1.T - TP0, dxa, dxc, A, FP1);
+                    flux<ND, CA>(XP, wP1, du, ZS ? (wP1.T - TP0) * sB : wP1.T - TP0, dxa, dxc, A, FP1);
                 }
             }
             // (6) out(j): corrector (Eq. 32), average and TVD term (Eq. 33), plate values
             if (FAST || (j >= l0 && exists(j))) {
                 double o[NF];
                 if (!FAST && WALL_M && j == 0) {
-                    plate(j, H0[0] - cdt * (FP1[0] - FP0[0]), o);            // 0.5 * (2 tau/dz) * dF
+                    plate(j, H0[0] - cw0 * (FP1[0] - FP0[0]), o);            // 0.5 * (2 tau/dz) * dF
                 } else if (!FAST && WALL_M && j == n - 1) {
                     plate(j, H0[0], o);
                 } else {
 #pragma unroll
-                    for (int f = 0; f < NF; ++f) o[f] = fma(-hcdt, FP1[f] - FP0[f], H0[f]);
+                    for (int f = 0; f < NF; ++f) o[f] = fma(-hcdt0, FP1[f] - FP0[f], H0[f]);
                 }
                 if (owner) store_at(o0, o);
             }

@@ -61,11 +61,14 @@ constexpr int MARCH3_STAGES = MC_MARCH3_STAGES;      // power of two
 __host__ __device__ constexpr size_t tile3_stage_bytes(int WB) { return (size_t)5 * 32 * (WB + 2) * sizeof(double); }
 __host__ __device__ constexpr size_t tile3_async_bytes(int WB) { return MARCH3_STAGES * tile3_stage_bytes(WB) + 8 * (2 * MARCH3_STAGES + 2 * WB); }
 
-template <int CA, int CB, int WB, bool WALL_M, bool WALL_B, int TVD, int MINB = 1, bool AS = false>
+// ZS: non-uniform z grid (R19 / R20; SweepArgs::zt): z is the sweep axis (L_z) or the tile's second direction (L_y).
+template <int CA, int CB, int WB, bool WALL_M, bool WALL_B, int TVD, int MINB = 1, bool AS = false, bool ZS = false>
 MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A, const __grid_constant__ CUtensorMap tmap)
 {
     constexpr int ND = 3, NF = 5;
     constexpr bool Z_IS_ALPHA = (CA == ND - 1);
+    constexpr bool ZA = ZS && Z_IS_ALPHA;             // the metric varies along the march
+    static_assert(!ZS || (Z_IS_ALPHA ? WALL_M : (WALL_B && CB == ND - 1)), "the non-uniform z grid lies between plates");
     constexpr int OB = WB - 2;                        // output rows per tile
     static_assert(WB >= 3 && WB % 4 == 0, "the SM allocates warps in fours: other row counts waste registers");
     constexpr int TILE = 32 * (WB + 2);               // shared-memory plane: tile rows plus the ring-2 rows
@@ -137,7 +140,8 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A, const __grid_co
     const unsigned off_base_o = (unsigned)(col_o + org);
     const double dsgn = (A.dir > 0) ? 1.0 : -1.0;
     const int pf_last = min(l1 + 1, n - 1) - MC_MARCH3_L2PF;                // last j + 3 whose L2 prefetch is issued
-    const double gz_fixed = A.g * ((double)gb * A.dz);                       // used when b is z
+    const double gz_fixed = (ZS && !Z_IS_ALPHA) ? zt_gz(A, gb) : A.g * ((double)gb * A.dz);   // used when b is z
+    const double szb = (ZS && !Z_IS_ALPHA) ? zt_icz(A, gb) : 1.0;            // 1 / (z_{k+1} - z_{k-1}) of this thread's row
 
     auto exists = [&](int l) MC_INL { return WALL_M ? (l >= 0 && l < n) : true; };
     auto lev = [&](int l) MC_INL { return WALL_M ? l : wrap1(l, n); };              // l in [-n, 2n)
@@ -152,8 +156,10 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A, const __grid_co
         for (int f = 0; f < NF; ++f) X[f] = inb[f][o];
     };
     auto load = [&](int l, double (&X)[NF]) MC_INL { load_at(off_of(l), X); };
+    auto kz = [&](int l) MC_INL { return clampk((A.dir > 0) ? l : n - 1 - l, n); }; // ZA: z index of level l (clamped: values beyond a plate are unused)
     auto gz_of = [&](int l) MC_INL {                         // g z_k of Eq. 17 for this thread's node at level l
         if (!Z_IS_ALPHA) return gz_fixed;
+        if (ZA) return zt_gz(A, kz(l));
         return A.g * ((double)phys_k(l) * A.dz);
     };
     // L2 prefetch of the thread's node at level l (no register, no scoreboard): hides the HBM latency
@@ -183,6 +189,7 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A, const __grid_co
         dxc[0] = s[1] - s[-1];
         dxa[CB] = s[CA * TILE + 32] - s[CA * TILE - 32];
         dxc[CB] = s[CB * TILE + 32] - s[CB * TILE - 32];
+        if (ZS && !Z_IS_ALPHA) { dxa[CB] *= szb; dxc[CB] *= szb; }
     };
     // plate values of a node on a plate of the marching direction: no slip,
     // T = T_w; only rho is free (R10)
@@ -192,7 +199,7 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A, const __grid_co
         X[0] = rho;
 #pragma unroll
         for (int c = 0; c < ND; ++c) X[1 + c] = 0.0;
-        X[NF - 1] = rho * (A.cv * Tw + A.g * ((double)k * A.dz));
+        X[NF - 1] = rho * (A.cv * Tw + (ZA ? zt_gz(A, k) : A.g * ((double)k * A.dz)));
     };
 
 
@@ -306,11 +313,11 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A, const __grid_co
 
     // W(L): primitives of X(L) (in `X`), Courant coefficient, velocities published into slot uslot(L);
     // a ring-1 row also publishes the velocities of its ring-2 neighbour row (from `Xo`).
-    auto stage_W = [&](auto role_tag, int par, double gz, const double (&X)[NF], const double (&Xo)[ND + 1],
+    auto stage_W = [&](auto role_tag, int par, double gz, double htod, const double (&X)[NF], const double (&Xo)[ND + 1],
                        Prim<ND> &w, double &hC) MC_INL {
         constexpr int ROLE = decltype(role_tag)::value;
         w = primitives<ND>(X, gz, A);
-        if (ROLE == ROLE_IN && TVD >= 0) hC = half_courant_coef(w.u[CA], w.T, half_tod, A);
+        if (ROLE == ROLE_IN && TVD >= 0) hC = half_courant_coef(w.u[CA], w.T, htod, A);
         publish(slotU, par, tidx, w.u);
         if (ROLE == ROLE_R1) {
             const double inv = rcp_fast(Xo[0]);
@@ -339,6 +346,21 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A, const __grid_co
 
         if (ROLE == ROLE_NONE) { level_sync(); return; }          // (AS: such rows have left already)
 
+        // ZA (R19): the outer differences of levels j and j+1 use the height of the node's cell (a plate's half cell
+        // carries the factor 2 of R10), the inner one-sided differences the spacing across the face, the TVD flux of
+        // face (j, j+1) is weighted by h / dzc (R20).  Uniform grid: the launch constants.
+        double cdt1 = cdt, hcdt1 = hcdt, hcdt0 = hcdt, cw1 = 2.0 * cdt, cw0 = cdt, htod2 = half_tod;
+        double sF = 1.0, sB = 1.0, tw0 = 1.0, tw1 = 1.0;
+        if (ZA) {
+            const int k0 = kz(j), k1 = kz(j + 1), k2 = kz(j + 2);
+            const double idc0 = zt_idc(A, k0), idc1 = zt_idc(A, k1), hf01 = zt_hf(A, min(k0, k1));
+            cdt1 = (tau * dsgn) * idc1; hcdt1 = 0.5 * cdt1; hcdt0 = (0.5 * tau * dsgn) * idc0;
+            cw1 = cdt1; cw0 = hcdt0;
+            htod2 = (0.5 * tau) * zt_idc(A, k2);
+            sF = zt_ihf(A, min(k1, k2)); sB = zt_ihf(A, min(k0, k1));
+            tw0 = hf01 * idc0; tw1 = hf01 * idc1;
+        }
+
         // (0) not AS: prefetch X(j+3) into registers and X(j+3+MC_MARCH3_L2PF) into L2;  AS: take X(j+2) out of its stage
         const bool ld3 = FAST || (ex3 && j + 3 <= l1 + 1);
         double Xq[NF], Xoq[ND + 1];
@@ -361,8 +383,8 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A, const __grid_co
         Prim<ND> w2 = w1;
         double hC2 = 0.0, gz2 = 0.0;
         if (ld2) {
-            gz2 = (FAST && Z_IS_ALPHA) ? A.g * (kd2c * A.dz) : gz_of(j + 2);
-            stage_W(role_tag, p2, gz2, Xn, Xon, w2, hC2);
+            gz2 = (FAST && Z_IS_ALPHA && !ZS) ? A.g * (kd2c * A.dz) : gz_of(j + 2);
+            stage_W(role_tag, p2, gz2, htod2, Xn, Xon, w2, hC2);
         }
 
         if (ROLE == ROLE_WALLROW) {
@@ -379,9 +401,9 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A, const __grid_co
         }
 
         // (2) TVD (Eqs. 34-39): Dh_{j+1/2} from dX_{j-1/2}, dX_{j+1/2}, dX_{j+3/2}
-        double d1[NF], Dh[NF], a1 = 0.0, b1 = 0.0;
+        double d1[NF], Dh[NF], Dh1[NF], a1 = 0.0, b1 = 0.0;       // Dh1: the same flux as level j+1 sees it (ZA: other weight)
 #pragma unroll
-        for (int f = 0; f < NF; ++f) { Dh[f] = 0.0; d1[f] = 0.0; }
+        for (int f = 0; f < NF; ++f) { Dh[f] = 0.0; Dh1[f] = 0.0; d1[f] = 0.0; }
         if (ROLE == ROLE_IN && TVD >= 0) {
 #pragma unroll
             for (int f = 0; f < NF; ++f) d1[f] = (ld1 && ld2) ? Xn[f] - Xc[f] : 0.0;
@@ -391,7 +413,10 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A, const __grid_co
             if (have) {
                 const double coef = tvd_coef<(TVD >= 0 ? TVD : 0)>(a0, a1, b0, hC0, hC1);
 #pragma unroll
-                for (int f = 0; f < NF; ++f) { Dh[f] = coef * d0[f]; H0[f] += Dh[f]; }
+                for (int f = 0; f < NF; ++f) {
+                    Dh[f] = (ZA ? coef * tw0 : coef) * d0[f]; H0[f] += Dh[f];
+                    Dh1[f] = ZA ? (coef * tw1) * d0[f] : Dh[f];
+                }
             }
         }
 
@@ -407,9 +432,9 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A, const __grid_co
             } else {
                 double du[ND], dxa[ND], dxc[ND];
 #pragma unroll
-                for (int c = 0; c < ND; ++c) du[c] = w2.u[c] - w1.u[c];
+                for (int c = 0; c < ND; ++c) du[c] = ZA ? (w2.u[c] - w1.u[c]) * sF : w2.u[c] - w1.u[c];
                 cross(slotU, p1, dxa, dxc);
-                flux<ND, CA>(Xc, w1, du, w2.T - w1.T, dxa, dxc, A, F1);
+                flux<ND, CA>(Xc, w1, du, ZA ? (w2.T - w1.T) * sF : w2.T - w1.T, dxa, dxc, A, F1);
             }
         }
         // (4) P(j+1): predictor (Eq. 31), plate values, primitives of X^P, publish
@@ -418,13 +443,13 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A, const __grid_co
             if (start_wall1) {
                 plate(j + 1, Xc[0], XP);                                      // rho unchanged
             } else if (end_wall1) {
-                plate(j + 1, Xc[0] - 2.0 * cdt * (F1[0] - F0[0]), XP);       // half-cell closure (R10)
+                plate(j + 1, Xc[0] - cw1 * (F1[0] - F0[0]), XP);             // half-cell closure (R10): 2 tau / dz
             } else {
 #pragma unroll
                 for (int f = 0; f < NF; ++f) {
                     const double dF = F1[f] - F0[f];
-                    XP[f] = fma(-cdt, dF, Xc[f]);
-                    H1[f] = fma(-hcdt, dF, Xc[f]) - Dh[f];                    // (X^P + X)/2 - Dh
+                    XP[f] = fma(-cdt1, dF, Xc[f]);
+                    H1[f] = fma(-hcdt1, dF, Xc[f]) - Dh1[f];                  // (X^P + X)/2 - Dh
                 }
                 if (Z_IS_ALPHA) {
                     XP[1 + CA] = fma(tsrc, Xc[0], XP[1 + CA]);
@@ -455,9 +480,9 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A, const __grid_co
                 } else {
                     double du[ND], dxa[ND], dxc[ND];
 #pragma unroll
-                    for (int c = 0; c < ND; ++c) du[c] = wP1.u[c] - uP0[c];
+                    for (int c = 0; c < ND; ++c) du[c] = ZA ? (wP1.u[c] - uP0[c]) * sB : wP1.u[c] - uP0[c];
                     cross(slotP, p1, dxa, dxc);
-                    flux<ND, CA>(XP, wP1, du, wP1.T - TP0, dxa, dxc, A, FP1);
+                    flux<ND, CA>(XP, wP1, du, ZA ? (wP1.T - TP0) * sB : wP1.T - TP0, dxa, dxc, A, FP1);
                 }
             }
             // (6) out(j): corrector (Eq. 32), average and TVD term (Eq. 33), plate values.  H0 already
@@ -465,17 +490,17 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A, const __grid_co
             if (FAST || (j >= l0 && exists(j))) {
                 double o[NF];
                 if (!FAST && WALL_M && j == 0) {
-                    plate(j, H0[0] - cdt * FP1[0], o);    // 0.5 (2 tau/dz) (F^P(1) - F^P(0)); the plate's own mass flux is 0
+                    plate(j, H0[0] - cw0 * FP1[0], o);    // 0.5 (2 tau/dz) (F^P(1) - F^P(0)); the plate's own mass flux is 0
                 } else if (!FAST && WALL_M && j == n - 1) {
                     plate(j, H0[0], o);
                 } else {
 #pragma unroll
-                    for (int f = 0; f < NF; ++f) o[f] = fma(-hcdt, FP1[f], H0[f]);
+                    for (int f = 0; f < NF; ++f) o[f] = fma(-hcdt0, FP1[f], H0[f]);
                 }
                 if (owner) store_at(o0, o);
             }
 #pragma unroll
-            for (int f = 0; f < NF; ++f) { H1[f] = fma(hcdt, FP1[f], H1[f]); d0[f] = d1[f]; }
+            for (int f = 0; f < NF; ++f) { H1[f] = fma(hcdt1, FP1[f], H1[f]); d0[f] = d1[f]; }
             a0 = a1; b0 = b1; hC0 = hC1; hC1 = hC2;
 #pragma unroll
             for (int c = 0; c < ND; ++c) uP0[c] = wP1.u[c];

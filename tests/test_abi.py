@@ -70,9 +70,16 @@ def test_init_rejects_bad_arguments_before_touching_the_device(lib):
     h = C.c_void_p()
     assert lib.mc_tvd_init(C.byref(g), C.byref(p), None, None, 0, None, C.byref(h)) == -1      # NULL buffers
     assert lib.mc_tvd_init(C.byref(g), C.byref(p), None, None, 0, None, None) == -1            # NULL out
-    z = (C.c_double * 16)()
-    g.z_nodes = C.cast(z, C.POINTER(C.c_double))
-    assert lib.mc_tvd_init(C.byref(g), C.byref(p), None, None, 0, None, C.byref(h)) == -5      # tanh grid: unsupported
+    z = (C.c_double * 16)()                                                                    # node heights all zero:
+    g.z_nodes = C.cast(z, C.POINTER(C.c_double))                                               # not increasing
+    assert lib.mc_tvd_init(C.byref(g), C.byref(p), None, None, 0, None, C.byref(h)) == -1
+    assert b"increasing" in lib.mc_tvd_last_error()
+    assert lib.mc_tvd_workspace_bytes(C.byref(g), C.byref(p)) == 0
+    for k in range(16):
+        z[k] = k / 15.0
+    assert lib.mc_tvd_workspace_bytes(C.byref(g), C.byref(p)) > 0                              # a valid non-uniform grid
+    pz = binding.make_params(inputs.make_params(bc_z=1))
+    assert lib.mc_tvd_workspace_bytes(C.byref(g), C.byref(pz)) == 0                            # node heights need plates
     assert lib.mc_tvd_step(None, 1) == -1
     assert lib.mc_tvd_debug_set_chunk(None, 4) == -1
     assert lib.mc_tvd_sweep(None, 0, 1, 0.1) == -1
