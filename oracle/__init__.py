@@ -64,6 +64,13 @@ class _Stats(C.Structure):
                 ("re", C.c_double), ("u_rms", C.c_double), ("nu_bar_sq", C.c_double), ("re_sq", C.c_double)]
 
 
+class _Forces(C.Structure):
+    _fields_ = [(n, C.c_double) for n in ("Fn_mean", "Fp_mean", "Fb_mean", "Fv_mean", "Fn_rms", "Fp_rms", "Fb_rms",
+                                          "Fv_rms", "FbFp_mean", "max_mach", "max_r", "volume")]
+
+
+HIST_BINS = 128
+
 _lib = None
 
 
@@ -85,6 +92,8 @@ def lib():
         L.orc_step_stats.restype = C.c_int
         L.orc_step_stats.argtypes = [C.POINTER(_Grid), C.POINTER(_Params), dp, C.c_int, C.c_int, dp,
                                      C.POINTER(_Stats), dp, dp, dp]
+        L.orc_flow_stats.restype = C.c_int
+        L.orc_flow_stats.argtypes = [C.POINTER(_Grid), C.POINTER(_Params), dp, C.POINTER(_Forces), C.POINTER(C.c_longlong)]
         L.orc_coefficients.restype = C.c_int
         L.orc_coefficients.argtypes = [C.POINTER(_Grid), C.POINTER(_Params), dp]
         _lib = L
@@ -202,6 +211,18 @@ def step_stats(prob: Problem, X: np.ndarray, n_steps: int, every: int = 1, dt_in
     if rc:
         raise ValueError(f"orc_step_stats failed: {rc}")
     return X, {n: getattr(st, n) for n, _ in _Stats._fields_}, Tp, rp, pp
+
+
+def flow_stats(prob: Problem, X: np.ndarray):
+    """Returns (dict of the force-balance averages of Eqs. 40-43 and the extrema, histogram of r as int64[HIST_BINS])."""
+    X = _check(prob, X)
+    g, p = prob.c_grid(), prob.c_params()
+    f = _Forces()
+    hist = np.zeros(HIST_BINS, dtype=np.int64)
+    rc = lib().orc_flow_stats(C.byref(g), C.byref(p), _dp(X), C.byref(f), hist.ctypes.data_as(C.POINTER(C.c_longlong)))
+    if rc:
+        raise ValueError(f"orc_flow_stats failed: {rc}")
+    return {n: getattr(f, n) for n, _ in _Forces._fields_}, hist
 
 
 def coefficients(prob: Problem) -> dict:

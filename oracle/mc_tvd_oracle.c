@@ -574,6 +574,94 @@ int orc_step_stats(const orc_grid *g, const orc_params *p, double *X, int n_step
     return 0;
 }
 
+/* Flow statistics of Sec. 5-6 (instantaneous; the paper averages them over the steady state):
+ *  - the z-momentum balance terms (Eqs. 40-43)
+ *        F_n = rho (u . grad) u_z,  F_p = -d_z p,  F_b = rho g,  F_v = d_i tau_iz
+ *    with tau_ij of Eq. 18 (dilatation coefficient lambda, R3), so for constant mu
+ *        F_v = mu [ lap u_z + (1 + lambda) d_z (div u) ];
+ *    "we compute the volume averages of the above four terms, along with <F_b> - <F_p>";
+ *  - the ratio r = K_e / I_e = (rho u^2/2)/(rho C_v T) "at every grid point" and its distribution (PAPER.md:395,
+ *    Fig. 5); the local Mach number, of which the paper quotes the maximum, is the same number up
+ *    to a constant: Mach^2 = u^2/(gamma R T) = 2 r / (gamma (gamma - 1)).
+ * The paper does not say how it differences these post-processing quantities (reading R21): second-order central
+ * differences on the node's 3x3x3 neighbourhood (first derivatives over the distance between the two neighbours,
+ * second derivatives and mixed derivatives compact), evaluated at the INTERIOR nodes k = 1 .. nz-2 (all nodes when z
+ * is periodic) and averaged with the cell heights of R16 / R19; the means and the root-mean-squares are both given
+ * (the signed mean of F_n and F_v nearly cancels).  Histogram: r > 0 falls into bin 4 (floor(log2 r) + 32) +
+ * (top two mantissa bits), clamped to [0, 127] -- quarter-octave bins from 2^-32 to 1, read off the bit pattern of
+ * the double so that both implementations take the decision on the same number; r = 0 goes to bin 0. */
+static int hist_bin(double r)
+{
+    if (!(r > 0.0)) return 0;
+    unsigned long long bits;
+    memcpy(&bits, &r, sizeof(bits));
+    long b = (long)(bits >> 50) - 4L * (1023 - 32);      /* 11 exponent bits and 2 mantissa bits */
+    return b < 0 ? 0 : (b > ORC_HIST_BINS - 1 ? ORC_HIST_BINS - 1 : (int)b);
+}
+
+int orc_flow_stats(const orc_grid *g, const orc_params *p, const double *X, orc_forces *out, long long *hist_r)
+{
+    ctx c;
+    if (ctx_init(&c, g, p) || !out) return -1;
+    if (c.nx < 3 || c.nz < 3 || (c.ndim == 3 && c.ny < 3)) return -1;
+    double *zeros = arr(c.N), *q[5], *w[5];
+    map_fields(&c, (double *)X, zeros, q);
+    for (int f = 0; f < 5; ++f) w[f] = arr(c.N);
+    primitives(&c, q, w);
+    memset(out, 0, sizeof(*out));
+    if (hist_r) memset(hist_r, 0, ORC_HIST_BINS * sizeof(long long));
+    double sum[4] = { 0, 0, 0, 0 }, sq[4] = { 0, 0, 0, 0 }, vol = 0.0, max_r = 0.0;
+    double dx2 = c.d[0] * c.d[0], dy2 = c.d[1] * c.d[1];
+    int k0 = c.walls ? 1 : 0, k1 = c.walls ? c.nz - 1 : c.nz;
+    for (int k = 0; k < c.nz; ++k) {
+        double ps[4] = { 0, 0, 0, 0 }, pq[4] = { 0, 0, 0, 0 };
+        for (int j = 0; j < c.ny; ++j)
+            for (int i = 0; i < c.nx; ++i) {
+                size_t n = at(&c, i, j, k);
+                double u2 = w[W_UX][n] * w[W_UX][n] + w[W_UY][n] * w[W_UY][n] + w[W_UZ][n] * w[W_UZ][n];
+                double r = (0.5 * u2) / (c.cv * w[W_T][n]);
+                if (r > max_r) max_r = r;
+                if (hist_r) hist_r[hist_bin(r)] += 1;
+                if (k < k0 || k >= k1) continue;
+                /* spacings along z around level k (face spacings below and above) */
+                double hm = c.z ? hface(&c, k - 1) : c.d[2], hp = c.z ? hface(&c, k) : c.d[2];
+                size_t xm = (size_t)nb(&c, i, j, k, 0, -1), xp = (size_t)nb(&c, i, j, k, 0, +1);
+                size_t ym = (size_t)nb(&c, i, j, k, 1, -1), yp = (size_t)nb(&c, i, j, k, 1, +1);
+                size_t zm = (size_t)nb(&c, i, j, k, 2, -1), zp = (size_t)nb(&c, i, j, k, 2, +1);
+                const double *uz = w[W_UZ];
+                double Fn = q[Q_RHO][n] * (w[W_UX][n] * deriv(&c, uz, i, j, k, 0, 0)
+                                           + w[W_UY][n] * deriv(&c, uz, i, j, k, 1, 0)
+                                           + w[W_UZ][n] * deriv(&c, uz, i, j, k, 2, 0));
+                double Fp = -deriv(&c, w[W_P], i, j, k, 2, 0);
+                double Fb = q[Q_RHO][n] * c.g;
+                double lap = (uz[xp] - 2.0 * uz[n] + uz[xm]) / dx2;
+                if (c.ndim == 3) lap += (uz[yp] - 2.0 * uz[n] + uz[ym]) / dy2;
+                double dzz = 2.0 * ((uz[zp] - uz[n]) / hp - (uz[n] - uz[zm]) / hm) / (hp + hm);
+                /* mixed derivatives d_z d_x u_x, d_z d_y u_y: central difference along z of the central differences */
+                int kp = (k + 1) % c.nz, km = (k - 1 + c.nz) % c.nz;    /* the levels of zp and zm (never wrapped between plates) */
+                double dzx = (deriv(&c, w[W_UX], i, j, kp, 0, 0) - deriv(&c, w[W_UX], i, j, km, 0, 0)) / (hp + hm);
+                double dzy = (c.ndim == 3)
+                           ? (deriv(&c, w[W_UY], i, j, kp, 1, 0) - deriv(&c, w[W_UY], i, j, km, 1, 0)) / (hp + hm) : 0.0;
+                double Fv = c.mu * (lap + dzz + (1.0 + c.lam) * (dzx + dzy + dzz));
+                double F[4] = { Fn, Fp, Fb, Fv };
+                for (int t = 0; t < 4; ++t) { ps[t] += F[t]; pq[t] += F[t] * F[t]; }
+            }
+        if (k < k0 || k >= k1) continue;
+        double wk = dzc(&c, k) / ((double)c.nx * (double)c.ny);
+        vol += dzc(&c, k);
+        for (int t = 0; t < 4; ++t) { sum[t] += wk * ps[t]; sq[t] += wk * pq[t]; }
+    }
+    double *m = &out->Fn_mean, *r = &out->Fn_rms;
+    for (int t = 0; t < 4; ++t) { m[t] = sum[t] / vol; r[t] = sqrt(sq[t] / vol); }
+    out->FbFp_mean = out->Fb_mean - out->Fp_mean;
+    out->max_r = max_r;
+    out->max_mach = sqrt(2.0 * max_r / (c.gamma * (c.gamma - 1.0)));
+    out->volume = vol;
+    for (int f = 0; f < 5; ++f) free(w[f]);
+    free(zeros);
+    return 0;
+}
+
 int orc_coefficients(const orc_grid *g, const orc_params *p, double *o)
 {
     ctx c;

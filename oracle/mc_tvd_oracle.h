@@ -98,6 +98,21 @@ typedef struct {
 int orc_step_stats(const orc_grid *g, const orc_params *p, double *X, int n_steps, int every,
                    const double *dt_in, orc_stats *out, double *T_prof, double *rho_prof, double *p_prof);
 
+/* Flow statistics of Sec. 5-6, instantaneous: volume averages (means and root-mean-squares) of the z-momentum balance
+ * terms of Eqs. 40-43 over the interior nodes, the largest local Mach number and ratio
+ * r = K_e / I_e, and the histogram of r over all nodes in ORC_HIST_BINS quarter-octave bins from 2^-32
+ * to 1 (bin = 4 (floor(log2 r) + 32) + top two mantissa bits, clamped; r = 0 in bin 0).  hist_r may be NULL.
+ * Reading R21 (the paper does not say how it differences them): see the comment in the .c file. */
+#define ORC_HIST_BINS 128
+typedef struct {
+    double Fn_mean, Fp_mean, Fb_mean, Fv_mean;
+    double Fn_rms, Fp_rms, Fb_rms, Fv_rms;
+    double FbFp_mean;                        /* <F_b> - <F_p> */
+    double max_mach, max_r;
+    double volume;                           /* the volume the averages run over (interior cells) */
+} orc_forces;
+int orc_flow_stats(const orc_grid *g, const orc_params *p, const double *X, orc_forces *out, long long *hist_r);
+
 /* Derived coefficients, in this order: R, c_v, g, mu, K, lambda, dx, dy, dz (9 doubles). */
 int orc_coefficients(const orc_grid *g, const orc_params *p, double *out9);
 
