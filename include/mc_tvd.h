@@ -161,6 +161,34 @@ int mc_tvd_stats_reset(mc_tvd_state *s);
 int mc_tvd_step_stats(mc_tvd_state *s, int n_steps, int every);
 int mc_tvd_stats_read(mc_tvd_state *s, mc_tvd_stats *out, double *T_prof, double *rho_prof, double *p_prof);
 
+/* Flow statistics of the paper's Sec. 5-6, one extra pass over the state:
+ *   - the terms of the z-momentum balance, Eqs. 40-43: F_n = rho (u . grad) u_z, F_p = -d_z p,
+ *     F_b = rho g, F_v = d_i tau_iz with tau_ij of Eq. 18, as volume means and root-mean-squares over the interior
+ *     cells ("the volume averages of the above four terms, along with <F_b> - <F_p>");
+ *   - r = K_e / I_e = (rho u^2 / 2) / (rho C_v T) "at every grid point": its largest value, the largest
+ *     local Mach number, and its histogram over all nodes (Fig. 5) in MC_TVD_HIST_BINS quarter-octave bins from 2^-32
+ *     to 1: bin = 4 (floor(log2 r) + 32) + (top two mantissa bits), clamped to [0, 127]; r = 0 in bin 0.
+ * The paper does not say how it differences these quantities; R21: second-order central differences on the
+ * 3 x 3 x 3 neighbourhood, cell-height weights.
+ * mc_tvd_flow_stats: instantaneous values of the current state into HOST memory (hist_r: MC_TVD_HIST_BINS counts, may
+ * be NULL); synchronises the stream.  mc_tvd_stats_flow(enable = 1): every sample mc_tvd_step_stats takes from now on
+ * also accumulates these numbers on the device (same weights as mc_tvd_stats).  mc_tvd_stats_read_flow: the time
+ * averages since the last mc_tvd_stats_reset -- means as they are, the rms fields as the root of the time-averaged
+ * mean square, max_mach / max_r as the time average of the instantaneous maxima ("the time average of maximum
+ * turbulent Mach number"), `volume` = the simulated time averaged over -- and the histogram summed over
+ * the samples; synchronises; MC_TVD_EINVAL with no sample yet. */
+#define MC_TVD_HIST_BINS 128
+typedef struct {
+    double Fn_mean, Fp_mean, Fb_mean, Fv_mean;   /* volume averages of Eqs. 40-43 */
+    double Fn_rms, Fp_rms, Fb_rms, Fv_rms;       /* square roots of the volume averages of their squares */
+    double FbFp_mean;                            /* <F_b> - <F_p> */
+    double max_mach, max_r;                      /* largest local Mach number and ratio r = K_e / I_e */
+    double volume;                               /* the volume averaged over (interior cells) */
+} mc_tvd_forces;
+int mc_tvd_flow_stats(mc_tvd_state *s, mc_tvd_forces *out, long long *hist_r);
+int mc_tvd_stats_flow(mc_tvd_state *s, int enable);
+int mc_tvd_stats_read_flow(mc_tvd_state *s, mc_tvd_forces *avg, long long *hist_r);
+
 /* Number of kernel launches this handle has enqueued so far (for bench.py's gpu_launches). */
 long long mc_tvd_launch_count(const mc_tvd_state *s);
 

@@ -47,6 +47,13 @@ class Stats(C.Structure):           # mc_tvd_stats
                 ("re", C.c_double), ("u_rms", C.c_double), ("nu_bar_sq", C.c_double), ("re_sq", C.c_double)]
 
 
+class Forces(C.Structure):          # mc_tvd_forces
+    _fields_ = [(n, C.c_double) for n in ("Fn_mean", "Fp_mean", "Fb_mean", "Fv_mean", "Fn_rms", "Fp_rms", "Fb_rms",
+                                          "Fv_rms", "FbFp_mean", "max_mach", "max_r", "volume")]
+
+
+HIST_BINS = 128                     # MC_TVD_HIST_BINS
+
 # every symbol include/mc_tvd.h declares: name -> (restype, argtypes)
 SYMBOLS = {
     "mc_tvd_workspace_bytes": (C.c_size_t, [C.POINTER(Grid), C.POINTER(Params)]),
@@ -62,6 +69,9 @@ SYMBOLS = {
     "mc_tvd_stats_reset": (C.c_int, [C.c_void_p]),
     "mc_tvd_step_stats": (C.c_int, [C.c_void_p, C.c_int, C.c_int]),
     "mc_tvd_stats_read": (C.c_int, [C.c_void_p, C.POINTER(Stats), _DP, _DP, _DP]),
+    "mc_tvd_flow_stats": (C.c_int, [C.c_void_p, C.POINTER(Forces), C.POINTER(C.c_longlong)]),
+    "mc_tvd_stats_flow": (C.c_int, [C.c_void_p, C.c_int]),
+    "mc_tvd_stats_read_flow": (C.c_int, [C.c_void_p, C.POINTER(Forces), C.POINTER(C.c_longlong)]),
     "mc_tvd_launch_count": (C.c_longlong, [C.c_void_p]),
     "mc_tvd_timing_enable": (C.c_int, [C.c_void_p, C.c_int]),
     "mc_tvd_timing_read": (C.c_int, [C.c_void_p, _DP, C.POINTER(C.c_longlong)]),
@@ -225,6 +235,23 @@ class MCTVD:
         self._check(self.lib.mc_tvd_stats_read(self._h, C.byref(st), Tp.ctypes.data_as(_DP), rp.ctypes.data_as(_DP),
                                                pp.ctypes.data_as(_DP)))
         return {n: getattr(st, n) for n, _ in Stats._fields_}, Tp, rp, pp
+
+    def flow_stats(self):
+        """Returns (dict of the force-balance averages of Eqs. 40-43 and the extrema, histogram of r as int64[HIST_BINS])."""
+        f = Forces()
+        hist = np.zeros(HIST_BINS, dtype=np.int64)
+        self._check(self.lib.mc_tvd_flow_stats(self._h, C.byref(f), hist.ctypes.data_as(C.POINTER(C.c_longlong))))
+        return {n: getattr(f, n) for n, _ in Forces._fields_}, hist
+
+    def stats_flow(self, enable: bool = True):
+        self._check(self.lib.mc_tvd_stats_flow(self._h, int(bool(enable))))
+
+    def stats_read_flow(self):
+        """Time averages of the flow statistics since the last stats_reset: (dict, summed histogram)."""
+        f = Forces()
+        hist = np.zeros(HIST_BINS, dtype=np.int64)
+        self._check(self.lib.mc_tvd_stats_read_flow(self._h, C.byref(f), hist.ctypes.data_as(C.POINTER(C.c_longlong))))
+        return {n: getattr(f, n) for n, _ in Forces._fields_}, hist
 
     def launch_count(self) -> int:
         return int(self.lib.mc_tvd_launch_count(self._h))

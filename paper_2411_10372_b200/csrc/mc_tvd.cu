@@ -14,6 +14,7 @@
 #include "mc_async.cuh"
 #include "mc_common.cuh"
 #include "reduce_kernels.cuh"
+#include "flow_stats.cuh"
 #include "sweep_lane.cuh"
 #include "sweep_lane2.cuh"
 #include "sweep_lane3.cuh"
@@ -83,6 +84,7 @@ constexpr int DIAG_MAX_BLOCKS = 16;    // blocks per plane in the diagnostics pa
 
 struct Layout {                        // byte offsets inside the workspace
     size_t Y, scalars, partial, ext, plane_sums, plane_ext, diag_out, stats, stats_out, zt, total;
+    size_t flow_partial, flow_ext, flow_hist, flow_out, flow_acc, flow_hist_acc;
     int diag_blocks;
 };
 
@@ -99,6 +101,10 @@ struct mc_tvd_state {
     double *X, *Y;
     mc::Scalars *S;
     double *partial, *ext, *plane_sums, *plane_ext, *diag_out, *stats, *stats_out;
+    double *flow_partial, *flow_ext, *flow_out, *flow_acc;
+    unsigned long long *flow_hist, *flow_hist_acc;
+    bool flow_in_stats;                // samples of mc_tvd_step_stats also accumulate the flow statistics
+    int slab_next;                     // mc_tvd_slab_op: the operator of the current step that comes next
     const double *zt;                  // device z-metric tables of the non-uniform grid (R19 / R20), or null
     double zt_max_icfl;                // max over levels of the CFL rule's reciprocal z spacing
     long long stat_steps;              // steps taken through mc_tvd_step_stats since the last reset
@@ -170,6 +176,12 @@ Layout make_layout(const mc_tvd_grid *g)
     L.stats = o;      o = align_up(o + (mc::ST_HEAD + 3 * (size_t)g->nz) * sizeof(double), 256);
     L.stats_out = o;  o = align_up(o + (4 + mc::ST_NSUM + 3 * (size_t)g->nz) * sizeof(double), 256);
     L.zt = o;         o = align_up(o + 5 * (size_t)g->nz * sizeof(double), 256);       // z-metric tables (SweepArgs::zt)
+    L.flow_partial = o;  o = align_up(o + (size_t)g->nz * nb * mc::FLOW_NQ * sizeof(double), 256);
+    L.flow_ext = o;      o = align_up(o + (size_t)g->nz * nb * sizeof(double), 256);
+    L.flow_hist = o;     o = align_up(o + mc::FLOW_BINS * sizeof(unsigned long long), 256);
+    L.flow_out = o;      o = align_up(o + mc::FLOW_NOUT * sizeof(double), 256);
+    L.flow_acc = o;      o = align_up(o + mc::FLOW_NOUT * sizeof(double), 256);
+    L.flow_hist_acc = o; o = align_up(o + mc::FLOW_BINS * sizeof(unsigned long long), 256);
     L.total = o;
     return L;
 }
@@ -454,6 +466,7 @@ mc::PointArgs point_args(const mc_tvd_state *s)
         P.inv_d[comp_of_axis(s->nd, a)] = 1.0 / s->d[a];
     }
     P.zt = s->zt;
+    P.own_axis = -1; P.nx = s->grid.nx;
     return P;
 }
 
@@ -525,6 +538,13 @@ int mc_tvd_init(const mc_tvd_grid *grid, const mc_tvd_params *params, double *d_
     s->diag_out = (double *)(w + L.diag_out);
     s->stats = (double *)(w + L.stats);
     s->stats_out = (double *)(w + L.stats_out);
+    s->flow_partial = (double *)(w + L.flow_partial);
+    s->flow_ext = (double *)(w + L.flow_ext);
+    s->flow_hist = (unsigned long long *)(w + L.flow_hist);
+    s->flow_out = (double *)(w + L.flow_out);
+    s->flow_acc = (double *)(w + L.flow_acc);
+    s->flow_hist_acc = (unsigned long long *)(w + L.flow_hist_acc);
+    s->flow_in_stats = false;
     s->zt = nullptr; s->zt_max_icfl = 0.0;
     s->grid.z_nodes = nullptr;         // the caller's array is not kept: its numbers live in the device tables
     s->diag_blocks = L.diag_blocks;
@@ -676,13 +696,8 @@ int mc_tvd_dt(mc_tvd_state *s, double *dt_host)
 }  // extern "C"
 
 namespace {
-// Enqueue the three diagnostics kernels (Eqs. 22-26): the result block lands in s->diag_out on the device.
-int enqueue_diagnostics(mc_tvd_state *s)
+mc::DiagArgs diag_args(const mc_tvd_state *s)
 {
-    mc::PointArgs P = point_args(s);
-    dim3 grid((unsigned)s->diag_blocks, (unsigned)s->grid.nz, 1);
-    if (s->nd == 2) { auto kfn = mc::k_plane_partials<2>; MC_LAUNCH(kfn, grid, mc::DIAG_THREADS, 0, s->stream, P, s->partial, s->ext); }
-    else { auto kfn = mc::k_plane_partials<3>; MC_LAUNCH(kfn, grid, mc::DIAG_THREADS, 0, s->stream, P, s->partial, s->ext); }
     mc::DiagArgs G;
     memset(&G, 0, sizeof(G));
     G.partial = s->partial; G.ext = s->ext; G.plane_sums = s->plane_sums; G.out = s->diag_out; G.S = s->S;
@@ -691,26 +706,50 @@ int enqueue_diagnostics(mc_tvd_state *s)
     G.dz = s->d[2]; G.dxdy = s->d[0] * s->d[1];
     G.eps = s->par.eps; G.D = s->par.D; G.Ra = s->par.Ra; G.Pr = s->par.Pr;
     G.zt = s->zt;
+    return G;
+}
+
+// Stages 1-2 of the diagnostics (Eqs. 22-26): per-plane sums and extrema of the nodes whose index along own_axis lies in
+// [lo, hi) (own_axis = -1: every node) land in s->plane_sums / s->plane_ext.
+int enqueue_diag_planes(mc_tvd_state *s, int own_axis, int lo, int hi)
+{
+    mc::PointArgs P = point_args(s);
+    P.own_axis = own_axis; P.own_lo = lo; P.own_hi = hi;
+    dim3 grid((unsigned)s->diag_blocks, (unsigned)s->grid.nz, 1);
+    if (s->nd == 2) { auto kfn = mc::k_plane_partials<2>; MC_LAUNCH(kfn, grid, mc::DIAG_THREADS, 0, s->stream, P, s->partial, s->ext); }
+    else { auto kfn = mc::k_plane_partials<3>; MC_LAUNCH(kfn, grid, mc::DIAG_THREADS, 0, s->stream, P, s->partial, s->ext); }
+    mc::DiagArgs G = diag_args(s);
     { auto kfn = mc::k_diag_planes; MC_LAUNCH(kfn, (unsigned)((s->grid.nz + 3) / 4), 128, 0, s->stream, G, s->plane_ext); }
-    { auto kfn = mc::k_diag_finish; MC_LAUNCH(kfn, 1, mc::DIAG_THREADS, 0, s->stream, G, s->plane_ext); }
-    s->launches += 3;
+    s->launches += 2;
     return cuda_check(cudaGetLastError(), "diagnostics launch");
 }
-}  // namespace
 
-extern "C" {
-
-int mc_tvd_diagnostics(mc_tvd_state *s, mc_tvd_diag *out, double *T_prof, double *rho_prof, double *p_prof)
+// Stage 3: plane sums -> the result block in s->diag_out.  nplane: nodes per z plane the sums run over.
+int enqueue_diag_finish(mc_tvd_state *s, double nplane)
 {
-    if (!s || !out) return fail(MC_TVD_EINVAL, "bad handle or out");
-    static_assert(sizeof(mc_tvd_diag) == 19 * sizeof(double), "mc_tvd_diag layout");
-    int rc = enqueue_diagnostics(s);
-    if (rc != MC_TVD_OK) return rc;
+    mc::DiagArgs G = diag_args(s);
+    G.nplane = nplane;
+    { auto kfn = mc::k_diag_finish; MC_LAUNCH(kfn, 1, mc::DIAG_THREADS, 0, s->stream, G, s->plane_ext); }
+    s->launches += 1;
+    return cuda_check(cudaGetLastError(), "diagnostics launch");
+}
+
+// Enqueue the three diagnostics kernels (Eqs. 22-26): the result block lands in s->diag_out on the device.
+int enqueue_diagnostics(mc_tvd_state *s)
+{
+    int rc = enqueue_diag_planes(s, -1, 0, 0);
+    if (rc == MC_TVD_OK) rc = enqueue_diag_finish(s, (double)s->grid.nx * (double)s->grid.ny);
+    return rc;
+}
+
+// copy the diagnostics block out of s->diag_out (synchronises)
+int read_diag_block(mc_tvd_state *s, mc_tvd_diag *out, double *T_prof, double *rho_prof, double *p_prof)
+{
     const size_t nz = (size_t)s->grid.nz;
     double *h = (double *)malloc((19 + 3 * nz) * sizeof(double));
     if (!h) return fail(MC_TVD_ENOMEM, "host allocation failed");
-    rc = cuda_check(cudaMemcpyAsync(h, s->diag_out, (19 + 3 * nz) * sizeof(double), cudaMemcpyDeviceToHost, s->stream),
-                    "diagnostics copy");
+    int rc = cuda_check(cudaMemcpyAsync(h, s->diag_out, (19 + 3 * nz) * sizeof(double), cudaMemcpyDeviceToHost, s->stream),
+                        "diagnostics copy");
     if (rc == MC_TVD_OK) rc = cuda_check(cudaStreamSynchronize(s->stream), "diagnostics sync");
     if (rc == MC_TVD_OK) {
         memcpy(out, h, sizeof(*out));
@@ -722,13 +761,114 @@ int mc_tvd_diagnostics(mc_tvd_state *s, mc_tvd_diag *out, double *T_prof, double
     return rc;
 }
 
+// Enqueue the flow statistics of Sec. 5-6 (flow_stats.cuh): the 12 numbers land in s->flow_out, the histogram of this
+// sample is ADDED to s->flow_hist (the caller clears or consumes it).
+int enqueue_flow_stats(mc_tvd_state *s)
+{
+    mc::FlowArgs G;
+    memset(&G, 0, sizeof(G));
+    G.P = point_args(s);
+    G.nx = s->grid.nx; G.ny = s->grid.ny; G.walls = s->walls ? 1 : 0;
+    G.mu = s->mu; G.lam = s->par.lambda_coef; G.cv = s->cv;
+    G.inv_2dx = 0.5 / s->d[0]; G.inv_dx2 = 1.0 / (s->d[0] * s->d[0]);
+    G.inv_2dy = 0.5 / s->d[1]; G.inv_dy2 = 1.0 / (s->d[1] * s->d[1]);
+    dim3 grid((unsigned)s->diag_blocks, (unsigned)s->grid.nz, 1);
+    if (s->nd == 2) { auto kfn = mc::k_flow_partials<2>; MC_LAUNCH(kfn, grid, mc::DIAG_THREADS, 0, s->stream, G, s->flow_partial, s->flow_ext, s->flow_hist); }
+    else { auto kfn = mc::k_flow_partials<3>; MC_LAUNCH(kfn, grid, mc::DIAG_THREADS, 0, s->stream, G, s->flow_partial, s->flow_ext, s->flow_hist); }
+    { auto kfn = mc::k_flow_finish; MC_LAUNCH(kfn, 1, mc::DIAG_THREADS, 0, s->stream, G, s->flow_partial, s->flow_ext, s->diag_blocks, s->par.gamma, s->flow_out); }
+    s->launches += 2;
+    return cuda_check(cudaGetLastError(), "flow statistics launch");
+}
+}  // namespace
+
+extern "C" {
+
+int mc_tvd_diagnostics(mc_tvd_state *s, mc_tvd_diag *out, double *T_prof, double *rho_prof, double *p_prof)
+{
+    if (!s || !out) return fail(MC_TVD_EINVAL, "bad handle or out");
+    static_assert(sizeof(mc_tvd_diag) == 19 * sizeof(double), "mc_tvd_diag layout");
+    int rc = enqueue_diagnostics(s);
+    if (rc != MC_TVD_OK) return rc;
+    return read_diag_block(s, out, T_prof, rho_prof, p_prof);
+}
+
+// ---- slab decomposition hooks (include/mc_tvd.h "Slab decomposition") ------------------------------------------------
+int mc_tvd_slab_op(mc_tvd_state *s, int op)
+{
+    const int nops = s ? 2 * s->nd : 0;
+    if (!s || op < 0 || op >= nops) return fail(MC_TVD_EINVAL, "bad handle or operator number");
+    if (op != s->slab_next) return fail(MC_TVD_EINVAL, "operators of a step must be enqueued in order, each once");
+    const int half = op / s->nd, a = (s->nd == 2) ? (op % 2 == 0 ? 2 : 0) : 2 - (op % 3);      // L_z, [L_y,] L_x (Eq. 30)
+    const int dir = (half == 1 && s->par.dir_mode == 1) ? -1 : +1;
+    const double *src = (op % 2 == 0) ? s->X : s->Y;
+    double *dst = (op % 2 == 0) ? s->Y : s->X;
+    int rc = launch_sweep(s, src, dst, a, dir, 0.0, true, false);   // no fused CFL reduction: the halo copies are stale here
+    s->ev_open = false;
+    if (rc == MC_TVD_OK) s->slab_next = op + 1;
+    return rc;
+}
+
+int mc_tvd_slab_reduce(mc_tvd_state *s)
+{
+    if (!s) return fail(MC_TVD_EINVAL, "bad handle");
+    if (s->slab_next != 0 && s->slab_next != 2 * s->nd) return fail(MC_TVD_EINVAL, "a step is half done: the state is not in d_fields");
+    mc::PointArgs P = point_args(s);
+    int blocks = (int)((s->N + 255) / 256);
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    if (s->nd == 2) { auto kfn = mc::k_max_speed<2>; MC_LAUNCH(kfn, blocks, 256, 0, s->stream, P, &s->S->smax_bits); }
+    else { auto kfn = mc::k_max_speed<3>; MC_LAUNCH(kfn, blocks, 256, 0, s->stream, P, &s->S->smax_bits); }
+    s->launches += 1;
+    return cuda_check(cudaGetLastError(), "max-speed launch");
+}
+
+int mc_tvd_slab_commit(mc_tvd_state *s, int advance)
+{
+    if (!s) return fail(MC_TVD_EINVAL, "bad handle");
+    if (advance && s->slab_next != 2 * s->nd) return fail(MC_TVD_EINVAL, "the step's operators have not all been enqueued");
+    { auto kfn = mc::k_dt_update; MC_LAUNCH(kfn, 1, 32, 0, s->stream, s->S, advance ? 1 : 0); }
+    s->launches += 1;
+    if (advance) s->slab_next = 0;
+    return cuda_check(cudaGetLastError(), "dt launch");
+}
+
+int mc_tvd_slab_pointers(mc_tvd_state *s, double **fields_now, unsigned long long **smax_bits, double **plane_sums,
+                         double **plane_ext)
+{
+    if (!s) return fail(MC_TVD_EINVAL, "bad handle");
+    if (fields_now) *fields_now = (s->slab_next % 2 == 0) ? s->X : s->Y;
+    if (smax_bits) *smax_bits = &s->S->smax_bits;
+    if (plane_sums) *plane_sums = s->plane_sums;
+    if (plane_ext) *plane_ext = s->plane_ext;
+    return MC_TVD_OK;
+}
+
+int mc_tvd_slab_diag_partial(mc_tvd_state *s, int axis, int lo, int hi)
+{
+    if (!s || (axis != 0 && axis != 1) || lo < 0 || hi < lo) return fail(MC_TVD_EINVAL, "bad handle, axis or range");
+    if (s->slab_next != 0 && s->slab_next != 2 * s->nd) return fail(MC_TVD_EINVAL, "a step is half done: the state is not in d_fields");
+    return enqueue_diag_planes(s, axis, lo, hi);
+}
+
+int mc_tvd_slab_diag_finish(mc_tvd_state *s, double nplane_global, mc_tvd_diag *out, double *T_prof, double *rho_prof,
+                            double *p_prof)
+{
+    if (!s || !out || !(nplane_global >= 1.0)) return fail(MC_TVD_EINVAL, "bad handle, out or node count");
+    int rc = enqueue_diag_finish(s, nplane_global);
+    if (rc != MC_TVD_OK) return rc;
+    return read_diag_block(s, out, T_prof, rho_prof, p_prof);
+}
+
 int mc_tvd_stats_reset(mc_tvd_state *s)
 {
     if (!s) return fail(MC_TVD_EINVAL, "bad handle");
     { auto kfn = mc::k_stats_reset; MC_LAUNCH(kfn, 1, 256, 0, s->stream, s->stats, s->S, s->grid.nz); }
     s->launches += 1;
     s->stat_steps = 0;
-    return cuda_check(cudaGetLastError(), "stats reset launch");
+    int rc = cuda_check(cudaGetLastError(), "stats reset launch");
+    if (rc == MC_TVD_OK) rc = cuda_check(cudaMemsetAsync(s->flow_acc, 0, mc::FLOW_NOUT * sizeof(double), s->stream), "flow reset");
+    if (rc == MC_TVD_OK) rc = cuda_check(cudaMemsetAsync(s->flow_hist_acc, 0, mc::FLOW_BINS * sizeof(unsigned long long), s->stream), "flow reset");
+    if (rc == MC_TVD_OK) rc = cuda_check(cudaMemsetAsync(s->flow_hist, 0, mc::FLOW_BINS * sizeof(unsigned long long), s->stream), "flow reset");
+    return rc;
 }
 
 int mc_tvd_step_stats(mc_tvd_state *s, int n_steps, int every)
@@ -741,6 +881,12 @@ int mc_tvd_step_stats(mc_tvd_state *s, int n_steps, int every)
         if (s->stat_steps % every) continue;
         rc = enqueue_diagnostics(s);
         if (rc != MC_TVD_OK) return rc;
+        if (s->flow_in_stats) {            // before k_stats_accumulate, which moves the time of the previous sample
+            rc = enqueue_flow_stats(s);
+            if (rc != MC_TVD_OK) return rc;
+            { auto kfn = mc::k_flow_accumulate; MC_LAUNCH(kfn, 1, 128, 0, s->stream, s->flow_acc, s->flow_out, s->stats, s->S, s->flow_hist_acc, s->flow_hist); }
+            s->launches += 1;
+        }
         { auto kfn = mc::k_stats_accumulate; MC_LAUNCH(kfn, 1, 256, 0, s->stream, s->stats, s->diag_out, s->S, s->grid.nz); }
         s->launches += 1;
         rc = cuda_check(cudaGetLastError(), "stats accumulate launch");
@@ -772,6 +918,47 @@ int mc_tvd_stats_read(mc_tvd_state *s, mc_tvd_stats *out, double *T_prof, double
     }
     free(h);
     return rc;
+}
+
+int mc_tvd_flow_stats(mc_tvd_state *s, mc_tvd_forces *out, long long *hist_r)
+{
+    if (!s || !out) return fail(MC_TVD_EINVAL, "bad handle or out");
+    static_assert(sizeof(mc_tvd_forces) == mc::FLOW_NOUT * sizeof(double), "mc_tvd_forces layout");
+    static_assert(MC_TVD_HIST_BINS == mc::FLOW_BINS, "histogram size");
+    int rc = cuda_check(cudaMemsetAsync(s->flow_hist, 0, mc::FLOW_BINS * sizeof(unsigned long long), s->stream), "histogram clear");
+    if (rc == MC_TVD_OK) rc = enqueue_flow_stats(s);
+    unsigned long long h[mc::FLOW_BINS];
+    if (rc == MC_TVD_OK) rc = cuda_check(cudaMemcpyAsync(out, s->flow_out, sizeof(*out), cudaMemcpyDeviceToHost, s->stream), "flow copy");
+    if (rc == MC_TVD_OK) rc = cuda_check(cudaMemcpyAsync(h, s->flow_hist, sizeof(h), cudaMemcpyDeviceToHost, s->stream), "histogram copy");
+    if (rc == MC_TVD_OK) rc = cuda_check(cudaStreamSynchronize(s->stream), "flow sync");
+    if (rc == MC_TVD_OK) rc = cuda_check(cudaMemsetAsync(s->flow_hist, 0, sizeof(h), s->stream), "histogram clear");
+    if (rc == MC_TVD_OK && hist_r) for (int i = 0; i < mc::FLOW_BINS; ++i) hist_r[i] = (long long)h[i];
+    return rc;
+}
+
+int mc_tvd_stats_flow(mc_tvd_state *s, int enable)
+{
+    if (!s) return fail(MC_TVD_EINVAL, "bad handle");
+    s->flow_in_stats = enable != 0;
+    return MC_TVD_OK;
+}
+
+int mc_tvd_stats_read_flow(mc_tvd_state *s, mc_tvd_forces *avg, long long *hist_r)
+{
+    if (!s || !avg) return fail(MC_TVD_EINVAL, "bad handle or avg");
+    double a[mc::FLOW_NOUT];
+    unsigned long long h[mc::FLOW_BINS];
+    int rc = cuda_check(cudaMemcpyAsync(a, s->flow_acc, sizeof(a), cudaMemcpyDeviceToHost, s->stream), "flow copy");
+    if (rc == MC_TVD_OK) rc = cuda_check(cudaMemcpyAsync(h, s->flow_hist_acc, sizeof(h), cudaMemcpyDeviceToHost, s->stream), "histogram copy");
+    if (rc == MC_TVD_OK) rc = cuda_check(cudaStreamSynchronize(s->stream), "flow sync");
+    if (rc != MC_TVD_OK) return rc;
+    if (!(a[11] > 0.0)) return fail(MC_TVD_EINVAL, "no flow sample has been accumulated since the last mc_tvd_stats_reset (see mc_tvd_stats_flow)");
+    double *o = &avg->Fn_mean;
+    for (int t = 0; t < 4; ++t) { o[t] = a[t] / a[11]; o[4 + t] = sqrt(a[4 + t] / a[11]); }
+    for (int t = 8; t < 11; ++t) o[t] = a[t] / a[11];
+    o[11] = a[11];                     // `volume` carries the total weight (simulated time averaged over)
+    if (hist_r) for (int i = 0; i < mc::FLOW_BINS; ++i) hist_r[i] = (long long)h[i];
+    return MC_TVD_OK;
 }
 
 long long mc_tvd_launch_count(const mc_tvd_state *s) { return s ? s->launches : 0; }

@@ -22,6 +22,9 @@ struct PointArgs {                   // what a pointwise pass over the state nee
     double dz, g, icv, R, gamma, D;
     double inv_d[3];
     const double *zt;                // non-uniform z grid: the tables of SweepArgs::zt, or null
+    // slab decomposition (diagnostics only): sum the nodes whose index along own_axis (0: x, 1: y; -1: all) lies in
+    // [own_lo, own_hi) -- the rows a rank owns, without its halo copies
+    int own_axis, own_lo, own_hi, nx;
 };
 
 MC_DEV double point_z(const PointArgs &P, int k) { return P.zt ? P.zt[k] : (double)k * P.dz; }
@@ -117,6 +120,10 @@ MC_KERNEL void k_plane_partials(PointArgs P, double *partial, double *ext)
     const double *base = P.X + (long long)k * P.plane;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < P.plane;
          i += (long long)gridDim.x * blockDim.x) {
+        if (P.own_axis >= 0) {
+            const int idx = (P.own_axis == 0) ? (int)(i % P.nx) : (int)(i / P.nx);
+            if (idx < P.own_lo || idx >= P.own_hi) continue;
+        }
         double X[NF], u[ND];
 #pragma unroll
         for (int f = 0; f < NF; ++f) X[f] = base[(long long)f * P.N + i];
