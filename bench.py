@@ -48,6 +48,9 @@ def parse_args():
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
     ap.add_argument("--no-2d", action="store_true", help="skip the extra 2-D roofline leg (C3 at its 200 steps) of the default C5 run")
     ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--slabs", action="store_true",
+                    help="N > 1 only: ONE box cut into N slabs (paper_2411_10372_b200/slab.py, halo exchange over NCCL) instead "
+                         "of N replicas; strong scaling.  Built and parity-tested, never timed on more than one GPU")
     return ap.parse_args()
 
 
@@ -411,10 +414,50 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_slabs(args):
+    """--slabs under torchrun: the workload's ONE box as N slabs, one per GPU, halo exchange and the dt
+    all-reduce inside the timed region.  value = cells of the whole box x steps / slowest rank's device time."""
+    import torch
+    import torch.distributed as dist
+
+    world, rank, local = int(os.environ["WORLD_SIZE"]), int(os.environ["RANK"]), int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    from paper_2411_10372_b200 import binding, slab
+    name = args.workload
+    grid, params, _ = inputs.config(name)
+    X0 = inputs.conduction_state(grid, params)
+    drv = slab.make_dist_driver(binding, grid, params, X0, device=f"cuda:{local}")
+    del X0
+    drv.step(args.warmup)
+    dist.barrier(); torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local) as clocks:
+        e0.record(drv.ranks[0].stream)
+        drv.step(args.steps)
+        e1.record(drv.ranks[0].stream)
+        dist.barrier(); torch.cuda.synchronize()
+    ms = max_over_ranks(e0.elapsed_time(e1), world, f"cuda:{local}")
+    dt_now = drv.dt()
+    if rank == 0:
+        N = inputs.num_nodes(grid)
+        print(json.dumps({
+            "metric": METRIC, "value": N * args.steps / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong",
+            "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic (seeded hydrostatic conduction state + T noise, DESIGN.md input recipe)",
+            "config": dict(workload_config(name, grid, params), decomposition=f"{world} slabs along {slab.slab_axis(grid)}, halo 2, "
+                           "exchange after every operator (NCCL send/recv), dt all-reduce"),
+            "clocks": clocks.summary(), "gpu_launches": int(drv.ranks[0].launch_count()), "state_check": {"dt": dt_now}}), flush=True)
+    dist.destroy_process_group()
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.slabs and int(os.environ.get("WORLD_SIZE", "1")) > 1:
+        run_slabs(args)
     else:
         run_ours(args)
 

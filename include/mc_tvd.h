@@ -189,6 +189,37 @@ int mc_tvd_flow_stats(mc_tvd_state *s, mc_tvd_forces *out, long long *hist_r);
 int mc_tvd_stats_flow(mc_tvd_state *s, int enable);
 int mc_tvd_stats_read_flow(mc_tvd_state *s, mc_tvd_forces *avg, long long *hist_r);
 
+/* Slab decomposition: the hooks a multi-GPU driver needs to run one box as slabs along a periodic
+ * horizontal direction, one handle per GPU, as the paper's multi-GPU runs do (App. A :573-577).  A
+ * rank's handle is an ordinary handle on its LOCAL box: the rows it owns plus H >= 2 halo rows on either side, treated
+ * as periodic (the wrap only corrupts the outermost 2 rows per operator, which are halo rows).  Every operator has
+ * radius 2 across and along the slab axis, so the driver refreshes the halo rows from the neighbours after every
+ * operator (paper_2411_10372_b200/slab.py does this with NCCL send/recv, or with device copies when several slabs
+ * live on one GPU):
+ *   mc_tvd_slab_op(s, op)       enqueue operator number op = 0 .. 2 ndim - 1 of the current step (Eq. 30 order: L_z,
+ *                               [L_y,] L_x with dir +1, then again with dir -1), without the fused CFL reduction;
+ *                               operators must come in order;
+ *   mc_tvd_slab_pointers        device addresses the driver exchanges / all-reduces: the buffer that holds the state
+ *                               right now (it alternates between d_fields and the workspace after every operator),
+ *                               the bit pattern of the running maximum of (|u_a| + c_s)/dx_a, the per-plane sums
+ *                               (nz x 11 doubles) and extrema (nz x 3: max Mach^2, min rho, min T) of the diagnostics;
+ *   mc_tvd_slab_reduce(s)       after the last halo exchange of a step (or of the initial state): max-speed reduction
+ *                               over the local box into the running maximum; the driver then all-reduces it (MAX);
+ *   mc_tvd_slab_commit(s, adv)  dt from the maximum (R12); adv = 1 also advances time and the step count;
+ *   mc_tvd_slab_diag_partial    per-plane sums of Eqs. 22-26 over the nodes whose index along axis (0 x, 1 y) lies in
+ *                               [lo, hi) -- the owned rows; the driver all-reduces sums (SUM) and extrema (MAX, MIN);
+ *   mc_tvd_slab_diag_finish     the diagnostics from the all-reduced plane sums; nplane_global = nodes per z plane of
+ *                               the whole box.  Synchronises.
+ * All asynchronous on the handle's stream except the last.  mc_tvd_step on such a handle would use stale halos. */
+int mc_tvd_slab_op(mc_tvd_state *s, int op);
+int mc_tvd_slab_reduce(mc_tvd_state *s);
+int mc_tvd_slab_commit(mc_tvd_state *s, int advance);
+int mc_tvd_slab_pointers(mc_tvd_state *s, double **fields_now, unsigned long long **smax_bits, double **plane_sums,
+                         double **plane_ext);
+int mc_tvd_slab_diag_partial(mc_tvd_state *s, int axis, int lo, int hi);
+int mc_tvd_slab_diag_finish(mc_tvd_state *s, double nplane_global, mc_tvd_diag *out, double *T_prof, double *rho_prof,
+                            double *p_prof);
+
 /* Number of kernel launches this handle has enqueued so far (for bench.py's gpu_launches). */
 long long mc_tvd_launch_count(const mc_tvd_state *s);
 

@@ -72,6 +72,13 @@ SYMBOLS = {
     "mc_tvd_flow_stats": (C.c_int, [C.c_void_p, C.POINTER(Forces), C.POINTER(C.c_longlong)]),
     "mc_tvd_stats_flow": (C.c_int, [C.c_void_p, C.c_int]),
     "mc_tvd_stats_read_flow": (C.c_int, [C.c_void_p, C.POINTER(Forces), C.POINTER(C.c_longlong)]),
+    "mc_tvd_slab_op": (C.c_int, [C.c_void_p, C.c_int]),
+    "mc_tvd_slab_reduce": (C.c_int, [C.c_void_p]),
+    "mc_tvd_slab_commit": (C.c_int, [C.c_void_p, C.c_int]),
+    "mc_tvd_slab_pointers": (C.c_int, [C.c_void_p, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p), C.POINTER(C.c_void_p),
+                                       C.POINTER(C.c_void_p)]),
+    "mc_tvd_slab_diag_partial": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int]),
+    "mc_tvd_slab_diag_finish": (C.c_int, [C.c_void_p, C.c_double, C.POINTER(Diag), _DP, _DP, _DP]),
     "mc_tvd_launch_count": (C.c_longlong, [C.c_void_p]),
     "mc_tvd_timing_enable": (C.c_int, [C.c_void_p, C.c_int]),
     "mc_tvd_timing_read": (C.c_int, [C.c_void_p, _DP, C.POINTER(C.c_longlong)]),
@@ -252,6 +259,45 @@ class MCTVD:
         hist = np.zeros(HIST_BINS, dtype=np.int64)
         self._check(self.lib.mc_tvd_stats_read_flow(self._h, C.byref(f), hist.ctypes.data_as(C.POINTER(C.c_longlong))))
         return {n: getattr(f, n) for n, _ in Forces._fields_}, hist
+
+    # -- slab decomposition hooks (used by paper_2411_10372_b200.slab) ------------------------------------------
+    def slab_op(self, op: int):
+        self._check(self.lib.mc_tvd_slab_op(self._h, int(op)))
+
+    def slab_reduce(self):
+        self._check(self.lib.mc_tvd_slab_reduce(self._h))
+
+    def slab_commit(self, advance: bool):
+        self._check(self.lib.mc_tvd_slab_commit(self._h, int(bool(advance))))
+
+    def _view(self, ptr: int, count: int, dtype):
+        """A torch view of `count` 8-byte elements at device address ptr, which lies inside self.fields or self.workspace."""
+        for t in (self.fields, self.workspace):
+            off = ptr - t.data_ptr()
+            if 0 <= off and off + 8 * count <= t.numel() * 8:
+                assert off % 8 == 0
+                return t[off // 8: off // 8 + count].view(dtype)
+        raise RuntimeError("pointer outside the handle's buffers")
+
+    def slab_views(self):
+        """(state buffer now as (nf, nz, ny, nx), running-maximum bits as int64[1], plane sums (nz, 11), plane extrema (nz, 3))."""
+        torch = self._torch
+        p = [C.c_void_p() for _ in range(4)]
+        self._check(self.lib.mc_tvd_slab_pointers(self._h, *[C.byref(x) for x in p]))
+        g = self.grid
+        f = self._view(p[0].value, self.nf * self.N, torch.float64).view(self.nf, self.nz, int(g.get("ny", 1)), int(g["nx"]))
+        return (f, self._view(p[1].value, 1, torch.int64), self._view(p[2].value, self.nz * 11, torch.float64).view(self.nz, 11),
+                self._view(p[3].value, self.nz * 3, torch.float64).view(self.nz, 3))
+
+    def slab_diag_partial(self, axis: int, lo: int, hi: int):
+        self._check(self.lib.mc_tvd_slab_diag_partial(self._h, int(axis), int(lo), int(hi)))
+
+    def slab_diag_finish(self, nplane_global: float):
+        d = Diag()
+        Tp, rp, pp = np.zeros(self.nz), np.zeros(self.nz), np.zeros(self.nz)
+        self._check(self.lib.mc_tvd_slab_diag_finish(self._h, float(nplane_global), C.byref(d), Tp.ctypes.data_as(_DP),
+                                                     rp.ctypes.data_as(_DP), pp.ctypes.data_as(_DP)))
+        return {n: getattr(d, n) for n, _ in Diag._fields_}, Tp, rp, pp
 
     def launch_count(self) -> int:
         return int(self.lib.mc_tvd_launch_count(self._h))

@@ -105,6 +105,9 @@ struct mc_tvd_state {
     unsigned long long *flow_hist, *flow_hist_acc;
     bool flow_in_stats;                // samples of mc_tvd_step_stats also accumulate the flow statistics
     int slab_next;                     // mc_tvd_slab_op: the operator of the current step that comes next
+    cudaGraphExec_t graph_exec;        // one step's launch list (mc_tvd_step replays it), or null
+    int graph_launches, graph_chunk;   // kernels in it; the chunk override it was captured with
+    bool graph_failed;
     const double *zt;                  // device z-metric tables of the non-uniform grid (R19 / R20), or null
     double zt_max_icfl;                // max over levels of the CFL rule's reciprocal z spacing
     long long stat_steps;              // steps taken through mc_tvd_step_stats since the last reset
@@ -251,7 +254,7 @@ int pick_chunk(const mc_tvd_state *s, int n_m, long long tiles, int blocks_per_s
 {
     if (s->chunk_override > 0) return s->chunk_override < n_m ? s->chunk_override : n_m;
     const long long slots = (long long)s->sm_count * blocks_per_sm;
-    const int c_max = n_m / 32 > 1 ? n_m / 32 : 1;
+    const int c_max = n_m / 8 > 1 ? n_m / 8 : 1;       // (chunks down to 8 levels: small boxes are bound by the march's latency, not by work)
     long long best_cost = -1;
     int best_chunk = n_m;
     for (int c = 1; c <= c_max; ++c) {
@@ -607,6 +610,58 @@ int mc_tvd_init(const mc_tvd_grid *grid, const mc_tvd_params *params, double *d_
     return MC_TVD_OK;
 }
 
+// Enqueue the launch list of ONE step of Eq. 30 on s->stream: 2 ndim operators + the dt update.
+static int enqueue_one_step(mc_tvd_state *s)
+{
+    const double *src = s->X;
+    double *dst = s->Y;
+    for (int half = 0; half < 2; ++half) {
+        int dir = (half == 1 && s->par.dir_mode == 1) ? -1 : +1;
+        for (int a = 2; a >= 0; --a) {                       // L_z, then L_y, then L_x (Eq. 30)
+            if (s->nd == 2 && a == 1) continue;
+            bool last = (half == 1 && a == 0);
+            int rc = launch_sweep(s, src, dst, a, dir, 0.0, true, last);
+            if (rc != MC_TVD_OK) return rc;
+            const double *t = src; src = dst; dst = (double *)t;
+        }
+    }
+    { auto kfn = mc::k_dt_update; MC_LAUNCH(kfn, 1, 32, 0, s->stream, s->S, 1); }
+    s->launches += 1;
+    s->ev_open = false;
+    return cuda_check(cudaGetLastError(), "dt launch");
+}
+
+// The step's launch list as an instantiated CUDA graph (the list is the same every step: the buffers ping-pong back to
+// d_fields, dt is read from device memory).  Captured once on a private stream (the caller's may be the legacy default
+// stream, which cannot be captured) and replayed on the caller's.  Small boxes are launch-bound: 5-7 launches of a few
+// microseconds each per step.  Returns false (and leaves the plain path to run) if capture is not possible.
+static bool ensure_step_graph(mc_tvd_state *s)
+{
+    if (s->graph_exec && s->graph_chunk == s->chunk_override) return true;
+    if (s->graph_failed) return false;
+    if (s->graph_exec) { cudaGraphExecDestroy(s->graph_exec); s->graph_exec = nullptr; }
+    cudaStream_t cap = nullptr, user = s->stream;
+    cudaGraph_t graph = nullptr;
+    const long long launches0 = s->launches;
+    bool ok = cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking) == cudaSuccess;
+    if (ok) ok = cudaStreamBeginCapture(cap, cudaStreamCaptureModeRelaxed) == cudaSuccess;
+    if (ok) {
+        s->stream = cap;
+        const int rc = enqueue_one_step(s);
+        s->stream = user;
+        const cudaError_t e = cudaStreamEndCapture(cap, &graph);
+        ok = (rc == MC_TVD_OK) && e == cudaSuccess && graph;
+    }
+    s->graph_launches = (int)(s->launches - launches0);
+    s->launches = launches0;                                   // nothing ran yet
+    if (ok) ok = cudaGraphInstantiate(&s->graph_exec, graph, 0) == cudaSuccess;
+    if (graph) cudaGraphDestroy(graph);
+    if (cap) cudaStreamDestroy(cap);
+    if (!ok) { cudaGetLastError(); s->graph_exec = nullptr; s->graph_failed = true; return false; }
+    s->graph_chunk = s->chunk_override;
+    return true;
+}
+
 int mc_tvd_step(mc_tvd_state *s, int n_steps)
 {
     if (!s || n_steps < 0) return fail(MC_TVD_EINVAL, "bad handle or n_steps");
@@ -614,24 +669,18 @@ int mc_tvd_step(mc_tvd_state *s, int n_steps)
         const cudaError_t q = cudaStreamQuery(s->stream);
         if (q != cudaSuccess && q != cudaErrorNotReady) return cuda_check(q, "earlier work on the stream failed");
     }
+    if (s->slab_next != 0) return fail(MC_TVD_EINVAL, "a step enqueued operator by operator (mc_tvd_slab_op) is half done");
+    // per-operator timing records events between the launches: plain launches then
+    const bool graphed = !s->timing && n_steps >= 2 && ensure_step_graph(s);
     for (int it = 0; it < n_steps; ++it) {
-        const double *src = s->X;
-        double *dst = s->Y;
-        for (int half = 0; half < 2; ++half) {
-            int dir = (half == 1 && s->par.dir_mode == 1) ? -1 : +1;
-            for (int a = 2; a >= 0; --a) {                       // L_z, then L_y, then L_x (Eq. 30)
-                if (s->nd == 2 && a == 1) continue;
-                bool last = (half == 1 && a == 0);
-                int rc = launch_sweep(s, src, dst, a, dir, 0.0, true, last);
-                if (rc != MC_TVD_OK) return rc;
-                const double *t = src; src = dst; dst = (double *)t;
-            }
+        if (graphed) {
+            int rc = cuda_check(cudaGraphLaunch(s->graph_exec, s->stream), "step graph launch");
+            if (rc != MC_TVD_OK) return rc;
+            s->launches += s->graph_launches;
+        } else {
+            int rc = enqueue_one_step(s);
+            if (rc != MC_TVD_OK) return rc;
         }
-        { auto kfn = mc::k_dt_update; MC_LAUNCH(kfn, 1, 32, 0, s->stream, s->S, 1); }
-        s->launches += 1;
-        s->ev_open = false;
-        int rc = cuda_check(cudaGetLastError(), "dt launch");
-        if (rc != MC_TVD_OK) return rc;
     }
     return MC_TVD_OK;
 }
@@ -1003,6 +1052,7 @@ int mc_tvd_destroy(mc_tvd_state *s)
 {
     if (!s) return MC_TVD_OK;
     cudaError_t e = cudaStreamSynchronize(s->stream);
+    if (s->graph_exec) cudaGraphExecDestroy(s->graph_exec);
     if (s->ev) for (int i = 0; i < 2 * MC_TVD_MAX_TIMED + 2; ++i) if (s->ev[i]) cudaEventDestroy(s->ev[i]);
     free(s->ev); free(s->rec_kind); free(s->rec_ev);
     delete s;

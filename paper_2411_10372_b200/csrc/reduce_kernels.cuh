@@ -36,10 +36,12 @@ MC_DEV void node_primitives(const PointArgs &P, long long n, int k, double (&X)[
 {
 #pragma unroll
     for (int f = 0; f < ND + 2; ++f) X[f] = P.X[(long long)f * P.N + n];
+    // the same sequence of roundings as cfl_speed (mc_common.cuh), so that this reduction and the one fused into the
+    // step's last operator give the same dt bit for bit (the slab driver uses this one every step)
     double inv = rcp(X[0]), ke = 0.0;
 #pragma unroll
-    for (int c = 0; c < ND; ++c) { u[c] = X[1 + c] * inv; ke += u[c] * u[c]; }
-    T = (X[ND + 1] * inv - 0.5 * ke - point_gz(P, k)) * P.icv;                 // Eq. 17
+    for (int c = 0; c < ND; ++c) { u[c] = X[1 + c] * inv; ke = fma(u[c], u[c], ke); }
+    T = (fma(-0.5, ke, X[ND + 1] * inv) - point_gz(P, k)) * P.icv;             // Eq. 17
 }
 
 // s = max over nodes and directions of (|u_a| + c_s)/dx_a (R12); NaN if rho or T is not positive.
@@ -54,7 +56,7 @@ MC_KERNEL void k_max_speed(PointArgs P, unsigned long long *smax_bits)
         node_primitives<ND>(P, n, k, X, u, T);
         double s = 0.0;
         if (!(X[0] > 0.0) || !(T > 0.0)) s = NAN;
-        double cs = sqrt(P.gamma * P.R * T);
+        double cs = sqrt_pos((P.gamma * P.R) * T);
         // non-uniform z (R19): the cell height; a plate node takes the full adjacent spacing
         const double idz = P.zt ? P.zt[2 * P.nz + k] * ((k == 0 || k == P.nz - 1) ? 0.5 : 1.0) : P.inv_d[ND - 1];
 #pragma unroll

@@ -21,7 +21,8 @@ CASES = {
     "table2-1": dict(ndim=2, Ra=1e4, D=0.49, Gamma=2.0, gamma=5.0 / 3.0, Pr=0.7, eps=0.1, nx=256, ny=1, nz=129,
                      t_spin=150.0, t_avg=50.0, paper=(2.175, 0.005, 26.98, 0.05), ref=(2.1, 26.3), cite="Table 2 case 1"),
     "table2-1-fine": dict(ndim=2, Ra=1e4, D=0.49, Gamma=2.0, gamma=5.0 / 3.0, Pr=0.7, eps=0.1, nx=512, ny=1, nz=257,
-                          cfl=0.2, t_spin=150.0, t_avg=50.0,      # (the diffusive limit binds at this Ra: see "-tanh") paper=(2.175, 0.005, 26.98, 0.05), ref=(2.1, 26.3),
+                          cfl=0.2, t_spin=150.0, t_avg=50.0,      # (the diffusive limit binds at this Ra: see "-tanh")
+                          paper=(2.175, 0.005, 26.98, 0.05), ref=(2.1, 26.3),
                           cite="Table 2 case 1, grid doubled"),
     # the paper's own z grid is tangent-hyperbolic; stretching 1.5 is this repo's choice.  At Ra = 1e4 the
     # plate spacing puts the explicit diffusive limit below the acoustic step of R12, hence the smaller CFL number.

@@ -1,0 +1,73 @@
+"""GPU: the slab decomposition (paper_2411_10372_b200/slab.py over the mc_tvd_slab_* hooks) against the
+undivided box.  All slabs live on this one GPU and run one after the other (`LocalComm`: device copies instead of NCCL
+send/recv; the driver and the kernels are the ones a multi-GPU run uses)."""
+from __future__ import annotations
+
+import numpy as np
+import pytest
+
+from paper_2411_10372_b200 import inputs, slab
+from tests.helpers import parity_err
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    assert torch.cuda.is_available(), "these tests need a CUDA device"
+    from paper_2411_10372_b200 import binding
+    binding.load_library()
+    return binding
+
+
+@pytest.mark.parametrize("ndim,nx,ny,nz,world,stretch", [
+    (3, 64, 48, 33, 2, None), (3, 60, 84, 19, 4, None), (3, 45, 36, 17, 3, 1.5),
+    (2, 480, 1, 65, 4, None), (2, 366, 1, 40, 3, 1.5)])
+def test_slabs_match_the_undivided_box(gpu, orc, ndim, nx, ny, nz, world, stretch):
+    grid = inputs.make_grid(ndim, nx, nz, ny, z_stretch=stretch)
+    params = inputs.make_params(Ra=1e5)
+    X0 = inputs.moving_state(grid, params, amplitude=1e-2, u_amp=0.1)
+    one = gpu.MCTVD(grid, params, X0)
+    drv = slab.make_local_driver(gpu, grid, params, X0, world)
+    n = 4
+    for _ in range(n):
+        # the all-reduced maximum; bit for bit when the local box reproduces the spacing exactly (slab._length_with_spacing)
+        assert drv.dt() == pytest.approx(one.dt(), rel=4e-16)
+        one.step(1)
+        drv.step(1)
+    ref = one.state()
+    got = slab.gather_state(drv.local_states(), grid)
+    # the same kernels on the same numbers; only a tile's position relative to the seam differs (fast / general loop body)
+    assert parity_err(grid, params, got, ref).max() <= 1e-13
+    d1, T1, r1, p1 = one.diagnostics()
+    d2, T2, r2, p2 = drv.diagnostics()
+    for k in ("nu_bottom", "nu_top", "nu_bar", "nu_bulk", "re", "mass", "energy", "max_mach", "min_rho", "min_T"):
+        assert d2[k] == pytest.approx(d1[k], rel=1e-10), k
+    assert d2["time"] == pytest.approx(d1["time"], rel=1e-15) and d2["step"] == d1["step"] == n
+    assert np.allclose(T2, T1, rtol=1e-12) and np.allclose(r2, r1, rtol=1e-12) and np.allclose(p2, p1, rtol=1e-12)
+    # against the oracle too (the undivided box), so that the comparison above is not two wrongs agreeing
+    want, _, _ = orc.step(orc.Problem(grid, params), X0, n)
+    assert parity_err(grid, params, got, want).max() <= 4e-12
+    one.close()
+    for r in drv.ranks:
+        r.close()
+
+
+def test_slab_hooks_reject_misuse(gpu):
+    grid = inputs.make_grid(3, 16, 9, 12)
+    params = inputs.make_params()
+    s = gpu.MCTVD(grid, params, inputs.conduction_state(grid, params))
+    with pytest.raises(gpu.MCTVDError):
+        s.slab_op(1)                                     # operators come in order
+    s.slab_op(0)
+    with pytest.raises(gpu.MCTVDError):
+        s.slab_reduce()                                  # mid-step: the state is not in d_fields
+    with pytest.raises(gpu.MCTVDError):
+        s.slab_commit(True)
+    for op in range(1, 6):
+        s.slab_op(op)
+    s.slab_reduce()
+    s.slab_commit(True)
+    assert s.diagnostics()[0]["step"] == 1
+    s.close()
