@@ -401,9 +401,10 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A, const __grid_co
         }
 
         // (2) TVD (Eqs. 34-39): Dh_{j+1/2} from dX_{j-1/2}, dX_{j+1/2}, dX_{j+3/2}
-        double d1[NF], Dh[NF], Dh1[NF], a1 = 0.0, b1 = 0.0;       // Dh1: the same flux as level j+1 sees it (ZA: other weight)
+        double d1[NF], a1 = 0.0, b1 = 0.0;
+        double cD1 = 0.0;                                          // coefficient of Dh_{j+1/2} = cD1 dX_{j+1/2} as level j+1 sees it
 #pragma unroll
-        for (int f = 0; f < NF; ++f) { Dh[f] = 0.0; Dh1[f] = 0.0; d1[f] = 0.0; }
+        for (int f = 0; f < NF; ++f) d1[f] = 0.0;
         if (ROLE == ROLE_IN && TVD >= 0) {
 #pragma unroll
             for (int f = 0; f < NF; ++f) d1[f] = (ld1 && ld2) ? Xn[f] - Xc[f] : 0.0;
@@ -413,10 +414,10 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A, const __grid_co
             if (have) {
                 const double coef = tvd_coef<(TVD >= 0 ? TVD : 0)>(a0, a1, b0, hC0, hC1);
 #pragma unroll
-                for (int f = 0; f < NF; ++f) {
-                    Dh[f] = (ZA ? coef * tw0 : coef) * d0[f]; H0[f] += Dh[f];
-                    Dh1[f] = ZA ? (coef * tw1) * d0[f] : Dh[f];
-                }
+                const double cD0 = ZA ? coef * tw0 : coef;           // (ZA: the R20 weights of levels j and j+1)
+                cD1 = ZA ? coef * tw1 : coef;
+#pragma unroll
+                for (int f = 0; f < NF; ++f) H0[f] = fma(cD0, d0[f], H0[f]);
             }
         }
 
@@ -449,7 +450,7 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A, const __grid_co
                 for (int f = 0; f < NF; ++f) {
                     const double dF = F1[f] - F0[f];
                     XP[f] = fma(-cdt1, dF, Xc[f]);
-                    H1[f] = fma(-hcdt1, dF, Xc[f]) - Dh1[f];                  // (X^P + X)/2 - Dh
+                    H1[f] = fma(-cD1, d0[f], fma(-hcdt1, dF, Xc[f]));         // (X^P + X)/2 - Dh_{j+1/2}
                 }
                 if (Z_IS_ALPHA) {
                     XP[1 + CA] = fma(tsrc, Xc[0], XP[1 + CA]);
