@@ -1,6 +1,6 @@
 // mc_async.cuh -- sm_100a asynchronous-copy plumbing of the 3-D sweep kernels: TMA tile loads
-// (cp.async.bulk.tensor through a CUtensorMap) completing on shared-memory mbarriers, and mbarriers used as
-// point-to-point "row has published level j" signals between neighbouring warps.  Thin inline-PTX wrappers, no
+// (cp.async.bulk.tensor through a CUtensorMap) completing on shared-memory mbarriers ("full" per stage), and the
+// "empty" mbarriers on which the consumer warps hand a stage back to the producer lane.  Thin inline-PTX wrappers, no
 // arithmetic of the method.
 #pragma once
 

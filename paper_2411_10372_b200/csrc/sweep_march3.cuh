@@ -25,12 +25,14 @@
 // register prefetch (X(j+3) and the ring-2 row: 9 doubles less carried), no L2 prefetch instructions, no
 // per-thread load addresses, and no exposed HBM latency.  Nodes the box cannot deliver -- columns or rows that
 // wrap around the periodic seam -- are zero-filled by the TMA unit and loaded by their thread directly.
-// The per-level __syncthreads is replaced by DATAFLOW between neighbouring rows: each row (warp) owns an
-// mbarrier on which it arrives once it has published u(j+2) and u^P(j+1); before F^P(j+1) it waits only for
-// rows r-1 and r+1.  Neighbouring rows thus stay within one level of each other (which is all the double
-// buffered velocity planes need: see the hazard analysis in DESIGN.md 7), but rows far apart -- and with them
-// the three or four warps sharing an SM sub-partition -- drift by several levels, so one warp's dependent
-// chain overlaps another's instead of all warps draining into the barrier together.
+// The per-level __syncthreads is replaced by DATAFLOW between neighbouring rows: once a row (warp) has published
+// u(j+2) and u^P(j+1) it meets row r-1 and then row r+1 at a hardware named barrier of 64 threads (one barrier per
+// pair of adjacent rows, ids 1 .. WB-1; every row takes its lower pair first, so the chain of rendezvous cannot
+// deadlock).  Neighbouring rows thus stay within one level of each other (which is all the double buffered
+// velocity planes need), but rows far apart -- and with them the three warps sharing an SM sub-partition -- drift
+// by several levels, so one warp's dependent chain overlaps another's instead of all warps draining into one
+// barrier together.  (Measured on C5: block barrier L_z 6.52 / L_y 6.44 ms, an mbarrier pair per row polled with
+// try_wait 6.59 / 6.22, named pair barriers 6.15 / 6.03.)
 #pragma once
 #include <type_traits>
 
@@ -59,7 +61,7 @@ constexpr int MARCH3_STAGES = MC_MARCH3_STAGES;      // power of two
 // dynamic shared memory of k_march3 / k_lane3 with asynchronous staging: stage ring (128-byte aligned) +
 // mbarriers + velocity planes
 __host__ __device__ constexpr size_t tile3_stage_bytes(int WB) { return (size_t)5 * 32 * (WB + 2) * sizeof(double); }
-__host__ __device__ constexpr size_t tile3_async_bytes(int WB) { return MARCH3_STAGES * tile3_stage_bytes(WB) + 8 * (2 * MARCH3_STAGES + 2 * WB); }
+__host__ __device__ constexpr size_t tile3_async_bytes(int WB) { return MARCH3_STAGES * tile3_stage_bytes(WB) + 8 * (2 * MARCH3_STAGES); }
 
 // ZS: non-uniform z grid (R19 / R20; SweepArgs::zt): z is the sweep axis (L_z) or the tile's second direction (L_y).
 template <int CA, int CB, int WB, bool WALL_M, bool WALL_B, int TVD, int MINB = 1, bool AS = false, bool ZS = false>
@@ -70,14 +72,14 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A, const __grid_co
     constexpr bool ZA = ZS && Z_IS_ALPHA;             // the metric varies along the march
     static_assert(!ZS || (Z_IS_ALPHA ? WALL_M : (WALL_B && CB == ND - 1)), "the non-uniform z grid lies between plates");
     constexpr int OB = WB - 2;                        // output rows per tile
-    static_assert(WB >= 3 && WB % 4 == 0, "the SM allocates warps in fours: other row counts waste registers");
+    static_assert(WB >= 3 && WB % 4 == 0 && WB <= 16, "the SM allocates warps in fours; named barriers 1 .. WB-1 pair the rows");
     constexpr int TILE = 32 * (WB + 2);               // shared-memory plane: tile rows plus the ring-2 rows
     constexpr int S = MARCH3_STAGES;
     static_assert((S & (S - 1)) == 0, "stage count must be a power of two");
     MC_SHARED_DECL(double, smem_raw);
-    // AS: [stage ring (the dynamic shared memory is 128-byte aligned)][full[S], empty[S], row[2][WB]][velocity planes]
+    // AS: [stage ring (the dynamic shared memory is 128-byte aligned)][full[S], empty[S]][velocity planes]
     constexpr int RING_DOUBLES = AS ? S * (int)(tile3_stage_bytes(WB) / sizeof(double)) : 0;
-    constexpr int BAR_DOUBLES = AS ? 2 * S + 2 * WB : 0;
+    constexpr int BAR_DOUBLES = AS ? 2 * S : 0;
     const double *const ring = smem_raw;
     double *const bars = smem_raw + RING_DOUBLES;
     double *const smem = smem_raw + RING_DOUBLES + BAR_DOUBLES + 2;   // two pad doubles in front
@@ -204,7 +206,7 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A, const __grid_co
 
 
     // ---- AS: stage ring, barriers ----------------------------------------------------------------
-    const unsigned bar0 = AS ? smem_addr(bars) : 0u;                   // full[S], empty[S], row[WB]
+    const unsigned bar0 = AS ? smem_addr(bars) : 0u;                   // full[S], empty[S]
     const unsigned ring0 = AS ? smem_addr(ring) : 0u;
     const int j_start = (WALL_M && l0 == 0) ? -2 : l0 - 4;             // below a plate there is nothing to warm up
     const int n_lev = l1 + 2 - (j_start + 2);                          // levels j_start+2 .. l1+1 are staged, one per iteration
@@ -224,7 +226,6 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A, const __grid_co
     if (AS) {
         if (threadIdx.x == 0 && threadIdx.y == 0) {
             for (int i = 0; i < S; ++i) { mbar_init(bar0 + 8u * i, 1); mbar_init(bar0 + 8u * (S + i), (unsigned)(ty_hi - ty_lo + 1)); }
-            for (int i = 0; i < 2 * WB; ++i) mbar_init(bar0 + 8u * (2 * S + i), 1);
             mbar_init_fence();
         }
         __syncthreads();
@@ -273,17 +274,12 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A, const __grid_co
             issue(it + S - 1);
         }
     };
-    // AS: the row has published u(j+2), u^P(j+1); wait for the two neighbouring rows to have done the same
+    // AS: the row has published u(j+2), u^P(j+1): rendezvous with the existing neighbour rows, the lower one first
     const bool wait_lo = ty > ty_lo, wait_hi = ty < ty_hi;
-    // two barriers per row, used alternately: a neighbour may complete iteration it + 1 on its OTHER barrier
-    // before this row has observed iteration it, but it + 2 needs this row's arrival for it + 1
     auto level_sync = [&]() MC_INL {
         if (!AS) { __syncthreads(); return; }
-        const unsigned rb = bar0 + 8u * (2 * S + ((unsigned)it & 1u) * WB + ty), ph = ((unsigned)it >> 1) & 1u;
-        __syncwarp();
-        mbar_arrive_if(rb, tx == 0);
-        if (wait_lo) mbar_wait(rb - 8u, ph);
-        if (wait_hi) mbar_wait(rb + 8u, ph);
+        if (wait_lo) asm volatile("barrier.sync.aligned %0, 64;" ::"r"(ty) : "memory");          // pair (ty - 1, ty)
+        if (wait_hi) asm volatile("barrier.sync.aligned %0, 64;" ::"r"(ty + 1) : "memory");      // pair (ty, ty + 1)
     };
 
     // ---- carried state (levels relative to the current output level j) -------------------------
