@@ -210,7 +210,21 @@ int mc_tvd_stats_read_flow(mc_tvd_state *s, mc_tvd_forces *avg, long long *hist_
  *                               [lo, hi) -- the owned rows; the driver all-reduces sums (SUM) and extrema (MAX, MIN);
  *   mc_tvd_slab_diag_finish     the diagnostics from the all-reduced plane sums; nplane_global = nodes per z plane of
  *                               the whole box.  Synchronises.
- * All asynchronous on the handle's stream except the last.  mc_tvd_step on such a handle would use stale halos. */
+ * All asynchronous on the handle's stream except the last.  mc_tvd_step on such a handle would use stale halos.
+ *
+ * Fused halo push (3-D box between plates, even nx, uniform z; MC_TVD_EUNSUPPORTED otherwise): after
+ *   mc_tvd_slab_buffers(s, &X, &Y)    the handle's two state buffers (d_fields and its copy in the workspace), and
+ *   mc_tvd_slab_peers(s, lo_X, lo_Y, hi_X, hi_Y, own_lo, own_hi, halo)
+ * with the same two buffers of the ranks that own the rows below (lo) and above (hi) this slab -- device addresses this
+ * GPU can store to: another slab on the same GPU, or peer-mapped memory of another GPU -- every operator stores only the
+ * owned rows [own_lo, own_hi) of the slab axis y and writes its first / last `halo` owned rows straight into the
+ * neighbours' halo rows from inside the sweep kernel; no exchange between the launches, only a barrier across the ranks
+ * (every rank must have finished operator k before any starts k + 1).  The last operator then carries the CFL
+ * reduction over the owned rows, so mc_tvd_slab_reduce is not needed: all-reduce the maximum and commit.  Four NULLs
+ * switch back to plain operators. */
+int mc_tvd_slab_buffers(mc_tvd_state *s, double **d_fields, double **d_second);
+int mc_tvd_slab_peers(mc_tvd_state *s, double *lo_fields, double *lo_second, double *hi_fields, double *hi_second,
+                      int own_lo, int own_hi, int halo);
 int mc_tvd_slab_op(mc_tvd_state *s, int op);
 int mc_tvd_slab_reduce(mc_tvd_state *s);
 int mc_tvd_slab_commit(mc_tvd_state *s, int advance);

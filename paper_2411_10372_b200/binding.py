@@ -75,6 +75,8 @@ SYMBOLS = {
     "mc_tvd_slab_op": (C.c_int, [C.c_void_p, C.c_int]),
     "mc_tvd_slab_reduce": (C.c_int, [C.c_void_p]),
     "mc_tvd_slab_commit": (C.c_int, [C.c_void_p, C.c_int]),
+    "mc_tvd_slab_buffers": (C.c_int, [C.c_void_p, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p)]),
+    "mc_tvd_slab_peers": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int]),
     "mc_tvd_slab_pointers": (C.c_int, [C.c_void_p, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p), C.POINTER(C.c_void_p),
                                        C.POINTER(C.c_void_p)]),
     "mc_tvd_slab_diag_partial": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int]),
@@ -269,6 +271,19 @@ class MCTVD:
 
     def slab_commit(self, advance: bool):
         self._check(self.lib.mc_tvd_slab_commit(self._h, int(bool(advance))))
+
+    def slab_buffers(self):
+        """Device addresses of the handle's two state buffers (d_fields, its copy in the workspace)."""
+        a, b = C.c_void_p(), C.c_void_p()
+        self._check(self.lib.mc_tvd_slab_buffers(self._h, C.byref(a), C.byref(b)))
+        return a.value, b.value
+
+    def slab_peers(self, lo, hi, own_lo: int, own_hi: int, halo: int):
+        """lo / hi: slab_buffers() of the ranks below / above (None, None switches the fused halo push off)."""
+        if lo is None and hi is None:
+            self._check(self.lib.mc_tvd_slab_peers(self._h, None, None, None, None, 0, 0, 0))
+        else:
+            self._check(self.lib.mc_tvd_slab_peers(self._h, lo[0], lo[1], hi[0], hi[1], int(own_lo), int(own_hi), int(halo)))
 
     def _view(self, ptr: int, count: int, dtype):
         """A torch view of `count` 8-byte elements at device address ptr, which lies inside self.fields or self.workspace."""

@@ -105,6 +105,10 @@ struct mc_tvd_state {
     unsigned long long *flow_hist, *flow_hist_acc;
     bool flow_in_stats;                // samples of mc_tvd_step_stats also accumulate the flow statistics
     int slab_next;                     // mc_tvd_slab_op: the operator of the current step that comes next
+    // fused halo push (mc_tvd_slab_peers): the neighbours' two state buffers [0] = their d_fields, [1] = their workspace copy
+    bool slab_fused;
+    double *peer_lo[2], *peer_hi[2];
+    int own_lo, own_hi, halo;
     cudaGraphExec_t graph_exec;        // one step's launch list (mc_tvd_step replays it), or null
     int graph_launches, graph_chunk;   // kernels in it; the chunk override it was captured with
     bool graph_failed;
@@ -235,6 +239,12 @@ void fill_common(const mc_tvd_state *s, mc::SweepArgs &A, const double *in, doub
             A.mu_h = mu * A.inv_h; A.two_mu_h = 2.0 * mu * A.inv_h; A.lam_mu_h = lam * mu * A.inv_h; A.K_h = s->K * A.inv_h;
         }
     }
+    if (s->slab_fused) {
+        const int b = (out == s->X) ? 0 : 1;                  // the neighbours write the same one of their two buffers
+        A.peer_lo = s->peer_lo[b]; A.peer_hi = s->peer_hi[b];
+        A.own_lo = s->own_lo; A.own_hi = s->own_hi; A.halo = s->halo;
+        A.slab_shift = (long long)(s->own_hi - s->own_lo) * s->grid.nx;      // y rows of nx nodes
+    }
     A.R = s->R; A.cv = s->cv; A.icv = s->icv; A.g = s->g;
     A.gamma = s->par.gamma; A.gammaR = s->par.gamma * s->R;
     A.Tw0 = s->par.T_bot; A.Tw1 = s->par.T_top;
@@ -276,6 +286,12 @@ template <class F> void with_bool(bool b, F f)
 template <class W, class F> void with_zs(const mc_tvd_state *s, W, F f)
 {
     if constexpr (W::value) { if (s->zt) { f(std::true_type()); return; } }
+    f(std::false_type());
+}
+// the fused halo push exists for the TMA-staged 3-D kernels between plates on a uniform z grid
+template <class W, class Z, class F> void with_sl(const mc_tvd_state *s, W, Z, F f)
+{
+    if constexpr (W::value && !Z::value) { if (s->slab_fused) { f(std::true_type()); return; } }
     f(std::false_type());
 }
 // MC_ONLY_DEFAULT_SWITCHES (tuning builds only): instantiate just the plates + Davis/Yee kernels
@@ -397,9 +413,9 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
             A.chunk = pick_chunk(s, nz, xt * bt, 1);
             dim3 mblock(32, MW, 1), grid((unsigned)xt, (unsigned)bt, (unsigned)((nz + A.chunk - 1) / A.chunk));
             size_t smem = mc::tile3_async_bytes(MW) + ((size_t)4 * 3 * 32 * (MW + 2) + 4) * sizeof(double);
-            with_walls(wl, [&](auto W) { with_tvd(s, [&](auto T) { with_zs(s, W, [&](auto Z) {
-                launch_kernel(mc::k_march3<2, 1, MW, decltype(W)::value, false, decltype(T)::value, 1, true, decltype(Z)::value>, grid, mblock, smem, st, A, s->tm_rows_y[ibuf]);
-            }); }); });
+            with_walls(wl, [&](auto W) { with_tvd(s, [&](auto T) { with_zs(s, W, [&](auto Z) { with_sl(s, W, Z, [&](auto L) {
+                launch_kernel(mc::k_march3<2, 1, MW, decltype(W)::value, false, decltype(T)::value, 1, true, decltype(Z)::value, decltype(L)::value>, grid, mblock, smem, st, A, s->tm_rows_y[ibuf]);
+            }); }); }); });
         } else if (alpha == 1 && s->async3) {   // y-sweep, TMA-staged tiles: march y, tile (x, z)
             constexpr int MW = MARCH3_WB_AS, MO = MW - 2;
             A.n_b = nz; A.s_b = (long long)nx * ny; A.n_m = ny; A.s_m = nx;
@@ -408,9 +424,9 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
             A.chunk = pick_chunk(s, ny, xt * bt, 1);
             dim3 mblock(32, MW, 1), grid((unsigned)xt, (unsigned)bt, (unsigned)((ny + A.chunk - 1) / A.chunk));
             size_t smem = mc::tile3_async_bytes(MW) + ((size_t)4 * 3 * 32 * (MW + 2) + 4) * sizeof(double);
-            with_walls(wl, [&](auto W) { with_tvd(s, [&](auto T) { with_zs(s, W, [&](auto Z) {
-                launch_kernel(mc::k_march3<1, 2, MW, false, decltype(W)::value, decltype(T)::value, 1, true, decltype(Z)::value>, grid, mblock, smem, st, A, s->tm_rows_z[ibuf]);
-            }); }); });
+            with_walls(wl, [&](auto W) { with_tvd(s, [&](auto T) { with_zs(s, W, [&](auto Z) { with_sl(s, W, Z, [&](auto L) {
+                launch_kernel(mc::k_march3<1, 2, MW, false, decltype(W)::value, decltype(T)::value, 1, true, decltype(Z)::value, decltype(L)::value>, grid, mblock, smem, st, A, s->tm_rows_z[ibuf]);
+            }); }); }); });
         } else if (alpha == 2) {            // z-sweep: march z, tile (x, y)
             constexpr int MW = MARCH3_WB, MO = MW - 2;
             A.n_b = ny; A.s_b = nx; A.n_m = nz; A.s_m = (long long)nx * ny;
@@ -441,9 +457,9 @@ int launch_sweep(mc_tvd_state *s, const double *in, double *out, int alpha, int 
             A.chunk = pick_chunk(s, nz, xt * bt, 1);
             dim3 lblock(32, LW, 1), grid((unsigned)xt, (unsigned)bt, (unsigned)((nz + A.chunk - 1) / A.chunk));
             size_t smem = (size_t)4 * 2 * 32 * (LW + 2) * sizeof(double);
-            with_walls(wl, [&](auto W) { with_tvd(s, [&](auto T) { with_bool(reduce, [&](auto Rd) { with_zs(s, W, [&](auto Z) {
-                launch_kernel(mc::k_lane3<1, 2, LW, decltype(W)::value, decltype(T)::value, decltype(Rd)::value, decltype(Z)::value>, grid, lblock, smem, st, A);
-            }); }); }); });
+            with_walls(wl, [&](auto W) { with_tvd(s, [&](auto T) { with_bool(reduce, [&](auto Rd) { with_zs(s, W, [&](auto Z) { with_sl(s, W, Z, [&](auto L) {
+                launch_kernel(mc::k_lane3<1, 2, LW, decltype(W)::value, decltype(T)::value, decltype(Rd)::value, decltype(Z)::value, decltype(L)::value>, grid, lblock, smem, st, A);
+            }); }); }); }); });
         }
     }
     s->geom[alpha][0] = geo_x; s->geom[alpha][1] = geo_b; s->geom[alpha][2] = A.chunk;
@@ -851,7 +867,9 @@ int mc_tvd_slab_op(mc_tvd_state *s, int op)
     const int dir = (half == 1 && s->par.dir_mode == 1) ? -1 : +1;
     const double *src = (op % 2 == 0) ? s->X : s->Y;
     double *dst = (op % 2 == 0) ? s->Y : s->X;
-    int rc = launch_sweep(s, src, dst, a, dir, 0.0, true, false);   // no fused CFL reduction: the halo copies are stale here
+    // the CFL reduction is fused into the last operator only where it can be restricted to the owned rows (fused halo
+    // push); otherwise the halo copies are stale here and mc_tvd_slab_reduce follows the last exchange
+    int rc = launch_sweep(s, src, dst, a, dir, 0.0, true, s->slab_fused && op == nops - 1);
     s->ev_open = false;
     if (rc == MC_TVD_OK) s->slab_next = op + 1;
     return rc;
@@ -878,6 +896,32 @@ int mc_tvd_slab_commit(mc_tvd_state *s, int advance)
     s->launches += 1;
     if (advance) s->slab_next = 0;
     return cuda_check(cudaGetLastError(), "dt launch");
+}
+
+int mc_tvd_slab_buffers(mc_tvd_state *s, double **d_fields, double **d_second)
+{
+    if (!s || !d_fields || !d_second) return fail(MC_TVD_EINVAL, "bad handle or output pointer");
+    *d_fields = s->X; *d_second = s->Y;
+    return MC_TVD_OK;
+}
+
+int mc_tvd_slab_peers(mc_tvd_state *s, double *lo_fields, double *lo_second, double *hi_fields, double *hi_second,
+                      int own_lo, int own_hi, int halo)
+{
+    if (!s) return fail(MC_TVD_EINVAL, "bad handle");
+    if (!lo_fields && !lo_second && !hi_fields && !hi_second) { s->slab_fused = false; return MC_TVD_OK; }
+    if (!lo_fields || !lo_second || !hi_fields || !hi_second) return fail(MC_TVD_EINVAL, "all four peer buffers or none");
+    if (s->nd != 3 || !s->async3 || s->zt || !s->walls) {
+        fail(MC_TVD_EUNSUPPORTED, "the fused halo push serves the 3-D box between plates with an even nx on a uniform z grid");
+        return MC_TVD_EUNSUPPORTED;
+    }
+    if (halo < 2 || own_lo != halo || own_hi <= own_lo + 2 * halo - 1 || own_hi + halo != s->grid.ny)
+        return fail(MC_TVD_EINVAL, "owned rows [own_lo, own_hi) must sit between two halos of >= 2 rows each");
+    if (s->slab_next != 0) return fail(MC_TVD_EINVAL, "a step is half done");
+    s->peer_lo[0] = lo_fields; s->peer_lo[1] = lo_second; s->peer_hi[0] = hi_fields; s->peer_hi[1] = hi_second;
+    s->own_lo = own_lo; s->own_hi = own_hi; s->halo = halo;
+    s->slab_fused = true;
+    return MC_TVD_OK;
 }
 
 int mc_tvd_slab_pointers(mc_tvd_state *s, double **fields_now, unsigned long long **smax_bits, double **plane_sums,

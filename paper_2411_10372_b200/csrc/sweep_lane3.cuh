@@ -27,7 +27,9 @@ namespace mc {
 // direction m (z); WB: warps (rows) per block; WALL_M: m is z with plates; TVD: -1 / 0 / 1 as in
 // k_march; REDUCE: fold the CFL max-reduction of the output into the epilogue (R12).  alpha is x.
 // ZS: non-uniform z grid (R19; SweepArgs::zt): z is the marching direction, a cross direction of this sweep.
-template <int CB, int CM, int WB, bool WALL_M, int TVD, bool REDUCE, bool ZS = false>
+// SL: this box is one slab of a larger one (y is the slab axis): store the owned rows only, push the boundary rows into
+// the neighbours' halos (SweepArgs::peer_*), and reduce the CFL maximum over the owned rows only.
+template <int CB, int CM, int WB, bool WALL_M, int TVD, bool REDUCE, bool ZS = false, bool SL = false>
 MC_KERNEL void __maxnreg__(((65536 / (32 * WB)) / 8 * 8) > 248 ? 248 : ((65536 / (32 * WB)) / 8 * 8)) k_lane3(SweepArgs A)
 {
     constexpr int ND = 3, NF = 5;
@@ -56,7 +58,8 @@ MC_KERNEL void __maxnreg__(((65536 / (32 * WB)) / 8 * 8) > 248 ? 248 : ((65536 /
     const unsigned off_base = (unsigned)(ix + (long long)wrap(gb, A.n_b) * A.s_b);
     const unsigned off_base_o = (unsigned)(ix + (long long)wrap(go, A.n_b) * A.s_b);
     const int tidx_o = tidx + (ty == 0 ? -32 : 32);
-    const bool owner = warp_on && !edge && gb < A.n_b && xi >= 2 && xi < 2 + LANE_OUT && gx >= 0 && gx < A.nx;
+    const SlabRows srow = SL ? slab_rows(A, gb) : SlabRows{true, false, false};
+    const bool owner = warp_on && !edge && gb < A.n_b && xi >= 2 && xi < 2 + LANE_OUT && gx >= 0 && gx < A.nx && srow.mine;
 
     // ---- sweep constants ------------------------------------------------------------------
     const double tau = A.dt_ptr ? 0.5 * (*A.dt_ptr) : A.tau_fixed;
@@ -248,6 +251,7 @@ MC_KERNEL void __maxnreg__(((65536 / (32 * WB)) / 8 * 8) > 248 ? 248 : ((65536 /
                     const unsigned oo = FAST ? o0c : off_base + (unsigned)lev(j) * sm;
 #pragma unroll
                     for (int f = 0; f < NF; ++f) outb[f][oo] = o[f];
+                    if (SL) slab_push<NF>(A, srow, oo, o);
                 }
                 if (REDUCE) {                                        // CFL max-reduction of the new state (R12)
                     const double gzj = gz0;

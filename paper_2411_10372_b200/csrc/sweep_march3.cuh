@@ -64,7 +64,9 @@ __host__ __device__ constexpr size_t tile3_stage_bytes(int WB) { return (size_t)
 __host__ __device__ constexpr size_t tile3_async_bytes(int WB) { return MARCH3_STAGES * tile3_stage_bytes(WB) + 8 * (2 * MARCH3_STAGES); }
 
 // ZS: non-uniform z grid (R19 / R20; SweepArgs::zt): z is the sweep axis (L_z) or the tile's second direction (L_y).
-template <int CA, int CB, int WB, bool WALL_M, bool WALL_B, int TVD, int MINB = 1, bool AS = false, bool ZS = false>
+// SL: this box is one slab of a larger one (y is the slab axis: the tile's b for L_z, the march itself for L_y): store the
+// owned rows only and push the boundary rows into the neighbours' halos (SweepArgs::peer_*).
+template <int CA, int CB, int WB, bool WALL_M, bool WALL_B, int TVD, int MINB = 1, bool AS = false, bool ZS = false, bool SL = false>
 MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A, const __grid_constant__ CUtensorMap tmap)
 {
     constexpr int ND = 3, NF = 5;
@@ -112,7 +114,9 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A, const __grid_co
     const long long col = ix + (long long)gb * A.s_b;
     const long long col_o = ix + (long long)go * A.s_b;
     const int tidx_o = tidx + (ty == 0 ? -32 : 32);
-    const bool owner = row_exists && rx >= 2 && !edge && gx < A.nx && gb_raw < A.n_b;
+    constexpr bool SL_B = SL && CB == 1, SL_M = SL && CA == 1;        // the slab axis y is b (L_z) or the march (L_y)
+    const SlabRows srow_b = SL_B ? slab_rows(A, gb_raw) : SlabRows{true, false, false};
+    const bool owner = row_exists && rx >= 2 && !edge && gx < A.nx && gb_raw < A.n_b && srow_b.mine;
     int role = ROLE_IN;
     if (!row_exists) role = ROLE_NONE;
     else if (wallrow) role = ROLE_WALLROW;
@@ -174,9 +178,14 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A, const __grid_co
 #pragma unroll
         for (int f = 0; f <= ND; ++f) X[f] = inb[f][o];
     };
-    auto store_at = [&](unsigned o, const double (&v)[NF]) MC_INL {
+    // (SL: `l` is the marching level of the node, which is its y index in L_y)
+    auto store_at = [&](unsigned o, const double (&v)[NF], int l) MC_INL {
+        const SlabRows r = SL_M ? slab_rows(A, phys_k(l)) : srow_b;
+        if (!SL || r.mine) {
 #pragma unroll
-        for (int f = 0; f < NF; ++f) outb[f][o] = v[f];
+            for (int f = 0; f < NF; ++f) outb[f][o] = v[f];
+        }
+        if (SL) slab_push<NF>(A, r, o, v);
     };
     auto publish = [&](double *slot, int parity, int at, const double (&u)[ND]) MC_INL {
 #pragma unroll
@@ -387,7 +396,7 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A, const __grid_co
             // a plate row of b (y-sweep): X^P = X and the output is X (R10); publish u^P = u of level j+1
             if (ld1) publish(slotP, p1, tidx, w1.u);
             level_sync();
-            if (j >= l0 && owner) store_at(o0, H0);
+            if (j >= l0 && owner) store_at(o0, H0, j);
 #pragma unroll
             for (int f = 0; f < NF; ++f) { H0[f] = Xc[f]; Xc[f] = Xn[f]; if (!AS) Xn[f] = Xq[f]; }
             w1 = w2;
@@ -494,7 +503,7 @@ MC_KERNEL void __maxnreg__(MC_MARCH3_REGS) k_march3(SweepArgs A, const __grid_co
 #pragma unroll
                     for (int f = 0; f < NF; ++f) o[f] = fma(-hcdt0, FP1[f], H0[f]);
                 }
-                if (owner) store_at(o0, o);
+                if (owner) store_at(o0, o, j);
             }
 #pragma unroll
             for (int f = 0; f < NF; ++f) { H1[f] = fma(hcdt1, FP1[f], H1[f]); d0[f] = d1[f]; }

@@ -97,6 +97,14 @@ class LocalComm:
             f.narrow(dim, 0, halo).copy_(hi[(r - 1) % w])
             f.narrow(dim, halo + own, halo).copy_(lo[(r + 1) % w])
 
+    def barrier(self, tensors):
+        """Every slab's queued work has finished (one device and one stream: stream order already says so)."""
+        import torch
+        devs = {t.device for t in tensors if t.is_cuda}
+        if len(devs) > 1:
+            for d in devs:
+                torch.cuda.synchronize(d)
+
     def allreduce(self, tensors, op: str):
         import torch
         red = {"max": torch.maximum, "min": torch.minimum, "sum": torch.add}[op]
@@ -153,12 +161,28 @@ class DistComm:
 class SlabDriver:
     """Runs the local slabs `ranks` (objects with the slab_* methods of binding.MCTVD) as one box through `comm`."""
 
-    def __init__(self, ranks, comm, grid: dict, halo: int = HALO):
+    def __init__(self, ranks, comm, grid: dict, halo: int = HALO, fused: bool = False):
         self.ranks, self.comm, self.grid, self.halo = list(ranks), comm, dict(grid), halo
         self.dim = 2 if slab_axis(grid) == "y" else 3
         _, self.own = local_grid(grid, comm.world, halo)
         self.nops = 2 * int(grid["ndim"])
+        self.fused = False
+        if fused:
+            self.enable_fused()
         self._refresh_dt(advance=False)        # the initial dt must be the global one
+
+    def enable_fused(self):
+        """Fused halo push (include/mc_tvd.h): every operator writes its boundary rows straight into the neighbours' halo
+        rows, so nothing is exchanged between the launches.  The neighbours' buffers must be addressable from this
+        process (`LocalComm`: the same GPU, or GPUs of this process with peer access); raises where the library does
+        not support it (2-D, odd nx, non-uniform z)."""
+        if not isinstance(self.comm, LocalComm):
+            raise NotImplementedError("the fused halo push needs the neighbours' device addresses: all slabs in one process")
+        bufs = [r.slab_buffers() for r in self.ranks]
+        w = len(self.ranks)
+        for i, r in enumerate(self.ranks):
+            r.slab_peers(bufs[(i - 1) % w], bufs[(i + 1) % w], self.halo, self.halo + self.own, self.halo)
+        self.fused = True
 
     def _fields(self):
         return [r.slab_views()[0] for r in self.ranks]
@@ -176,8 +200,16 @@ class SlabDriver:
             for op in range(self.nops):
                 for r in self.ranks:
                     r.slab_op(op)
-                self.comm.exchange(self._fields(), self.dim, self.halo, self.own)
-            self._refresh_dt(advance=True)
+                if self.fused:
+                    self.comm.barrier(self._fields())      # the kernels have pushed the halos themselves
+                else:
+                    self.comm.exchange(self._fields(), self.dim, self.halo, self.own)
+            if self.fused:                                  # the last operator reduced the maximum over the owned rows
+                self.comm.allreduce([r.slab_views()[1] for r in self.ranks], "max")
+                for r in self.ranks:
+                    r.slab_commit(True)
+            else:
+                self._refresh_dt(advance=True)
 
     def dt(self) -> float:
         return self.ranks[0].dt()
@@ -199,7 +231,8 @@ class SlabDriver:
         return [r.state() for r in self.ranks]
 
 
-def make_local_driver(binding, grid: dict, params: dict, X0: np.ndarray, n_slabs: int, device="cuda:0", devices=None):
+def make_local_driver(binding, grid: dict, params: dict, X0: np.ndarray, n_slabs: int, device="cuda:0", devices=None,
+                      fused: bool = False):
     """All slabs driven by this process.  One device (default): the slabs run one after the other, the single-GPU
     emulation of the multi-GPU path.  devices = ["cuda:0", "cuda:1", ...] (one per slab): a single process drives several
     GPUs and `LocalComm`'s copies become peer-to-peer copies over NVLink (never run here: this box has one GPU)."""
@@ -207,7 +240,7 @@ def make_local_driver(binding, grid: dict, params: dict, X0: np.ndarray, n_slabs
     devs = list(devices) if devices is not None else [device] * n_slabs
     assert len(devs) == n_slabs
     ranks = [binding.MCTVD(gl, params, scatter_state(X0, grid, r, n_slabs), device=devs[r]) for r in range(n_slabs)]
-    return SlabDriver(ranks, LocalComm(n_slabs), grid)
+    return SlabDriver(ranks, LocalComm(n_slabs), grid, fused=fused)
 
 
 def make_dist_driver(binding, grid: dict, params: dict, X0: np.ndarray, device, group=None):

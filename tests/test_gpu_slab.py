@@ -54,6 +54,44 @@ def test_slabs_match_the_undivided_box(gpu, orc, ndim, nx, ny, nz, world, stretc
         r.close()
 
 
+@pytest.mark.parametrize("nx,ny,nz,world", [(64, 48, 33, 2), (60, 84, 19, 4), (56, 8, 12, 1)])
+def test_fused_halo_push_matches_the_undivided_box(gpu, orc, nx, ny, nz, world):
+    """mc_tvd_slab_peers: the sweep kernels store their owned rows and push the boundary rows into the neighbours' halos
+    themselves; no copies between the launches, the CFL maximum reduced inside the last operator over the owned rows."""
+    grid = inputs.make_grid(3, nx, nz, ny)
+    params = inputs.make_params(Ra=1e5)
+    X0 = inputs.moving_state(grid, params, amplitude=1e-2, u_amp=0.1)
+    one = gpu.MCTVD(grid, params, X0)
+    drv = slab.make_local_driver(gpu, grid, params, X0, world, fused=True)
+    assert drv.fused
+    n = 4
+    for _ in range(n):
+        assert drv.dt() == pytest.approx(one.dt(), rel=4e-16)
+        one.step(1)
+        drv.step(1)
+    got = slab.gather_state(drv.local_states(), grid)
+    assert parity_err(grid, params, got, one.state()).max() <= 1e-13
+    want, _, _ = orc.step(orc.Problem(grid, params), X0, n)
+    assert parity_err(grid, params, got, want).max() <= 4e-12
+    for r, st in enumerate(drv.local_states()):              # the halo rows hold the neighbours' rows (pushed by them)
+        assert parity_err(slab.local_grid(grid, world)[0], params, st, slab.scatter_state(got, grid, r, world)).max() <= 1e-15
+    d1, d2 = one.diagnostics()[0], drv.diagnostics()[0]
+    for k in ("nu_bar", "nu_bulk", "re", "mass"):
+        assert d2[k] == pytest.approx(d1[k], rel=1e-10), k
+    one.close()
+    for r in drv.ranks:
+        r.close()
+
+
+def test_fused_halo_push_is_refused_where_it_is_not_built(gpu):
+    for grid in (inputs.make_grid(2, 64, 17), inputs.make_grid(3, 45, 17, 24), inputs.make_grid(3, 32, 17, 24, z_stretch=1.5)):
+        params = inputs.make_params()
+        X0 = inputs.conduction_state(grid, params)
+        with pytest.raises(gpu.MCTVDError) as e:
+            slab.make_local_driver(gpu, grid, params, X0, 2, fused=True)
+        assert e.value.code == -5
+
+
 def test_slab_hooks_reject_misuse(gpu):
     grid = inputs.make_grid(3, 16, 9, 12)
     params = inputs.make_params()
