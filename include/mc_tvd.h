@@ -7,8 +7,11 @@
  * form PAPER.md:255-263, Eqs. 27-28) by the operator-split MacCormack predictor-corrector scheme with
  * a TVD correction (Eqs. 29-39), chooses the time step by an acoustic CFL rule
  * (reading R12; the paper is silent) and evaluates the Nusselt / Reynolds diagnostics
- * (Eqs. 22-26).  Every step of that path runs in CUDA kernels; there is no CPU
- * fallback.  All arithmetic is fp64.
+ * (Eqs. 22-26).  Around that path: the paper's non-uniform z grid (mc_tvd_grid.z_nodes,
+ * PAPER.md:249), device-resident time averages (mc_tvd_stats_*), the flow statistics of
+ * Sec. 5-6 (mc_tvd_flow_stats: Eqs. 40-43, the ratio K_e / I_e), and hooks for running one box as slabs over
+ * several GPUs (mc_tvd_slab_*).  Every step of all of it runs in CUDA kernels; there is no CPU fallback.  All
+ * arithmetic is fp64.
  *
  * Conventions
  *   - Plain C: POD structs, raw pointers, sizes.  No torch / C++ types.  "d_" = DEVICE pointer,
@@ -16,7 +19,7 @@
  *   - Field layout (device): nf = 4 (2-D: rho, rho u_x, rho u_z, E) or 5 (3-D: rho, rho u_x,
  *     rho u_y, rho u_z, E) arrays of N = nx*ny*nz doubles, one after the other (SoA); node (i,j,k)
  *     at (k*ny + j)*nx + i; x fastest.  x_i = i lx/nx and y_j = j ly/ny are periodic; z_k = k lz/(nz-1)
- *     with k = 0 and k = nz-1 ON the plates (z_k = k lz/nz when bc_z = 1).
+ *     with k = 0 and k = nz-1 ON the plates (z_k = k lz/nz when bc_z = 1), or the caller's node heights.
  *   - Ownership: the caller owns every device buffer (d_fields, d_workspace) and the stream; the
  *     library owns only the host-side handle.  d_fields and d_workspace must stay valid and must
  *     not be touched by the caller between a call and the next stream synchronisation.

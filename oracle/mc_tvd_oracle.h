@@ -7,7 +7,7 @@
  * (Eqs. 22-26).  It follows the paper's algorithm step by
  * step, in the paper's order and notation: whole-array passes, no blocking,
  * no fusion, no reordering.  Where the paper is silent or garbled it takes
- * the readings listed in DESIGN.md ("Readings of the paper", R1..R18).
+ * the readings listed in DESIGN.md ("Readings of the paper", R1..R21).
  *
  * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
  * --impl reference legs may call this.  It shares no code, header, table or
@@ -19,9 +19,15 @@
  * attenuation, hydrostatic conduction state, closed-form diagnostics,
  * axis-permutation identities, stationary contact (Eqs. 34-39 in closed form),
  * one-operator Taylor expansion with gravity (S^P of Eq. 32), compact viscous
- * stencil rate (R7), operator sequence of Eq. 30.  Parity unpinned: R11 only
- * (TVD flux dropped on plate-adjacent interfaces; the paper is silent) -- see
- * DESIGN.md.
+ * stencil rate (R7), operator sequence of Eq. 30; the non-uniform z grid (R19:
+ * uniform heights give the uniform scheme, mass to round-off, second-order
+ * hydrostatic drift / viscous decay / mixed stress derivative, exact plate
+ * gradients for a quadratic, dt rule); the flow statistics (R21: second-order
+ * convergence to the symbolically differentiated Eqs. 40-43, histogram bins).
+ * Parity unpinned: R11 (TVD flux dropped on plate-adjacent interfaces) and the
+ * interface weight of R20 (TVD term on the non-uniform grid): the paper is
+ * silent on both and no mathematical criterion decides; each has a test that
+ * records its closed form -- see DESIGN.md.
  *
  * Field layout (all calls): nf = 4 (2-D: rho, rho*u_x, rho*u_z, E) or
  * nf = 5 (3-D: rho, rho*u_x, rho*u_y, rho*u_z, E) arrays of N = nx*ny*nz
