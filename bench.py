@@ -456,7 +456,7 @@ def main():
     args = parse_args()
     if args.impl == "reference":
         run_reference(args)
-    elif args.slabs and int(os.environ.get("WORLD_SIZE", "1")) > 1:
+    elif args.slabs and "WORLD_SIZE" in os.environ:            # under torchrun (any world size, 1 included)
         run_slabs(args)
     else:
         run_ours(args)

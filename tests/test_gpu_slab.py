@@ -92,6 +92,29 @@ def test_fused_halo_push_is_refused_where_it_is_not_built(gpu):
         assert e.value.code == -5
 
 
+def test_bench_slabs_mode_runs_under_a_one_rank_nccl_group():
+    """bench.py --slabs through torch.distributed with the NCCL backend and a world of one rank (this box has one GPU):
+    the DistComm code path (process group, all_reduce of the CFL maximum, the local wrap of the halos) end to end."""
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = dict(os.environ, RANK="0", LOCAL_RANK="0", WORLD_SIZE="1", MASTER_ADDR="127.0.0.1",
+               MASTER_PORT=str(24000 + os.getpid() % 3000))
+    res = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--slabs", "--workload", "C1", "--steps", "5",
+                          "--warmup", "3"], capture_output=True, text=True, timeout=600, cwd=root, env=env)
+    assert res.returncode == 0, res.stderr[-2000:]
+    rec = json.loads([l for l in res.stdout.splitlines() if l.startswith("{")][-1])
+    assert rec["scaling"] == "strong" and rec["n_gpus"] == 1 and rec["value"] > 0 and rec["state_check"]["dt"] > 0
+    ref = subprocess.run([sys.executable, "-c",
+                          "from paper_2411_10372_b200 import binding, inputs\n"
+                          "g, p, _ = inputs.config('C1'); s = binding.MCTVD(g, p, inputs.conduction_state(g, p)); s.step(8); print(repr(s.dt()))"],
+                         capture_output=True, text=True, timeout=600, cwd=root)
+    assert ref.returncode == 0, ref.stderr[-2000:]
+    assert rec["state_check"]["dt"] == pytest.approx(float(ref.stdout.strip().splitlines()[-1]), rel=1e-14)   # 3 + 5 steps
+
+
 def test_slab_hooks_reject_misuse(gpu):
     grid = inputs.make_grid(3, 16, 9, 12)
     params = inputs.make_params()
