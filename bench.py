@@ -51,6 +51,9 @@ def parse_args():
     ap.add_argument("--slabs", action="store_true",
                     help="N > 1 only: ONE box cut into N slabs (paper_2411_10372_b200/slab.py, halo exchange over NCCL) instead "
                          "of N replicas; strong scaling.  Built and parity-tested, never timed on more than one GPU")
+    ap.add_argument("--fused-halo", action="store_true",
+                    help="with --slabs: the sweep kernels push their boundary rows into the neighbours' halos themselves "
+                         "(CUDA-IPC-mapped peer buffers) instead of NCCL send/recv between the launches (3-D, even nx)")
     return ap.parse_args()
 
 
@@ -427,7 +430,7 @@ def run_slabs(args):
     name = args.workload
     grid, params, _ = inputs.config(name)
     X0 = inputs.conduction_state(grid, params)
-    drv = slab.make_dist_driver(binding, grid, params, X0, device=f"cuda:{local}")
+    drv = slab.make_dist_driver(binding, grid, params, X0, device=f"cuda:{local}", fused=args.fused_halo)
     del X0
     drv.step(args.warmup)
     dist.barrier(); torch.cuda.synchronize()
@@ -447,7 +450,8 @@ def run_slabs(args):
             "vs_baseline": None, "dtype": "f64",
             "data": "synthetic (seeded hydrostatic conduction state + T noise, DESIGN.md input recipe)",
             "config": dict(workload_config(name, grid, params), decomposition=f"{world} slabs along {slab.slab_axis(grid)}, halo 2, "
-                           "exchange after every operator (NCCL send/recv), dt all-reduce"),
+                           + ("halo rows pushed by the sweep kernels into the neighbours' buffers (CUDA IPC), a barrier per operator"
+                              if args.fused_halo else "exchange after every operator (NCCL send/recv)") + ", dt all-reduce"),
             "clocks": clocks.summary(), "gpu_launches": int(drv.ranks[0].launch_count()), "state_check": {"dt": dt_now}}), flush=True)
     dist.destroy_process_group()
 

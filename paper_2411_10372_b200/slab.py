@@ -97,6 +97,12 @@ class LocalComm:
             f.narrow(dim, 0, halo).copy_(hi[(r - 1) % w])
             f.narrow(dim, halo + own, halo).copy_(lo[(r + 1) % w])
 
+    def neighbour_buffers(self, ranks):
+        """Per slab: the (d_fields, second buffer) device addresses of the slab below and of the slab above."""
+        bufs = [r.slab_buffers() for r in ranks]
+        w = len(ranks)
+        return [(bufs[(i - 1) % w], bufs[(i + 1) % w]) for i in range(w)]
+
     def barrier(self, tensors):
         """Every slab's queued work has finished (one device and one stream: stream order already says so)."""
         import torch
@@ -129,6 +135,8 @@ class DistComm:
         left, right = (self.rank0 - 1) % self.world, (self.rank0 + 1) % self.world
         lo = f.narrow(dim, halo, halo).contiguous()
         hi = f.narrow(dim, own, halo).contiguous()
+        if f.is_cuda and self.world > 1 and dist.get_backend(self.group) == "gloo":
+            lo, hi = lo.cpu(), hi.cpu()          # gloo moves host memory only (tests; NCCL sends device memory)
         if self.world == 1:
             f.narrow(dim, 0, halo).copy_(hi)
             f.narrow(dim, halo + own, halo).copy_(lo)
@@ -149,12 +157,42 @@ class DistComm:
         f.narrow(dim, 0, halo).copy_(from_hi)                  # left neighbour's last owned rows
         f.narrow(dim, halo + own, halo).copy_(from_lo)         # right neighbour's first owned rows
 
+    def neighbour_buffers(self, ranks):
+        """The neighbouring PROCESSES' state buffers, opened through CUDA IPC (torch's tensor sharing): each rank
+        publishes its two tensors, opens those of the ranks below and above and returns their addresses in its own
+        address space.  Same node only; on several GPUs the mapping is peer memory, the stores travel over NVLink."""
+        from torch.multiprocessing.reductions import reduce_tensor
+        (r,) = ranks
+        X, Y = r.slab_buffers()
+        if self.world == 1:
+            return [((X, Y), (X, Y))]
+        mine = (reduce_tensor(r.fields), reduce_tensor(r.workspace), X - r.fields.data_ptr(), Y - r.workspace.data_ptr())
+        everyone = [None] * self.world
+        self.dist.all_gather_object(everyone, mine, group=self.group)
+        self._ipc = []                                       # keep the opened tensors alive as long as the driver
+        out = []
+        for nb in ((self.rank0 - 1) % self.world, (self.rank0 + 1) % self.world):
+            (ff, fa), (wf, wa), offx, offy = everyone[nb]
+            tf, tw = ff(*fa), wf(*wa)
+            self._ipc += [tf, tw]
+            out.append((tf.data_ptr() + offx, tw.data_ptr() + offy))
+        return [(out[0], out[1])]
+
+    def barrier(self, tensors):
+        """Every rank's queued work has finished: the operator's pushes have landed before anyone reads them."""
+        import torch
+        for t in tensors:
+            if t.is_cuda:
+                torch.cuda.synchronize(t.device)
+        self.dist.barrier(group=self.group)
+
     def allreduce(self, tensors, op: str):
         dist, (t,) = self.dist, tensors
         red = {"max": dist.ReduceOp.MAX, "min": dist.ReduceOp.MIN, "sum": dist.ReduceOp.SUM}[op]
-        buf = t.contiguous()
+        on_host = t.is_cuda and dist.get_backend(self.group) == "gloo"     # (the CPU tests' backend, and the two-process-one-GPU test)
+        buf = t.detach().cpu().contiguous() if on_host else t.contiguous()
         dist.all_reduce(buf, op=red, group=self.group)
-        if buf.data_ptr() != t.data_ptr():
+        if on_host or buf.data_ptr() != t.data_ptr():
             t.copy_(buf)
 
 
@@ -173,15 +211,11 @@ class SlabDriver:
 
     def enable_fused(self):
         """Fused halo push (include/mc_tvd.h): every operator writes its boundary rows straight into the neighbours' halo
-        rows, so nothing is exchanged between the launches.  The neighbours' buffers must be addressable from this
-        process (`LocalComm`: the same GPU, or GPUs of this process with peer access); raises where the library does
+        rows, so nothing is exchanged between the launches.  The neighbours' buffers are addressed directly: slabs of this
+        process (`LocalComm`) or of neighbouring processes through CUDA IPC (`DistComm`); raises where the library does
         not support it (2-D, odd nx, non-uniform z)."""
-        if not isinstance(self.comm, LocalComm):
-            raise NotImplementedError("the fused halo push needs the neighbours' device addresses: all slabs in one process")
-        bufs = [r.slab_buffers() for r in self.ranks]
-        w = len(self.ranks)
-        for i, r in enumerate(self.ranks):
-            r.slab_peers(bufs[(i - 1) % w], bufs[(i + 1) % w], self.halo, self.halo + self.own, self.halo)
+        for r, (lo, hi) in zip(self.ranks, self.comm.neighbour_buffers(self.ranks)):
+            r.slab_peers(lo, hi, self.halo, self.halo + self.own, self.halo)
         self.fused = True
 
     def _fields(self):
@@ -243,9 +277,10 @@ def make_local_driver(binding, grid: dict, params: dict, X0: np.ndarray, n_slabs
     return SlabDriver(ranks, LocalComm(n_slabs), grid, fused=fused)
 
 
-def make_dist_driver(binding, grid: dict, params: dict, X0: np.ndarray, device, group=None):
-    """One slab per process of an initialised torch.distributed group (NCCL: one process per GPU)."""
+def make_dist_driver(binding, grid: dict, params: dict, X0: np.ndarray, device, group=None, fused: bool = False):
+    """One slab per process of an initialised torch.distributed group (NCCL: one process per GPU).  fused: the halo push
+    inside the sweep kernels through CUDA-IPC-mapped neighbour buffers instead of send / recv between the launches."""
     comm = DistComm(group)
     gl, _ = local_grid(grid, comm.world)
     rank = binding.MCTVD(gl, params, scatter_state(X0, grid, comm.rank0, comm.world), device=device)
-    return SlabDriver([rank], comm, grid)
+    return SlabDriver([rank], comm, grid, fused=fused)

@@ -92,6 +92,62 @@ def test_fused_halo_push_is_refused_where_it_is_not_built(gpu):
         assert e.value.code == -5
 
 
+def _ipc_worker(rank: int, world: int, port: int, out_dir: str, fused: bool):
+    """One slab per PROCESS (both on cuda:0; host barriers only, no kernel waits on another process's kernel)."""
+    import os
+    import sys
+    import torch
+    import torch.distributed as dist
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    sys.path.insert(0, root)
+    from paper_2411_10372_b200 import binding
+    dist.init_process_group("gloo", init_method=f"tcp://127.0.0.1:{port}", rank=rank, world_size=world)
+    torch.cuda.set_device(0)
+    grid = inputs.make_grid(3, 64, 33, 48)
+    params = inputs.make_params(Ra=1e5)
+    X0 = inputs.moving_state(grid, params, amplitude=1e-2, u_amp=0.1)
+    drv = slab.make_dist_driver(binding, grid, params, X0, device="cuda:0", fused=fused)
+    dts = []
+    for _ in range(3):
+        dts.append(drv.dt())
+        drv.step(1)
+    d = drv.diagnostics()[0]
+    np.save(os.path.join(out_dir, f"state{rank}.npy"), drv.local_states()[0])
+    np.save(os.path.join(out_dir, f"dts{rank}.npy"), np.array(dts + [d["nu_bar"], d["mass"]]))
+    dist.barrier()
+    for r in drv.ranks:
+        r.close()
+    dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("fused", [False, True])
+def test_one_slab_per_process(gpu, tmp_path, fused):
+    """Two processes, one slab each, a gloo group between them: `DistComm` with send / recv of the halo rows (fused =
+    False) and with the fused halo push into the neighbour PROCESS's buffers opened through CUDA IPC (fused = True).
+    Both must reproduce the undivided box."""
+    import torch.multiprocessing as mp
+    import os
+    port = 26000 + (os.getpid() * 3 + int(fused)) % 3000
+    mp.spawn(_ipc_worker, args=(2, port, str(tmp_path), fused), nprocs=2, join=True)
+    grid = inputs.make_grid(3, 64, 33, 48)
+    params = inputs.make_params(Ra=1e5)
+    X0 = inputs.moving_state(grid, params, amplitude=1e-2, u_amp=0.1)
+    one = gpu.MCTVD(grid, params, X0)
+    dts = []
+    for _ in range(3):
+        dts.append(one.dt())
+        one.step(1)
+    d = one.diagnostics()[0]
+    parts = [np.load(tmp_path / f"state{r}.npy") for r in range(2)]
+    got = slab.gather_state(parts, grid)
+    assert parity_err(grid, params, got, one.state()).max() <= 1e-13
+    for r in range(2):
+        rec = np.load(tmp_path / f"dts{r}.npy")
+        assert np.allclose(rec[:3], dts, rtol=4e-16, atol=0)
+        assert rec[3] == pytest.approx(d["nu_bar"], rel=1e-10) and rec[4] == pytest.approx(d["mass"], rel=1e-12)
+    one.close()
+
+
 def test_bench_slabs_mode_runs_under_a_one_rank_nccl_group():
     """bench.py --slabs through torch.distributed with the NCCL backend and a world of one rank (this box has one GPU):
     the DistComm code path (process group, all_reduce of the CFL maximum, the local wrap of the halos) end to end."""
