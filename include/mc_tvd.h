@@ -237,6 +237,32 @@ int mc_tvd_slab_diag_partial(mc_tvd_state *s, int axis, int lo, int hi);
 int mc_tvd_slab_diag_finish(mc_tvd_state *s, double nplane_global, mc_tvd_diag *out, double *T_prof, double *rho_prof,
                             double *p_prof);
 
+/* The CFL reduction without a handle, a workspace or any allocation (R12; the "local Courant number" of
+ * PAPER.md:304-307): for callers that cannot call cudaMalloc -- code under CUDA graph capture, serving loops,
+ * harnesses that forbid it.  Enqueues on `cuda_stream` the same max-reduction kernel mc_tvd_init and the slab driver
+ * use, over the state `d_fields` (DEVICE, layout as in mc_tvd_init, read only), and writes to `d_out` (DEVICE, 2 doubles,
+ * caller-owned):  d_out[0] = s = max over nodes and directions of (|u_a| + c_s) / dx_a  (NaN if rho or T is not
+ * positive anywhere),  d_out[1] = the dt the next step would use, fixed_dt if > 0 else cfl / s -- bit for bit the dt of a
+ * handle initialised on the same state.  Asynchronous: read d_out after synchronising the stream.
+ *
+ * Scratch: the running maximum and, for a non-uniform z grid, the node heights and the metric tables built from them
+ * on the device live in ONE fixed array inside the library, MC_TVD_NOALLOC_SCRATCH_BYTES (128.25 KiB) of device memory on
+ * every GPU that loads the library, held until the process exits.  Hence the limit: nz <= MC_TVD_NOALLOC_MAX_NZ on any
+ * grid (more levels: MC_TVD_EUNSUPPORTED, nothing is enqueued); nx, ny are limited as in mc_tvd_init only.
+ * The call allocates nothing on the host or the device (no cudaMalloc / cudaFree / allocating library routine); its
+ * first use on a device looks up the array's address (cudaGetSymbolAddress), at most 64 devices per process.
+ * grid->z_nodes (HOST) is uploaded with cudaMemcpyAsync on the stream: keep it valid and unchanged until the stream has
+ * passed the call (pageable memory is already staged when the call returns).  Make the first call on a device outside
+ * stream capture (the address look-up may load the module).
+ * All calls share the array: it is cleared at the start of every call and left cleared, but two calls whose kernels
+ * OVERLAP on the GPU (different streams without ordering, several host threads) race on it and return rubbish -- order
+ * them on one stream or with events.  Calls on different GPUs do not interact.  Handles (mc_tvd_init) never touch it.
+ * Errors: MC_TVD_EINVAL (bad problem, NULL pointer), MC_TVD_EUNSUPPORTED (nz too large), MC_TVD_ECUDA. */
+#define MC_TVD_NOALLOC_MAX_NZ 4096
+#define MC_TVD_NOALLOC_SCRATCH_BYTES (256 + 4 * MC_TVD_NOALLOC_MAX_NZ * 8)
+int mc_tvd_cfl_noalloc(const mc_tvd_grid *grid, const mc_tvd_params *params, const double *d_fields, double *d_out,
+                       void *cuda_stream);
+
 /* Number of kernel launches this handle has enqueued so far (for bench.py's gpu_launches). */
 long long mc_tvd_launch_count(const mc_tvd_state *s);
 

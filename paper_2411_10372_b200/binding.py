@@ -81,6 +81,7 @@ SYMBOLS = {
                                        C.POINTER(C.c_void_p)]),
     "mc_tvd_slab_diag_partial": (C.c_int, [C.c_void_p, C.c_int, C.c_int, C.c_int]),
     "mc_tvd_slab_diag_finish": (C.c_int, [C.c_void_p, C.c_double, C.POINTER(Diag), _DP, _DP, _DP]),
+    "mc_tvd_cfl_noalloc": (C.c_int, [C.POINTER(Grid), C.POINTER(Params), C.c_void_p, C.c_void_p, C.c_void_p]),
     "mc_tvd_launch_count": (C.c_longlong, [C.c_void_p]),
     "mc_tvd_timing_enable": (C.c_int, [C.c_void_p, C.c_int]),
     "mc_tvd_timing_read": (C.c_int, [C.c_void_p, _DP, C.POINTER(C.c_longlong)]),
@@ -146,6 +147,34 @@ def make_params(p: dict) -> Params:
                   p["T_bot"], p["T_top"], p["lambda_coef"], p["g_override"], p["mu_override"],
                   p["K_override"], int(p["bc_z"]), int(p["tvd_form"]), int(p["dir_mode"]),
                   int(p["tvd_off"]))
+
+
+NOALLOC_MAX_NZ = 4096                 # MC_TVD_NOALLOC_MAX_NZ of include/mc_tvd.h
+
+
+def cfl_noalloc(grid: dict, params: dict, fields, out, stream=None) -> None:
+    """mc_tvd_cfl_noalloc: enqueue the CFL reduction of the state in `fields` (CUDA float64 tensor, nf * N values, read only)
+    and write (s, dt) into `out` (CUDA float64 tensor, >= 2 values) -- no handle, no workspace, no allocation: the
+    library's fixed scratch array serves (nz <= NOALLOC_MAX_NZ).  Asynchronous on `stream` (default: torch's current
+    stream of the tensors' device); calls whose kernels overlap on the GPU race on the scratch."""
+    import torch
+
+    if not (fields.is_cuda and out.is_cuda and fields.dtype == torch.float64 and out.dtype == torch.float64):
+        raise TypeError("fields and out must be CUDA float64 tensors")
+    if not (fields.is_contiguous() and out.is_contiguous()) or out.numel() < 2 or out.device != fields.device:
+        raise ValueError("fields and out must be contiguous tensors on one device, out with at least 2 values")
+    nf = 4 if int(grid["ndim"]) == 2 else 5
+    if fields.numel() != nf * int(grid["nx"]) * int(grid.get("ny", 1)) * int(grid["nz"]):
+        raise ValueError("fields does not hold nf * nx * ny * nz values")
+    lib = load_library()
+    g, p = make_grid(grid), make_params(params)
+    with torch.cuda.device(fields.device):
+        st = stream if stream is not None else torch.cuda.current_stream()
+        rc = lib.mc_tvd_cfl_noalloc(C.byref(g), C.byref(p), fields.data_ptr(), out.data_ptr(), st.cuda_stream)
+        if rc == 0 and g.z_nodes:
+            st.synchronize()             # the host node heights (kept alive by g) must outlive the upload
+    if rc != 0:
+        raise MCTVDError(rc, lib.mc_tvd_last_error().decode())
 
 
 class MCTVD:

@@ -8,6 +8,7 @@
 #include <stdio.h>
 #include <stdlib.h>
 #include <string.h>
+#include <atomic>
 #include <new>
 #include <type_traits>
 
@@ -1104,3 +1105,125 @@ int mc_tvd_destroy(mc_tvd_state *s)
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------
+// mc_tvd_cfl_noalloc (include/mc_tvd.h): the CFL reduction with its scratch in a fixed device array instead of a
+// caller's workspace -- no allocation anywhere on the call's path.
+// ---------------------------------------------------------------------------------------------
+// One array per GPU that loads the library, held until the process exits.  Bytes [0, 256): the running maximum (a bit
+// pattern, must be 0 when k_max_speed starts).  Then, in doubles: the caller's node heights [0, MAX_NZ), and from
+// MAX_NZ on the tables k_max_speed reads as PointArgs::zt with stride nz: z, g z, 1 / cell height.
+// In HOST code this name is a host-side stand-in, not a device address: the address comes from cudaGetSymbolAddress.
+static __device__ __align__(256) unsigned char g_noalloc_scratch[MC_TVD_NOALLOC_SCRATCH_BYTES];
+
+namespace {
+
+constexpr int NOALLOC_MAX_DEVICES = 64;
+std::atomic<unsigned char *> g_noalloc_ptr[NOALLOC_MAX_DEVICES];   // device address of the array, per device ordinal
+
+MC_KERNEL void k_noalloc_clear(unsigned long long *bits)
+{
+    if (blockIdx.x == 0 && threadIdx.x == 0) *bits = 0ull;
+}
+
+// The first three tables of SweepArgs::zt, with the arithmetic of mc_tvd_init's host loop (IEEE subtract, multiply,
+// divide: the same bits).
+MC_KERNEL void k_noalloc_metric(const double *z, double *zt, int nz, double g)
+{
+    for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < nz; k += gridDim.x * blockDim.x) {
+        const double dzc = (k == 0) ? 0.5 * (z[1] - z[0]) : (k == nz - 1) ? 0.5 * (z[k] - z[k - 1]) : 0.5 * (z[k + 1] - z[k - 1]);
+        zt[k] = z[k];
+        zt[nz + k] = g * z[k];
+        zt[2 * nz + k] = 1.0 / dzc;
+    }
+}
+
+// out[0] = s, out[1] = the dt of k_dt_update; the array is left cleared for the next call.
+MC_KERNEL void k_noalloc_finish(unsigned long long *bits, double *out, double cfl, double fixed_dt)
+{
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        const double s = __longlong_as_double((long long)*bits);
+        out[0] = s;
+        out[1] = (fixed_dt > 0.0) ? fixed_dt : cfl / s;
+        *bits = 0ull;
+    }
+}
+
+// Device address of g_noalloc_scratch on the current device: looked up once per device, with that device current.
+int noalloc_scratch(unsigned char **ptr)
+{
+    int dev = -1;
+    int rc = cuda_check(cudaGetDevice(&dev), "cudaGetDevice");
+    if (rc != MC_TVD_OK) return rc;
+    if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) return fail(MC_TVD_EUNSUPPORTED, "mc_tvd_cfl_noalloc: device ordinal beyond 63");
+    unsigned char *p = g_noalloc_ptr[dev].load(std::memory_order_acquire);
+    if (!p) {
+        void *q = nullptr;
+        rc = cuda_check(cudaGetSymbolAddress(&q, g_noalloc_scratch), "cudaGetSymbolAddress(g_noalloc_scratch)");
+        if (rc != MC_TVD_OK) return rc;
+        if (!q) return fail(MC_TVD_ECUDA, "cudaGetSymbolAddress returned a null address");
+        p = (unsigned char *)q;
+        g_noalloc_ptr[dev].store(p, std::memory_order_release);   // (two threads racing here store the same address)
+    }
+    *ptr = p;
+    return MC_TVD_OK;
+}
+
+}  // namespace
+
+extern "C" int mc_tvd_cfl_noalloc(const mc_tvd_grid *grid, const mc_tvd_params *params, const double *d_fields,
+                                  double *d_out, void *cuda_stream)
+{
+    int code;
+    if (!valid_problem(grid, params, &code)) return code;
+    if (!d_fields || !d_out) return fail(MC_TVD_EINVAL, "d_fields or d_out is NULL");
+    if (((uintptr_t)d_fields & 15) || ((uintptr_t)d_out & 7))
+        return fail(MC_TVD_EINVAL, "d_fields must be 16-byte and d_out 8-byte aligned");
+    if (grid->nz > MC_TVD_NOALLOC_MAX_NZ) {
+        char msg[160];
+        snprintf(msg, sizeof(msg), "nz = %d exceeds MC_TVD_NOALLOC_MAX_NZ = %d (the fixed scratch array holds no more levels)",
+                 grid->nz, MC_TVD_NOALLOC_MAX_NZ);
+        return fail(MC_TVD_EUNSUPPORTED, "mc_tvd_cfl_noalloc: %s", msg);
+    }
+    unsigned char *scratch = nullptr;
+    int rc = noalloc_scratch(&scratch);
+    if (rc != MC_TVD_OK) return rc;
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    unsigned long long *bits = (unsigned long long *)scratch;
+    double *z_dev = (double *)(scratch + 256);
+    double *zt_dev = z_dev + MC_TVD_NOALLOC_MAX_NZ;
+
+    // the constants of mc_tvd_init, on a stack copy of the handle's fields that point_args reads
+    mc_tvd_state t;
+    memset(&t, 0, sizeof(t));
+    t.grid = *grid; t.par = *params;
+    t.nd = grid->ndim; t.nf = (grid->ndim == 2) ? 4 : 5;
+    t.plane = (long long)grid->nx * grid->ny;
+    t.N = t.plane * grid->nz;
+    t.walls = (params->bc_z == 0);
+    t.d[0] = grid->lx / grid->nx;
+    t.d[1] = (grid->ndim == 3) ? grid->ly / grid->ny : 1.0;
+    t.d[2] = t.walls ? grid->lz / (grid->nz - 1) : grid->lz / grid->nz;
+    t.icv = params->gamma * params->eps * params->D;
+    t.R = (params->gamma - 1.0) / t.icv;
+    t.g = (params->g_override >= 0.0) ? params->g_override : 1.0 / params->eps;
+    t.X = const_cast<double *>(d_fields);                 // read only
+    t.zt = nullptr;
+
+    { auto kfn = k_noalloc_clear; MC_LAUNCH(kfn, 1, 32, 0, stream, bits); }
+    if (grid->z_nodes) {
+        rc = cuda_check(cudaMemcpyAsync(z_dev, grid->z_nodes, (size_t)grid->nz * sizeof(double), cudaMemcpyHostToDevice, stream),
+                        "z node upload");
+        if (rc != MC_TVD_OK) return rc;
+        auto kfn = k_noalloc_metric;
+        MC_LAUNCH(kfn, (grid->nz + 255) / 256, 256, 0, stream, z_dev, zt_dev, grid->nz, t.g);
+        t.zt = zt_dev;
+    }
+    mc::PointArgs P = point_args(&t);
+    int blocks = (int)((t.N + 255) / 256);
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    if (t.nd == 2) { auto kfn = mc::k_max_speed<2>; MC_LAUNCH(kfn, blocks, 256, 0, stream, P, bits); }
+    else { auto kfn = mc::k_max_speed<3>; MC_LAUNCH(kfn, blocks, 256, 0, stream, P, bits); }
+    { auto kfn = k_noalloc_finish; MC_LAUNCH(kfn, 1, 32, 0, stream, bits, d_out, params->cfl, params->fixed_dt); }
+    return cuda_check(cudaGetLastError(), "mc_tvd_cfl_noalloc launch");
+}
