@@ -42,6 +42,13 @@ CASES = {
                      t_spin=150.0, t_avg=50.0, paper=(7.3, 0.2, 330.0, 7.0), ref=(7.1, 322.0), cite="Table 2 case 3"),
     "table1-3": dict(ndim=3, Ra=1e6, D=0.5, Gamma=4.0, gamma=1.4, Pr=0.7, eps=0.1, nx=384, ny=384, nz=129,
                      t_spin=80.0, t_avg=50.0, paper=(6.89, 0.05, 406.0, 3.0), ref=(6.93, 407.0), cite="Table 1 case 3"),
+    # the same on the paper's kind of grid: levels clustered at the plates (3.3 x finer there, 1.7 x coarser mid-layer)
+    "table1-3-tanh": dict(ndim=3, Ra=1e6, D=0.5, Gamma=4.0, gamma=1.4, Pr=0.7, eps=0.1, nx=384, ny=384, nz=129,
+                          z_stretch=1.5, t_spin=80.0, t_avg=50.0, paper=(6.89, 0.05, 406.0, 3.0), ref=(6.93, 407.0),
+                          cite="Table 1 case 3"),
+    # and with every spacing halved (151 M nodes; about an hour on one B200)
+    "table1-3-fine": dict(ndim=3, Ra=1e6, D=0.5, Gamma=4.0, gamma=1.4, Pr=0.7, eps=0.1, nx=768, ny=768, nz=257,
+                          t_spin=70.0, t_avg=40.0, paper=(6.89, 0.05, 406.0, 3.0), ref=(6.93, 407.0), cite="Table 1 case 3"),
 }
 
 
