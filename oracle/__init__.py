@@ -66,7 +66,8 @@ class _Stats(C.Structure):
 
 class _Forces(C.Structure):
     _fields_ = [(n, C.c_double) for n in ("Fn_mean", "Fp_mean", "Fb_mean", "Fv_mean", "Fn_rms", "Fp_rms", "Fb_rms",
-                                          "Fv_rms", "FbFp_mean", "max_mach", "max_r", "volume")]
+                                          "Fv_rms", "FbFp_mean", "max_mach", "max_r", "volume", "corr_C", "flux_mean",
+                                          "rhouz_sq_mean", "Tsa_sq_mean")]
 
 
 HIST_BINS = 128
@@ -214,7 +215,8 @@ def step_stats(prob: Problem, X: np.ndarray, n_steps: int, every: int = 1, dt_in
 
 
 def flow_stats(prob: Problem, X: np.ndarray):
-    """Returns (dict of the force-balance averages of Eqs. 40-43 and the extrema, histogram of r as int64[HIST_BINS])."""
+    """Returns (dict of the force-balance averages of Eqs. 40-43, the extrema and the correlation C of Eq. 49 with its
+    three volume averages, histogram of r as int64[HIST_BINS])."""
     X = _check(prob, X)
     g, p = prob.c_grid(), prob.c_params()
     f = _Forces()

@@ -611,10 +611,12 @@ int orc_flow_stats(const orc_grid *g, const orc_params *p, const double *X, orc_
     memset(out, 0, sizeof(*out));
     if (hist_r) memset(hist_r, 0, ORC_HIST_BINS * sizeof(long long));
     double sum[4] = { 0, 0, 0, 0 }, sq[4] = { 0, 0, 0, 0 }, vol = 0.0, max_r = 0.0;
+    double cor[3] = { 0, 0, 0 }, vol_all = 0.0;      /* Eq. 49: <rho u_z T_sa>_V, <(rho u_z)^2>_V, <T_sa^2>_V */
     double dx2 = c.d[0] * c.d[0], dy2 = c.d[1] * c.d[1];
     int k0 = c.walls ? 1 : 0, k1 = c.walls ? c.nz - 1 : c.nz;
     for (int k = 0; k < c.nz; ++k) {
-        double ps[4] = { 0, 0, 0, 0 }, pq[4] = { 0, 0, 0, 0 };
+        double ps[4] = { 0, 0, 0, 0 }, pq[4] = { 0, 0, 0, 0 }, pc[3] = { 0, 0, 0 };
+        double TA = 1.0 - p->D * z_of(&c, k);        /* Eq. 19 */
         for (int j = 0; j < c.ny; ++j)
             for (int i = 0; i < c.nx; ++i) {
                 size_t n = at(&c, i, j, k);
@@ -622,6 +624,9 @@ int orc_flow_stats(const orc_grid *g, const orc_params *p, const double *X, orc_
                 double r = (0.5 * u2) / (c.cv * w[W_T][n]);
                 if (r > max_r) max_r = r;
                 if (hist_r) hist_r[hist_bin(r)] += 1;
+                /* the two factors of the correlation C of Eq. 49, at every node: <.>_V of Eq. 22 */
+                double mz = q[Q_RHO][n] * w[W_UZ][n], Tsa = w[W_T][n] - TA;
+                pc[0] += mz * Tsa; pc[1] += mz * mz; pc[2] += Tsa * Tsa;
                 if (k < k0 || k >= k1) continue;
                 /* spacings along z around level k (face spacings below and above) */
                 double hm = c.z ? hface(&c, k - 1) : c.d[2], hp = c.z ? hface(&c, k) : c.d[2];
@@ -646,6 +651,11 @@ int orc_flow_stats(const orc_grid *g, const orc_params *p, const double *X, orc_
                 double F[4] = { Fn, Fp, Fb, Fv };
                 for (int t = 0; t < 4; ++t) { ps[t] += F[t]; pq[t] += F[t] * F[t]; }
             }
+        {   /* <.>_V as in orc_diagnostics: cell heights, half cells at the plates (R16 / R19) */
+            double wa = c.z ? dzc(&c, k) : c.d[2] * ((c.walls && (k == 0 || k == c.nz - 1)) ? 0.5 : 1.0);
+            vol_all += wa;
+            for (int t = 0; t < 3; ++t) cor[t] += wa * (pc[t] / ((double)c.nx * (double)c.ny));
+        }
         if (k < k0 || k >= k1) continue;
         double wk = dzc(&c, k) / ((double)c.nx * (double)c.ny);
         vol += dzc(&c, k);
@@ -657,6 +667,10 @@ int orc_flow_stats(const orc_grid *g, const orc_params *p, const double *X, orc_
     out->max_r = max_r;
     out->max_mach = sqrt(2.0 * max_r / (c.gamma * (c.gamma - 1.0)));
     out->volume = vol;
+    out->flux_mean = cor[0] / vol_all;
+    out->rhouz_sq_mean = cor[1] / vol_all;
+    out->Tsa_sq_mean = cor[2] / vol_all;
+    out->corr_C = out->flux_mean / sqrt(out->rhouz_sq_mean * out->Tsa_sq_mean);     /* Eq. 49; 0/0 = NaN for a fluid at rest */
     for (int f = 0; f < 5; ++f) free(w[f]);
     free(zeros);
     return 0;

@@ -116,6 +116,11 @@ typedef struct {
     double FbFp_mean;                        /* <F_b> - <F_p> */
     double max_mach, max_r;
     double volume;                           /* the volume the averages run over (interior cells) */
+    /* Eq. 49: C = <rho u_z T_sa> / sqrt(<(rho u_z)^2> <T_sa^2>), the normalised correlation of the
+     * vertical mass flux and the superadiabatic temperature T_sa = T - T_A(z) (Eq. 19), and its three volume averages --
+     * <.>_V over the whole layer with the weights of Eq. 22's Nu_conv (orc_diagnostics), so that
+     * nu_conv = sqrt(Ra Pr) / eps * flux_mean. */
+    double corr_C, flux_mean, rhouz_sq_mean, Tsa_sq_mean;
 } orc_forces;
 int orc_flow_stats(const orc_grid *g, const orc_params *p, const double *X, orc_forces *out, long long *hist_r);
 

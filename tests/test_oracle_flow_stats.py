@@ -114,3 +114,74 @@ def test_histogram_of_r_and_the_largest_mach_number(orc):
     assert h.sum() == 144 and np.array_equal(h, want)
     assert f["max_r"] == pytest.approx(0.5 * ux.max() ** 2, rel=1e-13)
     assert f["max_mach"] == pytest.approx(ux.max() / np.sqrt(1.4 * 0.4), rel=1e-13)
+
+
+@pytest.mark.parametrize("ndim", [2, 3])
+@pytest.mark.parametrize("phase,want", [(0.0, 1.0), (np.pi / 3, 0.5), (np.pi / 2, 0.0), (np.pi, -1.0), (2.0, np.cos(2.0))])
+def test_correlation_of_mass_flux_and_superadiabatic_temperature(orc, ndim, phase, want):
+    """Eq. 49.  rho u_z = A sin(pi z) cos(2 pi x) and T_sa = T - (1 - D z) = B sin(pi z) cos(2 pi x +
+    phase): on a uniform grid the trapezoid rule integrates these trigonometric products exactly, so
+    <rho u_z T_sa> = A B cos(phase) / 4, <(rho u_z)^2> = A^2 / 4, <T_sa^2> = B^2 / 4 and C = cos(phase) to round-off --
+    the sign, the T_A(z) that is subtracted, the half cells at the plates and the normalisation all enter."""
+    A, B = 0.03, 0.02
+    g = inputs.make_grid(ndim, 16, 13, 8 if ndim == 3 else 1, lx=1.0, ly=1.0)
+    p = inputs.make_params(Ra=1e5, D=0.4)
+    R = inputs.closure_constants(p)["R"]
+    zz = inputs.z_nodes(g, p)
+    Z, Y, Xc = np.meshgrid(zz, np.arange(g["ny"]) / g["ny"], np.arange(16) / 16, indexing="ij")
+    rho = 1.0 + 0.3 * np.cos(2 * np.pi * Xc) * Z + 0.1 * np.sin(2 * np.pi * Y)
+    mz = A * np.sin(np.pi * Z) * np.cos(2 * np.pi * Xc)
+    T = (1.0 - p["D"] * Z) + B * np.sin(np.pi * Z) * np.cos(2 * np.pi * Xc + phase)
+    X = state_from_primitives(g, p, rho, 0.05 * np.sin(2 * np.pi * Xc), 0.0, mz / rho, R * rho * T)
+    f, _ = orc.flow_stats(orc.Problem(g, p), X)
+    assert f["flux_mean"] == pytest.approx(A * B * np.cos(phase) / 4, abs=1e-17)
+    assert f["rhouz_sq_mean"] == pytest.approx(A * A / 4, rel=1e-13)
+    assert f["Tsa_sq_mean"] == pytest.approx(B * B / 4, rel=1e-11)          # (T_sa is a difference of O(1) numbers)
+    assert f["corr_C"] == pytest.approx(want, abs=1e-11)
+
+
+@pytest.mark.parametrize("ndim,stretch", [(2, None), (3, None), (2, 1.5), (3, 2.0)])
+def test_correlation_agrees_with_nu_conv_and_is_bounded(orc, ndim, stretch):
+    """<rho u_z T_sa>_V of Eq. 49 is the average inside Nu_conv of Eq. 22: the two routines must agree,
+    on uniform and stretched grids; |C| <= 1 (Cauchy-Schwarz with non-negative weights), and C is unchanged when u_z is
+    scaled (it is a normalised correlation) and changes sign with u_z."""
+    g = inputs.make_grid(ndim, 12, 11, 10 if ndim == 3 else 1, z_stretch=stretch)
+    p = inputs.make_params(Ra=1e5)
+    X = inputs.rough_random_state(g, p, seed=17)
+    prob = orc.Problem(g, p)
+    f, _ = orc.flow_stats(prob, X)
+    d = orc.diagnostics(prob, X)[0]
+    assert np.sqrt(p["Ra"] * p["Pr"]) / p["eps"] * f["flux_mean"] == pytest.approx(d["nu_conv"], rel=1e-12)
+    assert abs(f["corr_C"]) <= 1.0 and f["rhouz_sq_mean"] > 0 and f["Tsa_sq_mean"] > 0
+    assert f["corr_C"] == pytest.approx(f["flux_mean"] / np.sqrt(f["rhouz_sq_mean"] * f["Tsa_sq_mean"]), rel=1e-15)
+    # scale u_z by -2 at fixed rho, u_x, u_y, T
+    nf = X.shape[0]
+    rho, mz = X[0], X[nf - 2]
+    Y = X.copy()
+    Y[nf - 2] = -2.0 * mz
+    Y[nf - 1] = X[nf - 1] + 0.5 * (4.0 - 1.0) * mz * mz / rho          # E keeps T: the kinetic energy of u_z grows 4-fold
+    f2, _ = orc.flow_stats(prob, Y)
+    assert f2["Tsa_sq_mean"] == pytest.approx(f["Tsa_sq_mean"], rel=1e-10)
+    assert f2["corr_C"] == pytest.approx(-f["corr_C"], rel=1e-9)
+    assert f2["rhouz_sq_mean"] == pytest.approx(4.0 * f["rhouz_sq_mean"], rel=1e-13)
+
+
+def test_correlation_on_the_stretched_grid_converges(orc):
+    """The same closed form (C = cos(phase), <rho u_z T_sa> = A B cos(phase) / 4) on the tanh grid, where the
+    cell-height weights (R19) integrate sin^2(pi z) only to second order."""
+    A, B, phase = 0.03, 0.02, 0.7
+    errs = []
+    for n in (16, 32, 64):
+        g = inputs.make_grid(2, 16, n + 1, lx=1.0, z_stretch=1.5)
+        p = inputs.make_params(Ra=1e5, D=0.4)
+        R = inputs.closure_constants(p)["R"]
+        zz = inputs.z_nodes(g, p)
+        Z, _, Xc = np.meshgrid(zz, np.zeros(1), np.arange(16) / 16, indexing="ij")
+        rho = 1.0 + 0.2 * Z
+        mz = A * np.sin(np.pi * Z) * np.cos(2 * np.pi * Xc)
+        T = (1.0 - p["D"] * Z) + B * np.sin(np.pi * Z) * np.cos(2 * np.pi * Xc + phase)
+        X = state_from_primitives(g, p, rho, 0.0, 0.0, mz / rho, R * rho * T)
+        f, _ = orc.flow_stats(orc.Problem(g, p), X)
+        assert f["corr_C"] == pytest.approx(np.cos(phase), abs=1e-10)       # the weights cancel in the ratio
+        errs.append(abs(f["flux_mean"] / (A * B * np.cos(phase) / 4) - 1.0))
+    assert errs[0] < 2e-2 and errs[0] / errs[1] > 3.5 and errs[1] / errs[2] > 3.5, errs
