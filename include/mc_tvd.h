@@ -171,6 +171,10 @@ int mc_tvd_stats_read(mc_tvd_state *s, mc_tvd_stats *out, double *T_prof, double
  *   - r = K_e / I_e = (rho u^2 / 2) / (rho C_v T) "at every grid point": its largest value, the largest
  *     local Mach number, and its histogram over all nodes (Fig. 5) in MC_TVD_HIST_BINS quarter-octave bins from 2^-32
  *     to 1: bin = 4 (floor(log2 r) + 32) + (top two mantissa bits), clamped to [0, 127]; r = 0 in bin 0.
+ *   - the normalised correlation C(Ra) of Eq. 49 between the vertical mass flux rho u_z and the
+ *     superadiabatic temperature T_sa = T - (1 - D z) (Eq. 19), with its three averages; these are <.>_V over the WHOLE
+ *     layer with the weights of Eq. 22 (half cells at the plates), so Nu_conv = sqrt(Ra Pr) / eps * flux_mean; the time
+ *     average forms C from the time-averaged three (the paper's <.> is <.>_{V,t}).
  * The paper does not say how it differences these quantities; R21: second-order central differences on the
  * 3 x 3 x 3 neighbourhood, cell-height weights.
  * mc_tvd_flow_stats: instantaneous values of the current state into HOST memory (hist_r: MC_TVD_HIST_BINS counts, may
@@ -187,6 +191,8 @@ typedef struct {
     double FbFp_mean;                            /* <F_b> - <F_p> */
     double max_mach, max_r;                      /* largest local Mach number and ratio r = K_e / I_e */
     double volume;                               /* the volume averaged over (interior cells) */
+    double corr_C;                               /* Eq. 49: <rho u_z T_sa> / sqrt(<(rho u_z)^2> <T_sa^2>); NaN at rest */
+    double flux_mean, rhouz_sq_mean, Tsa_sq_mean; /* its three averages <.>_V over the whole layer (weights of Eq. 22) */
 } mc_tvd_forces;
 int mc_tvd_flow_stats(mc_tvd_state *s, mc_tvd_forces *out, long long *hist_r);
 int mc_tvd_stats_flow(mc_tvd_state *s, int enable);

@@ -49,7 +49,8 @@ class Stats(C.Structure):           # mc_tvd_stats
 
 class Forces(C.Structure):          # mc_tvd_forces
     _fields_ = [(n, C.c_double) for n in ("Fn_mean", "Fp_mean", "Fb_mean", "Fv_mean", "Fn_rms", "Fp_rms", "Fb_rms",
-                                          "Fv_rms", "FbFp_mean", "max_mach", "max_r", "volume")]
+                                          "Fv_rms", "FbFp_mean", "max_mach", "max_r", "volume", "corr_C", "flux_mean",
+                                          "rhouz_sq_mean", "Tsa_sq_mean")]
 
 
 HIST_BINS = 128                     # MC_TVD_HIST_BINS

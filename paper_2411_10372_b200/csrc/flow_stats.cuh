@@ -3,7 +3,10 @@
 //         F_n = rho (u . grad) u_z,   F_p = -d_z p,   F_b = rho g,   F_v = d_i tau_iz = mu [lap u_z + (1 + lambda) d_z div u]
 //     (tau_ij of Eq. 18) as volume means and root-mean-squares, and <F_b> - <F_p>;
 //   * r = K_e / I_e = (rho u^2 / 2) / (rho C_v T) at every node: its largest value, the largest local
-//     Mach number (Mach^2 = 2 r / (gamma (gamma - 1))) and its histogram (Fig. 5).
+//     Mach number (Mach^2 = 2 r / (gamma (gamma - 1))) and its histogram (Fig. 5);
+//   * the normalised correlation C = <rho u_z T_sa> / sqrt(<(rho u_z)^2> <T_sa^2>) of Eq. 49 with
+//     T_sa = T - (1 - D z) (Eq. 19): three more sums over EVERY node, weighted as the <.>_V of Eq. 22 (cell heights,
+//     half cells at the plates: R16 / R19), so that Nu_conv = sqrt(Ra Pr) / eps <rho u_z T_sa>.
 // Reading R21 (the paper does not say how it differences its post-processing quantities): second-order
 // central differences on the node's 3 x 3 x 3 neighbourhood -- first derivatives over the distance between the two
 // neighbours, second and mixed derivatives compact -- at the interior nodes k = 1 .. nz-2 (every node when z is
@@ -17,8 +20,9 @@
 namespace mc {
 
 constexpr int FLOW_BINS = 128;
-constexpr int FLOW_NQ = 8;             // sums of F_n, F_p, F_b, F_v and of their squares
-constexpr int FLOW_NOUT = 12;          // layout of mc_tvd_forces
+constexpr int FLOW_NQ = 11;            // sums of F_n, F_p, F_b, F_v and of their squares; of m_z T_sa, m_z^2, T_sa^2 (Eq. 49)
+constexpr int FLOW_NF = 8;             // the first FLOW_NF run over the interior cells, the rest over every node
+constexpr int FLOW_NOUT = 16;          // layout of mc_tvd_forces
 
 struct FlowArgs {
     PointArgs P;
@@ -52,6 +56,7 @@ MC_KERNEL void k_flow_partials(FlowArgs G, double *partial, double *ext, unsigne
     const double hm = P.zt ? P.zt[4 * nz + (k >= 1 ? k - 1 : 0)] : P.dz, hp = P.zt ? P.zt[4 * nz + (k + 1 < nz ? k : nz - 2)] : P.dz;
     const double inv_2h = 1.0 / (hp + hm);
     const double gz = point_gz(P, k), gzp = point_gz(P, kp), gzm = point_gz(P, km);
+    const double TA = 1.0 - P.D * point_z(P, k);                               // Eq. 19
     auto fld = [&](int f, long long n) MC_INL { return P.X[(long long)f * P.N + n]; };
     auto vel = [&](int c, long long n) MC_INL { return fld(1 + c, n) / fld(0, n); };
     auto pres = [&](long long n, double gzn) MC_INL {
@@ -77,6 +82,10 @@ MC_KERNEL void k_flow_partials(FlowArgs G, double *partial, double *ext, unsigne
         const double r = (0.5 * u2) / (G.cv * T);
         rmax = fmax(rmax, r);
         atomicAdd(&sh_hist[flow_hist_bin(r)], 1u);
+        {
+            const double mz = fld(1 + CZ, n), Tsa = T - TA;                    // Eq. 49: rho u_z is the conserved momentum
+            acc[8] += mz * Tsa; acc[9] += mz * mz; acc[10] += Tsa * Tsa;
+        }
         if (!interior) continue;
         const long long row = (long long)k * P.plane + (long long)iy * G.nx;
         const int ixp = (ix + 1 < G.nx) ? ix + 1 : 0, ixm = (ix >= 1) ? ix - 1 : G.nx - 1;
@@ -131,37 +140,41 @@ MC_KERNEL void k_flow_partials(FlowArgs G, double *partial, double *ext, unsigne
         if (sh_hist[i]) atomicAdd(&hist[i], (unsigned long long)sh_hist[i]);
 }
 
-// plane partials -> the 12 numbers of mc_tvd_forces in out[0..12) (one block)
+// plane partials -> the 16 numbers of mc_tvd_forces in out[0..16) (one block)
 MC_KERNEL void k_flow_finish(FlowArgs G, const double *partial, const double *ext, int nblk, double gamma, double *out)
 {
-    __shared__ double sh[FLOW_NQ + 2][DIAG_THREADS];
+    __shared__ double sh[FLOW_NQ + 3][DIAG_THREADS];
     const PointArgs &P = G.P;
     const int nz = P.nz;
-    double v[FLOW_NQ + 1], rmax = 0.0;
+    double v[FLOW_NQ + 2], rmax = 0.0;            // [FLOW_NQ]: interior volume, [FLOW_NQ + 1]: whole volume
 #pragma unroll
-    for (int q = 0; q <= FLOW_NQ; ++q) v[q] = 0.0;
+    for (int q = 0; q <= FLOW_NQ + 1; ++q) v[q] = 0.0;
     const double nplane = (double)G.nx * (double)G.ny;
     for (int k = threadIdx.x; k < nz; k += blockDim.x) {
         for (int b = 0; b < nblk; ++b) rmax = fmax(rmax, ext[(long long)k * nblk + b]);
-        if (G.walls && (k == 0 || k == nz - 1)) continue;
-        const double dzc = P.zt ? 1.0 / P.zt[2 * nz + k] : P.dz;
+        const bool plate = G.walls && (k == 0 || k == nz - 1);
+        // cell height; a plate node owns half the adjacent spacing (the table holds that already)
+        const double dzc = P.zt ? 1.0 / P.zt[2 * nz + k] : (plate ? 0.5 * P.dz : P.dz);
         const double wk = dzc / nplane;
+#pragma unroll
         for (int q = 0; q < FLOW_NQ; ++q) {
+            if (plate && q < FLOW_NF) continue;                     // the force balance runs over the interior cells
             double t = 0.0;
             for (int b = 0; b < nblk; ++b) t += partial[((long long)k * nblk + b) * FLOW_NQ + q];
             v[q] += wk * t;
         }
-        v[FLOW_NQ] += dzc;
+        if (!plate) v[FLOW_NQ] += dzc;
+        v[FLOW_NQ + 1] += dzc;
     }
 #pragma unroll
-    for (int q = 0; q <= FLOW_NQ; ++q) sh[q][threadIdx.x] = v[q];
-    sh[FLOW_NQ + 1][threadIdx.x] = rmax;
+    for (int q = 0; q <= FLOW_NQ + 1; ++q) sh[q][threadIdx.x] = v[q];
+    sh[FLOW_NQ + 2][threadIdx.x] = rmax;
     __syncthreads();
     for (int o = blockDim.x >> 1; o > 0; o >>= 1) {
         if ((int)threadIdx.x < o) {
 #pragma unroll
-            for (int q = 0; q <= FLOW_NQ; ++q) sh[q][threadIdx.x] += sh[q][threadIdx.x + o];
-            sh[FLOW_NQ + 1][threadIdx.x] = fmax(sh[FLOW_NQ + 1][threadIdx.x], sh[FLOW_NQ + 1][threadIdx.x + o]);
+            for (int q = 0; q <= FLOW_NQ + 1; ++q) sh[q][threadIdx.x] += sh[q][threadIdx.x + o];
+            sh[FLOW_NQ + 2][threadIdx.x] = fmax(sh[FLOW_NQ + 2][threadIdx.x], sh[FLOW_NQ + 2][threadIdx.x + o]);
         }
         __syncthreads();
     }
@@ -169,14 +182,18 @@ MC_KERNEL void k_flow_finish(FlowArgs G, const double *partial, const double *ex
     const double vol = sh[FLOW_NQ][0];
     for (int t = 0; t < 4; ++t) { out[t] = sh[t][0] / vol; out[4 + t] = sqrt(sh[4 + t][0] / vol); }
     out[8] = out[2] - out[1];                                       // <F_b> - <F_p>
-    out[10] = sh[FLOW_NQ + 1][0];
+    out[10] = sh[FLOW_NQ + 2][0];
     out[9] = sqrt(2.0 * out[10] / (gamma * (gamma - 1.0)));
     out[11] = vol;
+    const double vol_all = sh[FLOW_NQ + 1][0];
+    for (int t = 0; t < 3; ++t) out[13 + t] = sh[FLOW_NF + t][0] / vol_all;
+    out[12] = out[13] / sqrt(out[14] * out[15]);                    // Eq. 49 (NaN for a fluid at rest: 0 / 0)
 }
 
 // Running time averages of the flow statistics (weights as in k_stats_accumulate: time since the previous sample).
 // acc: [0..4) weighted means, [4..8) weighted mean SQUARES (of the rms values), [8] <F_b - F_p>, [9] max Mach, [10] max r,
-// [11] weight.  hist_acc += hist (counts of every sample), then hist is cleared for the next sample.
+// [11] weight, [13..16) the three averages of Eq. 49 (C itself is formed from their time averages when they are read:
+// the paper's <.> there is <.>_{V,t}).  hist_acc += hist (counts of every sample), then hist is cleared for the next sample.
 MC_KERNEL void k_flow_accumulate(double *acc, const double *cur, const double *st, const Scalars *S,
                                  unsigned long long *hist_acc, unsigned long long *hist)
 {
@@ -186,6 +203,7 @@ MC_KERNEL void k_flow_accumulate(double *acc, const double *cur, const double *s
     else if (t < 8) acc[t] += w * (cur[t] * cur[t]);
     else if (t < 11) acc[t] += w * cur[t];
     else if (t == 11) acc[11] += w;
+    else if (t >= 13 && t < 16) acc[t] += w * cur[t];
     for (int i = t; i < FLOW_BINS; i += blockDim.x) { hist_acc[i] += hist[i]; hist[i] = 0ull; }
 }
 

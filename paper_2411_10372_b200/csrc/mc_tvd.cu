@@ -827,7 +827,7 @@ int read_diag_block(mc_tvd_state *s, mc_tvd_diag *out, double *T_prof, double *r
     return rc;
 }
 
-// Enqueue the flow statistics of Sec. 5-6 (flow_stats.cuh): the 12 numbers land in s->flow_out, the histogram of this
+// Enqueue the flow statistics of Sec. 5-6 (flow_stats.cuh): the 16 numbers land in s->flow_out, the histogram of this
 // sample is ADDED to s->flow_hist (the caller clears or consumes it).
 int enqueue_flow_stats(mc_tvd_state *s)
 {
@@ -1051,6 +1051,8 @@ int mc_tvd_stats_read_flow(mc_tvd_state *s, mc_tvd_forces *avg, long long *hist_
     for (int t = 0; t < 4; ++t) { o[t] = a[t] / a[11]; o[4 + t] = sqrt(a[4 + t] / a[11]); }
     for (int t = 8; t < 11; ++t) o[t] = a[t] / a[11];
     o[11] = a[11];                     // `volume` carries the total weight (simulated time averaged over)
+    for (int t = 13; t < 16; ++t) o[t] = a[t] / a[11];
+    o[12] = o[13] / sqrt(o[14] * o[15]);               // Eq. 49 with <.>_{V,t}
     if (hist_r) for (int i = 0; i < mc::FLOW_BINS; ++i) hist_r[i] = (long long)h[i];
     return MC_TVD_OK;
 }

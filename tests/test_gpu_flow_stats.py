@@ -1,5 +1,6 @@
 """GPU parity of the flow statistics (mc_tvd_flow_stats / mc_tvd_stats_flow / mc_tvd_stats_read_flow; Eqs. 40-43,
-PAPER.md:457-467, and the distribution of r = K_e / I_e) against the oracle on the same states."""
+PAPER.md:457-467, the distribution of r = K_e / I_e, and the correlation C of Eq. 49)
+against the oracle on the same states."""
 from __future__ import annotations
 
 import numpy as np
@@ -31,6 +32,12 @@ def _compare(d, do, h, ho, rms_tol=1e-10):
     assert d["max_r"] == pytest.approx(do["max_r"], rel=1e-12)
     assert d["max_mach"] == pytest.approx(do["max_mach"], rel=1e-12)
     assert d["volume"] == pytest.approx(do["volume"], rel=1e-13)
+    # Eq. 49: two sums of squares and one of signed products, measured against their Cauchy-Schwarz bound
+    bound = np.sqrt(do["rhouz_sq_mean"] * do["Tsa_sq_mean"])
+    assert d["rhouz_sq_mean"] == pytest.approx(do["rhouz_sq_mean"], rel=1e-12)
+    assert d["Tsa_sq_mean"] == pytest.approx(do["Tsa_sq_mean"], rel=1e-12)
+    assert abs(d["flux_mean"] - do["flux_mean"]) <= 1e-12 * bound
+    assert abs(d["corr_C"] - do["corr_C"]) <= 1e-11 and abs(d["corr_C"]) <= 1.0
     # the bin is read off the bit pattern of r; the two sides may round r differently in the last place, which moves
     # a node across a bin edge only if r sits within an ulp of it
     assert h.sum() == ho.sum()
@@ -48,7 +55,10 @@ def test_flow_stats_parity(gpu, orc, ndim, nx, ny, nz, stretch, bc_z):
     s = gpu.MCTVD(grid, params, X0)
     d, h = s.flow_stats()
     d2, h2 = s.flow_stats()                                   # a second call starts from a cleared histogram
+    nu_conv = s.diagnostics()[0]["nu_conv"]
     s.close()
+    if bc_z == 0:     # the average inside Nu_conv of Eq. 22 (another kernel) is the numerator of Eq. 49
+        assert np.sqrt(params["Ra"] * params["Pr"]) / params["eps"] * d["flux_mean"] == pytest.approx(nu_conv, rel=1e-10)
     assert do["Fn_rms"] > 0 and do["Fv_rms"] > 0 and (ho[1:] > 0).sum() >= 5
     _compare(d, do, h, ho)
     assert d2 == d and np.array_equal(h2, h)
@@ -70,7 +80,7 @@ def test_flow_stats_time_averages(gpu, orc):
     st = s.stats_read()[0]
     s.close()
     X, t, t_last, wsum = X0, 0.0, 0.0, 0.0
-    acc = {k: 0.0 for k in FORCE_KEYS + ("max_mach", "max_r")}
+    acc = {k: 0.0 for k in FORCE_KEYS + ("max_mach", "max_r", "flux_mean", "rhouz_sq_mean", "Tsa_sq_mean")}
     hsum = np.zeros(orc.HIST_BINS, dtype=np.int64)
     for n in range(n_steps):
         X, dts, _ = orc.step(prob, X, 1)
@@ -90,6 +100,12 @@ def test_flow_stats_time_averages(gpu, orc):
         scale = want[k[:2] + "_rms"] if k != "FbFp_mean" else want["Fb_rms"]
         assert abs(avg[k] - want[k]) <= 1e-9 * scale, k
     assert avg["max_mach"] == pytest.approx(want["max_mach"], rel=1e-9)
+    # Eq. 49 over volume AND time: C from the time-averaged three
+    bound = np.sqrt(want["rhouz_sq_mean"] * want["Tsa_sq_mean"])
+    assert avg["rhouz_sq_mean"] == pytest.approx(want["rhouz_sq_mean"], rel=1e-9)
+    assert avg["Tsa_sq_mean"] == pytest.approx(want["Tsa_sq_mean"], rel=1e-9)
+    assert abs(avg["flux_mean"] - want["flux_mean"]) <= 1e-9 * bound
+    assert abs(avg["corr_C"] - want["flux_mean"] / bound) <= 1e-9 and avg["corr_C"] != 0.0
     assert hist.sum() == hsum.sum() and np.abs(hist - hsum).sum() <= 4
 
 
