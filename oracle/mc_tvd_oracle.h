@@ -7,7 +7,7 @@
  * (Eqs. 22-26).  It follows the paper's algorithm step by
  * step, in the paper's order and notation: whole-array passes, no blocking,
  * no fusion, no reordering.  Where the paper is silent or garbled it takes
- * the readings listed in DESIGN.md ("Readings of the paper", R1..R21).
+ * the readings listed in DESIGN.md ("Readings of the paper", R1..R22).
  *
  * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
  * --impl reference legs may call this.  It shares no code, header, table or
@@ -23,7 +23,9 @@
  * uniform heights give the uniform scheme, mass to round-off, second-order
  * hydrostatic drift / viscous decay / mixed stress derivative, exact plate
  * gradients for a quadratic, dt rule); the flow statistics (R21: second-order
- * convergence to the symbolically differentiated Eqs. 40-43, histogram bins).
+ * convergence to the symbolically differentiated Eqs. 40-43, histogram bins;
+ * R22: the correlation of Eq. 49 in closed form, C = cos(phase), its numerator
+ * against Nu_conv of Eq. 22, bound, scale invariance, sign).
  * Parity unpinned: R11 (TVD flux dropped on plate-adjacent interfaces) and the
  * interface weight of R20 (TVD term on the non-uniform grid): the paper is
  * silent on both and no mathematical criterion decides; each has a test that
