@@ -44,7 +44,8 @@ class _Params(C.Structure):
                 ("D", C.c_double), ("cfl", C.c_double), ("fixed_dt", C.c_double),
                 ("T_bot", C.c_double), ("T_top", C.c_double), ("lambda_coef", C.c_double),
                 ("g_override", C.c_double), ("mu_override", C.c_double), ("K_override", C.c_double),
-                ("bc_z", C.c_int), ("tvd_form", C.c_int), ("dir_mode", C.c_int), ("tvd_off", C.c_int)]
+                ("bc_z", C.c_int), ("tvd_form", C.c_int), ("dir_mode", C.c_int), ("tvd_off", C.c_int),
+                ("co_mode", C.c_int)]
 
 
 class _Diag(C.Structure):
@@ -122,7 +123,7 @@ class Problem:
         return _Params(p["gamma"], p["Pr"], p["Ra"], p["eps"], p["D"], p["cfl"], p["fixed_dt"],
                        p["T_bot"], p["T_top"], p["lambda_coef"], p["g_override"], p["mu_override"],
                        p["K_override"], int(p["bc_z"]), int(p["tvd_form"]), int(p["dir_mode"]),
-                       int(p["tvd_off"]))
+                       int(p["tvd_off"]), int(p.get("co_mode", 0)))
 
     @property
     def nf(self) -> int:

@@ -28,7 +28,7 @@ typedef struct {
     double gamma, R, cv, icv, g, mu, K, lam;
     double Tw[2];                /* T at the bottom (k = 0) and top (k = nz-1) plates */
     int walls;                   /* 1: no-slip isothermal plates at k = 0, nz-1; 0: periodic in z */
-    int tvd_form, tvd_off, dir_mode;
+    int tvd_form, tvd_off, dir_mode, co_mode;
     double cfl, fixed_dt;
 } ctx;
 
@@ -67,7 +67,7 @@ static int ctx_init(ctx *c, const orc_grid *g, const orc_params *p)
     c->K = (p->K_override >= 0.0) ? p->K_override : 1.0 / (p->eps * p->D * sqrt(p->Ra * p->Pr));
     c->lam = p->lambda_coef;
     c->Tw[0] = p->T_bot; c->Tw[1] = p->T_top;
-    c->tvd_form = p->tvd_form; c->tvd_off = p->tvd_off; c->dir_mode = p->dir_mode;
+    c->tvd_form = p->tvd_form; c->tvd_off = p->tvd_off; c->dir_mode = p->dir_mode; c->co_mode = p->co_mode;
     c->cfl = p->cfl; c->fixed_dt = p->fixed_dt;
     return 0;
 }
@@ -269,7 +269,8 @@ static void tvd_interface_flux(const ctx *c, int a, double tau, double *const X[
             for (int i = 0; i < c->nx; ++i) {
                 size_t n = at(c, i, j, k);
                 double cs = sqrt(c->gamma * c->R * w[W_T][n]);
-                double Co = (fabs(w[a][n]) + cs) * tau / ((a == 2) ? dzc(c, k) : c->d[a]);
+                double speed = c->co_mode ? fabs(w[a][n]) : fabs(w[a][n]) + cs;      /* R5: the two readings of "local Courant number" */
+                double Co = speed * tau / ((a == 2) ? dzc(c, k) : c->d[a]);
                 Cn[n] = (Co <= 0.5) ? Co * (1.0 - Co) : 0.25;
             }
     for (int k = 0; k < c->nz; ++k)

@@ -60,6 +60,8 @@ typedef struct {
     int tvd_form;                  /* 0 = Eq. 34 as printed, 1 = Davis/Yee sum of two G's */
     int dir_mode;                  /* 0 = backward predictor always (paper), 1 = alternate per half step */
     int tvd_off;                   /* 1 = drop the TVD term T (tests only) */
+    int co_mode;                   /* local Courant number of Eq. 39 (PAPER.md:307 does not define it; R5):
+                                      0 = (|u_alpha| + c_s) tau / dx_alpha, 1 = |u_alpha| tau / dx_alpha */
 } orc_params;
 
 typedef struct {

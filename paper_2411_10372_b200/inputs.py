@@ -60,7 +60,7 @@ def make_params(**over) -> dict:
     p = dict(gamma=5.0 / 3.0, Pr=1.0, Ra=1e6, eps=0.1, D=0.4, cfl=0.5, fixed_dt=0.0,
              T_bot=1.0, T_top=None, lambda_coef=-2.0 / 3.0,
              g_override=-1.0, mu_override=-1.0, K_override=-1.0,
-             bc_z=0, tvd_form=1, dir_mode=1, tvd_off=0)
+             bc_z=0, tvd_form=1, dir_mode=1, tvd_off=0, co_mode=0)
     p.update(over)
     if p["T_top"] is None:
         p["T_top"] = 1.0 - p["eps"] - p["D"]

@@ -71,6 +71,7 @@ def run_case(name: str, device: str = "cuda:0", chunk: int = 2000, every: int = 
         if verbose and len(series) % 10 == 0:
             print(f"  {name}: t = {t:8.2f}  Nu_bar = {d['nu_bar']:.4f}  Nu_bulk = {d['nu_bulk']:.4f}  Re = {d['re']:.3f}", flush=True)
     s.stats_reset()
+    s.stats_flow(True)                   # Sec. 5-6: force balance of Eqs. 40-43, largest Mach number, C of Eq. 49
     t_end = t + c["t_avg"]
     while t < t_end:
         s.step_stats(chunk, every)
@@ -78,6 +79,7 @@ def run_case(name: str, device: str = "cuda:0", chunk: int = 2000, every: int = 
         t = d["time"]
         series.append((t, d["nu_bar"], d["re"]))
     st, Tp, rp, pp = s.stats_read()
+    fl, _ = s.stats_read_flow()
     steps = int(d["step"])
     s.close()
     nu, re = st["nu_bar"], st["re"]
@@ -88,7 +90,9 @@ def run_case(name: str, device: str = "cuda:0", chunk: int = 2000, every: int = 
            "parameters": {k: c[k] for k in ("Ra", "D", "Gamma", "gamma", "Pr", "eps")},
            "steps": steps, "t_end": t, "averaged_over": st["weight"], "samples": st["samples"],
            "nu_bar": nu, "nu_bar_sd": nu_sd, "nu_bulk": st["nu_bulk"], "nu_bottom": st["nu_bottom"], "nu_top": st["nu_top"],
-           "re": re, "re_sd": re_sd,
+           "re": re, "re_sd": re_sd, "nu_conv": st["nu_conv"], "nu_K": st["nu_K"],
+           "corr_C": fl["corr_C"], "max_mach": fl["max_mach"],
+           "force_balance_rms": {k: fl[k + "_rms"] for k in ("Fn", "Fp", "Fb", "Fv")}, "FbFp_mean": fl["FbFp_mean"],
            "paper": {"nu": c["paper"][0], "nu_pm": c["paper"][1], "re": c["paper"][2], "re_pm": c["paper"][3]},
            "earlier_code": {"nu": c["ref"][0], "re": c["ref"][1]},
            "nu_vs_paper_pct": 100.0 * (nu / c["paper"][0] - 1.0), "re_vs_paper_pct": 100.0 * (re / c["paper"][2] - 1.0),
@@ -96,7 +100,8 @@ def run_case(name: str, device: str = "cuda:0", chunk: int = 2000, every: int = 
     if verbose:
         print(f"{name} ({c['cite']}): Nu_bar = {nu:.4f} +- {nu_sd:.4f} (paper {c['paper'][0]} +- {c['paper'][1]}, "
               f"{out['nu_vs_paper_pct']:+.2f} %), Re = {re:.3f} +- {re_sd:.3f} (paper {c['paper'][2]} +- {c['paper'][3]}, "
-              f"{out['re_vs_paper_pct']:+.2f} %), {steps} steps in {out['wall_s']:.0f} s", flush=True)
+              f"{out['re_vs_paper_pct']:+.2f} %), Nu_conv = {st['nu_conv']:.3f}, Nu_K = {st['nu_K']:.3f}, "
+              f"C (Eq. 49) = {fl['corr_C']:.4f}, max Mach = {fl['max_mach']:.4f}, {steps} steps in {out['wall_s']:.0f} s", flush=True)
     return out
 
 

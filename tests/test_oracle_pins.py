@@ -375,6 +375,47 @@ def test_stationary_contact_pins_tvd_coefficient(orc, tvd_form, axis):
     assert amount == (0.25 if tvd_form == 1 else 0.125) * (rl - rr)
 
 
+@pytest.mark.parametrize("tvd_form", [0, 1])
+@pytest.mark.parametrize("axis", [0, 2])
+def test_advective_courant_number_in_the_tvd_coefficient(orc, tvd_form, axis):
+    """co_mode = 1, the second reading of the "local Courant number" of Eq. 39 (R5): Co = |u_alpha| tau/dx.
+    (a) A contact at rest has Co = 0, C = 0: one operator returns X bit for bit (with co_mode = 0 it does not).
+    (b) A contact carried by a uniform flow u along the axis (uniform p, mu = K = g = 0): the TVD term is additive in
+    Eq. 33 and computed from X^n alone, so sweep(TVD on) - sweep(TVD off) = T.  At an isolated jump dX_{k+1/2} =
+    drho (1, u, u^2/2) in (rho, rho u, E) with zero neighbours, r+- = 0, phi = 0, and Co is the SAME number |u| tau/dx
+    at every node, so T = +-C(Co) dX (Davis/Yee sum) or +-C(Co)/2 dX (Eq. 34 as printed), on both branches of Eq. 39."""
+    gam, p0, rl, rr = 1.4, 1.0, 1.0, 0.25
+    n, h = 16, 0.1
+    C = lambda Co: Co * (1.0 - Co) if Co <= 0.5 else 0.25
+    if axis == 0:
+        g, shape = periodic_grid(2, n, 6, lx=n * h, lz=0.6), (1, 1, n)
+    else:
+        g, shape = periodic_grid(2, 6, n, lx=0.6, lz=n * h), (n, 1, 1)
+    i = np.arange(n)
+    heavy = (i >= 4) & (i < 11)
+    rho = np.where(heavy, rl, rr).reshape(shape)
+    p1 = ideal_gas_params(gamma=gam, tvd_form=tvd_form, co_mode=1)
+    X = state_from_primitives(g, p1, rho, 0.0, 0.0, 0.0, p0)
+    for direction in (+1, -1):
+        assert np.array_equal(orc.sweep(orc.Problem(g, p1), X, axis, 0.03, direction), X)
+        p0m = ideal_gas_params(gamma=gam, tvd_form=tvd_form, co_mode=0)
+        assert not np.array_equal(orc.sweep(orc.Problem(g, p0m), X, axis, 0.03, direction), X)
+    for u, tau in ((0.8, 0.02), (-0.8, 0.02), (2.0, 0.04)):          # Co = 0.16, 0.16, 0.8
+        ux, uz = (u, 0.0) if axis == 0 else (0.0, u)
+        X = state_from_primitives(g, p1, rho, ux, 0.0, uz, p0)
+        off = ideal_gas_params(gamma=gam, tvd_off=1)
+        for direction in (+1, -1):
+            T = (orc.sweep(orc.Problem(g, p1), X, axis, tau, direction)
+                 - orc.sweep(orc.Problem(g, off), X, axis, tau, direction)).reshape(4, g["nz"], g["nx"])
+            coef = C(abs(u) * tau / h) * (1.0 if tvd_form == 1 else 0.5)
+            dX = (rl - rr) * np.array([1.0, ux, uz, 0.5 * u * u])    # the jump in (rho, rho u_x, rho u_z, E) at fixed p
+            for f in range(4):
+                line = T[f][:, 2] if axis == 2 else T[f][2, :]
+                want = np.zeros(n)
+                want[3], want[4], want[10], want[11] = +coef * dX[f], -coef * dX[f], -coef * dX[f], +coef * dX[f]
+                np.testing.assert_allclose(line, want, rtol=0, atol=5e-16 * max(1.0, abs(u)) ** 2)
+
+
 def test_contact_next_to_a_plate_records_R11(orc):
     """DESIGN.md R11 (the paper is silent): the dissipation flux of Eq. 34 is dropped on the two interfaces
     that touch a plate node, whose r+- would need a node outside the box.  A contact at rest sitting on the
