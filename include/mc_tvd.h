@@ -72,6 +72,8 @@ typedef struct {
     int tvd_form;                   /* 0 = Eq. 34 as printed; 1 = Davis/Yee sum of two G's (R4) */
     int dir_mode;                   /* 0 = backward predictor always (paper); 1 = alternate per half step (R9) */
     int tvd_off;                    /* 1 = drop the TVD term (tests) */
+    int co_mode;                    /* the "local Courant number" of Eq. 39, which PAPER.md:307 does not define (R5):
+                                       0 = (|u_alpha| + c_s) tau / dx_alpha, 1 = |u_alpha| tau / dx_alpha */
 } mc_tvd_params;
 
 /* Result of mc_tvd_diagnostics (host POD).  Instantaneous values; Eqs. 22-26. */

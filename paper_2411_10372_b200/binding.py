@@ -27,7 +27,8 @@ class Params(C.Structure):          # mc_tvd_params
                 ("D", C.c_double), ("cfl", C.c_double), ("fixed_dt", C.c_double),
                 ("T_bot", C.c_double), ("T_top", C.c_double), ("lambda_coef", C.c_double),
                 ("g_override", C.c_double), ("mu_override", C.c_double), ("K_override", C.c_double),
-                ("bc_z", C.c_int), ("tvd_form", C.c_int), ("dir_mode", C.c_int), ("tvd_off", C.c_int)]
+                ("bc_z", C.c_int), ("tvd_form", C.c_int), ("dir_mode", C.c_int), ("tvd_off", C.c_int),
+                ("co_mode", C.c_int)]
 
 
 class Diag(C.Structure):            # mc_tvd_diag
@@ -147,7 +148,7 @@ def make_params(p: dict) -> Params:
     return Params(p["gamma"], p["Pr"], p["Ra"], p["eps"], p["D"], p["cfl"], p["fixed_dt"],
                   p["T_bot"], p["T_top"], p["lambda_coef"], p["g_override"], p["mu_override"],
                   p["K_override"], int(p["bc_z"]), int(p["tvd_form"]), int(p["dir_mode"]),
-                  int(p["tvd_off"]))
+                  int(p["tvd_off"]), int(p.get("co_mode", 0)))
 
 
 NOALLOC_MAX_NZ = 4096                 # MC_TVD_NOALLOC_MAX_NZ of include/mc_tvd.h

@@ -153,8 +153,8 @@ bool valid_problem(const mc_tvd_grid *g, const mc_tvd_params *p, int *code)
     if (!(p->gamma > 1) || !(p->eps > 0) || !(p->D > 0) || !(p->Pr > 0) || !(p->Ra > 0))
         return fail(0, "need gamma > 1 and eps, D, Pr, Ra > 0"), false;
     if (!(p->fixed_dt > 0) && !(p->cfl > 0)) return fail(0, "need cfl > 0 or fixed_dt > 0"), false;
-    if ((p->bc_z | 1) != 1 || (p->tvd_form | 1) != 1 || (p->dir_mode | 1) != 1 || (p->tvd_off | 1) != 1)
-        return fail(0, "bc_z, tvd_form, dir_mode, tvd_off must be 0 or 1"), false;
+    if ((p->bc_z | 1) != 1 || (p->tvd_form | 1) != 1 || (p->dir_mode | 1) != 1 || (p->tvd_off | 1) != 1 || (p->co_mode | 1) != 1)
+        return fail(0, "bc_z, tvd_form, dir_mode, tvd_off, co_mode must be 0 or 1"), false;
     if (g->z_nodes) {                  // non-uniform z grid (R19): plates at the first and last node
         if (p->bc_z != 0) return fail(0, "z_nodes needs plates (bc_z = 0)"), false;
         for (int k = 0; k + 1 < g->nz; ++k)
@@ -248,6 +248,7 @@ void fill_common(const mc_tvd_state *s, mc::SweepArgs &A, const double *in, doub
     }
     A.R = s->R; A.cv = s->cv; A.icv = s->icv; A.g = s->g;
     A.gamma = s->par.gamma; A.gammaR = s->par.gamma * s->R;
+    A.co_cs = s->par.co_mode ? 0.0 : 1.0;
     A.Tw0 = s->par.T_bot; A.Tw1 = s->par.T_top;
     A.nz = s->grid.nz;
     double D = 0.0;

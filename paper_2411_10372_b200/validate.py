@@ -46,6 +46,21 @@ CASES = {
     "table1-3-tanh": dict(ndim=3, Ra=1e6, D=0.5, Gamma=4.0, gamma=1.4, Pr=0.7, eps=0.1, nx=384, ny=384, nz=129,
                           z_stretch=1.5, t_spin=80.0, t_avg=50.0, paper=(6.89, 0.05, 406.0, 3.0), ref=(6.93, 407.0),
                           cite="Table 1 case 3"),
+    # Table 1 with the advective reading of Eq. 39's local Courant number (co_mode = 1, R5): with the acoustic
+    # one the TVD term damps low-Mach convection
+    **{f"table1-{i + 1}-coadv": dict(ndim=3, Ra=1e6, D=D, Gamma=4.0, gamma=1.4, Pr=0.7, eps=0.1, nx=192, ny=192, nz=65,
+                                     over=dict(co_mode=1), t_spin=80.0, t_avg=60.0, paper=(nu, dnu, re, dre), ref=ref,
+                                     cite=f"Table 1 case {i + 1}")
+       for i, (D, nu, dnu, re, dre, ref) in enumerate(((0.1, 7.90, 0.06, 425.0, 3.0, (7.94, 424.0)),
+                                                       (0.34, 7.67, 0.08, 414.0, 4.0, (7.64, 414.0)),
+                                                       (0.5, 6.89, 0.05, 406.0, 3.0, (6.93, 407.0)),
+                                                       (0.6, 6.18, 0.09, 368.0, 5.0, (6.24, 370.0))))},
+    "table1-1-coadv-384": dict(ndim=3, Ra=1e6, D=0.1, Gamma=4.0, gamma=1.4, Pr=0.7, eps=0.1, nx=384, ny=384, nz=129,
+                               over=dict(co_mode=1), t_spin=80.0, t_avg=50.0, paper=(7.90, 0.06, 425.0, 3.0), ref=(7.94, 424.0),
+                               cite="Table 1 case 1"),
+    "table1-3-coadv-384": dict(ndim=3, Ra=1e6, D=0.5, Gamma=4.0, gamma=1.4, Pr=0.7, eps=0.1, nx=384, ny=384, nz=129,
+                               over=dict(co_mode=1), t_spin=80.0, t_avg=50.0, paper=(6.89, 0.05, 406.0, 3.0), ref=(6.93, 407.0),
+                               cite="Table 1 case 3"),
     # and with every spacing halved (151 M nodes; about an hour on one B200)
     "table1-3-fine": dict(ndim=3, Ra=1e6, D=0.5, Gamma=4.0, gamma=1.4, Pr=0.7, eps=0.1, nx=768, ny=768, nz=257,
                           t_spin=70.0, t_avg=40.0, paper=(6.89, 0.05, 406.0, 3.0), ref=(6.93, 407.0), cite="Table 1 case 3"),

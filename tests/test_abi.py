@@ -36,7 +36,8 @@ def test_every_declared_symbol_is_exported_and_bound(lib):
 def test_struct_layouts_match_header():
     assert C.sizeof(binding.Diag) == 19 * 8
     assert C.sizeof(binding.Grid) == 4 * 4 + 3 * 8 + 8
-    assert C.sizeof(binding.Params) == 13 * 8 + 4 * 4
+    assert C.sizeof(binding.Params) == 13 * 8 + 5 * 4 + 4           # 13 doubles, 5 ints (co_mode the last), padded to 8
+    assert C.sizeof(binding.Forces) == 16 * 8
 
 
 def test_workspace_bytes_and_validation(lib):
@@ -59,6 +60,8 @@ def test_workspace_bytes_and_validation(lib):
     assert lib.mc_tvd_workspace_bytes(C.byref(g), C.byref(pb)) == 0
     pb = binding.make_params(inputs.make_params(tvd_form=2))
     assert lib.mc_tvd_workspace_bytes(C.byref(g), C.byref(pb)) == 0
+    pb = binding.make_params(inputs.make_params(co_mode=2))
+    assert lib.mc_tvd_workspace_bytes(C.byref(g), C.byref(pb)) == 0 and b"co_mode" in lib.mc_tvd_last_error()
     huge = binding.make_grid(inputs.make_grid(3, 2048, 1024, 2048))   # 2^32 nodes per field: 32-bit node offsets
     assert lib.mc_tvd_workspace_bytes(C.byref(huge), C.byref(p)) == 0
     assert b"2^32" in lib.mc_tvd_last_error()

@@ -85,6 +85,43 @@ def test_sweep_parity(gpu, orc, ndim, nx, ny, nz, bc_z, tvd_form, kind):
             assert err <= TOL_SWEEP, (kind, alpha, direction, err)
 
 
+@pytest.mark.parametrize("ndim,nx,ny,nz,stretch", [(2, 300, 1, 70, None), (2, 301, 1, 40, 1.5), (3, 60, 21, 19, None),
+                                                   (3, 45, 17, 14, None), (3, 30, 9, 33, 2.0)])
+@pytest.mark.parametrize("tvd_form", [0, 1])
+def test_sweep_parity_advective_courant_number(gpu, orc, ndim, nx, ny, nz, stretch, tvd_form):
+    """co_mode = 1 (R5, second reading of Eq. 39's local Courant number: |u_alpha| tau / dx): every operator on
+    a rough state, where the TVD term is active and differs from the co_mode = 0 result; then one whole step."""
+    grid = inputs.make_grid(ndim, nx, nz, ny, z_stretch=stretch)
+    params = inputs.make_params(Ra=1e4, tvd_form=tvd_form, co_mode=1)
+    X0 = inputs.rough_random_state(grid, params, seed=23 + nx)
+    prob = orc.Problem(grid, params)
+    tau = 0.25 * orc.dt(prob, X0)
+    for alpha in ((0, 2) if ndim == 2 else (0, 1, 2)):
+        for direction in (1, -1):
+            ref = orc.sweep(prob, X0, alpha, tau, direction)
+            other = orc.sweep(orc.Problem(grid, dict(params, co_mode=0)), X0, alpha, tau, direction)
+            assert rel_err(other, ref).max() > 1e-6                      # the switch matters on this state
+            s = _solver(gpu, grid, params, X0)
+            s.sweep(alpha, direction, tau)
+            err = rel_err(s.state(), ref).max()
+            s.close()
+            assert err <= TOL_SWEEP, (alpha, direction, err)
+    ref, dts, _ = orc.step(prob, X0, 1)
+    s = _solver(gpu, grid, params, X0)
+    s.step(1)
+    err = parity_err(grid, params, s.state(), ref).max()
+    s.close()
+    assert err <= TOL_1STEP, err
+
+
+def test_bad_co_mode_is_rejected(gpu):
+    grid = inputs.make_grid(2, 16, 9)
+    params = inputs.make_params(co_mode=2)
+    with pytest.raises(gpu.MCTVDError) as e:
+        gpu.MCTVD(grid, params, inputs.conduction_state(grid, inputs.make_params()))
+    assert e.value.code == -1
+
+
 @pytest.mark.parametrize("ndim,nx,ny,nz", [(2, 300, 1, 70), (3, 60, 21, 19)])
 @pytest.mark.parametrize("chunk", [7, 16])
 @pytest.mark.parametrize("tvd_form", [0, 1])
