@@ -61,6 +61,13 @@ CASES = {
     "table1-3-coadv-384": dict(ndim=3, Ra=1e6, D=0.5, Gamma=4.0, gamma=1.4, Pr=0.7, eps=0.1, nx=384, ny=384, nz=129,
                                over=dict(co_mode=1), t_spin=80.0, t_avg=50.0, paper=(6.89, 0.05, 406.0, 3.0), ref=(6.93, 407.0),
                                cite="Table 1 case 3"),
+    # The Boussinesq limit as a check of the TVD term at low Mach number (2-D, Ra = 3e4, seconds each): Nu must not depend
+    # on eps.  D = 0.1 (eps = D = 0.02 for the smallest), three treatments of the TVD term.
+    **{f"lowmach-e{eps}-{tag}": dict(ndim=2, Ra=3e4, D=(0.02 if eps == 0.02 else 0.1), Gamma=4.0, gamma=1.4, Pr=0.7, eps=eps,
+                                     nx=256, ny=1, nz=49, over=over, t_spin=150.0, t_avg=50.0, paper=(float("nan"), 0.0, float("nan"), 0.0),
+                                     ref=(float("nan"), float("nan")), cite="Boussinesq limit (no table)")
+       for eps in (0.02, 0.05, 0.1, 0.2)
+       for tag, over in (("default", {}), ("tvdoff", dict(tvd_off=1)), ("coadv", dict(co_mode=1)))},
     # and with every spacing halved (151 M nodes; about an hour on one B200)
     "table1-3-fine": dict(ndim=3, Ra=1e6, D=0.5, Gamma=4.0, gamma=1.4, Pr=0.7, eps=0.1, nx=768, ny=768, nz=257,
                           t_spin=70.0, t_avg=40.0, paper=(6.89, 0.05, 406.0, 3.0), ref=(6.93, 407.0), cite="Table 1 case 3"),
