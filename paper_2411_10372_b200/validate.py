@@ -55,6 +55,12 @@ CASES = {
                                                        (0.34, 7.67, 0.08, 414.0, 4.0, (7.64, 414.0)),
                                                        (0.5, 6.89, 0.05, 406.0, 3.0, (6.93, 407.0)),
                                                        (0.6, 6.18, 0.09, 368.0, 5.0, (6.24, 370.0))))},
+    "table1-2-coadv-384": dict(ndim=3, Ra=1e6, D=0.34, Gamma=4.0, gamma=1.4, Pr=0.7, eps=0.1, nx=384, ny=384, nz=129,
+                               over=dict(co_mode=1), t_spin=80.0, t_avg=50.0, paper=(7.67, 0.08, 414.0, 4.0), ref=(7.64, 414.0),
+                               cite="Table 1 case 2"),
+    "table1-4-coadv-384": dict(ndim=3, Ra=1e6, D=0.6, Gamma=4.0, gamma=1.4, Pr=0.7, eps=0.1, nx=384, ny=384, nz=129,
+                               over=dict(co_mode=1), t_spin=80.0, t_avg=50.0, paper=(6.18, 0.09, 368.0, 5.0), ref=(6.24, 370.0),
+                               cite="Table 1 case 4"),
     "table1-1-coadv-384": dict(ndim=3, Ra=1e6, D=0.1, Gamma=4.0, gamma=1.4, Pr=0.7, eps=0.1, nx=384, ny=384, nz=129,
                                over=dict(co_mode=1), t_spin=80.0, t_avg=50.0, paper=(7.90, 0.06, 425.0, 3.0), ref=(7.94, 424.0),
                                cite="Table 1 case 1"),
