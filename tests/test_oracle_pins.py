@@ -83,7 +83,7 @@ def test_mass_conserved_between_plates(orc):
 
 
 # ----------------------------------------------------------------------------- check 3: Sod
-def _sod(orc, n, axis, tvd_form, ndim=2, t_end=0.2):
+def _sod(orc, n, axis, tvd_form, ndim=2, t_end=0.2, co_mode=0):
     """Classical two-state tube (8:1 density, 10:1 pressure, at rest, gamma 1.4), doubled so the
     periodic box holds two mirrored tubes; returns (x, rho(x), u(x), p(x)) along `axis`."""
     gam = 1.4
@@ -100,7 +100,7 @@ def _sod(orc, n, axis, tvd_form, ndim=2, t_end=0.2):
     else:
         g = periodic_grid(3, m, m, n, lx=m * 2.0 / n, ly=2.0, lz=m * 2.0 / n)
         shape = (1, n, 1)
-    p = ideal_gas_params(gamma=gam, tvd_form=tvd_form)
+    p = ideal_gas_params(gamma=gam, tvd_form=tvd_form, co_mode=co_mode)
     X = state_from_primitives(g, p, rho1.reshape(shape), 0.0, 0.0, 0.0, p1.reshape(shape))
     X, _ = advance_to(orc, orc.Problem(g, p), X, t_end)
     prim = primitives_of(g, p, X)
@@ -146,6 +146,20 @@ def test_tvd_form_decision(orc):
     assert tv(rho1) <= 1.001 * tv0
     assert tv(rho0) > 1.3 * tv0
     assert inputs.make_params()["tvd_form"] == 1
+
+
+def test_courant_number_reading_decision(orc):
+    """DESIGN.md R5: with the acoustic Courant number (co_mode 0) the Sod density stays free of oscillations (total
+    variation non-increasing); with the advective one (co_mode 1) the TVD coefficient is too small at the shock and the
+    total variation grows by a few per cent.  This is why co_mode = 0 is the default although the low-Mach validation
+    runs need co_mode = 1."""
+    tv0 = 2 * 0.875
+    tv = lambda r: np.abs(np.diff(np.r_[r, r[0]])).sum()
+    _, rho_a, _, _ = _sod(orc, 200, 0, tvd_form=1, co_mode=0)
+    _, rho_u, _, _ = _sod(orc, 200, 0, tvd_form=1, co_mode=1)
+    assert tv(rho_a) <= 1.001 * tv0
+    assert 1.01 * tv0 < tv(rho_u) < 1.10 * tv0
+    assert inputs.make_params()["co_mode"] == 0
 
 
 # ----------------------------------------------------------------------------- check 4: convergence
