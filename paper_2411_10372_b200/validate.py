@@ -40,6 +40,12 @@ CASES = {
                      t_spin=150.0, t_avg=50.0, paper=(4.0, 0.1, 100.0, 3.0), ref=(3.9, 102.0), cite="Table 2 case 2"),
     "table2-3": dict(ndim=2, Ra=1e6, D=0.49, Gamma=2.0, gamma=5.0 / 3.0, Pr=0.7, eps=0.1, nx=768, ny=1, nz=385,
                      t_spin=150.0, t_avg=50.0, paper=(7.3, 0.2, 330.0, 7.0), ref=(7.1, 322.0), cite="Table 2 case 3"),
+    # Table 2 with the advective Courant number in Eq. 39 (co_mode = 1): the 2-D cases barely depend on the reading
+    **{f"table2-{i}-coadv": dict(ndim=2, Ra=Ra, D=0.49, Gamma=2.0, gamma=5.0 / 3.0, Pr=0.7, eps=0.1, nx=nx, ny=1, nz=nz,
+                                 over=dict(co_mode=1), t_spin=150.0, t_avg=50.0, paper=paper, ref=ref, cite=f"Table 2 case {i}")
+       for i, Ra, nx, nz, paper, ref in ((1, 1e4, 256, 129, (2.175, 0.005, 26.98, 0.05), (2.1, 26.3)),
+                                         (2, 1e5, 384, 193, (4.0, 0.1, 100.0, 3.0), (3.9, 102.0)),
+                                         (3, 1e6, 768, 385, (7.3, 0.2, 330.0, 7.0), (7.1, 322.0)))},
     "table1-3": dict(ndim=3, Ra=1e6, D=0.5, Gamma=4.0, gamma=1.4, Pr=0.7, eps=0.1, nx=384, ny=384, nz=129,
                      t_spin=80.0, t_avg=50.0, paper=(6.89, 0.05, 406.0, 3.0), ref=(6.93, 407.0), cite="Table 1 case 3"),
     # the same on the paper's kind of grid: levels clustered at the plates (3.3 x finer there, 1.7 x coarser mid-layer)
