@@ -80,6 +80,12 @@ CASES = {
                                      ref=(float("nan"), float("nan")), cite="Boussinesq limit (no table)")
        for eps in (0.02, 0.05, 0.1, 0.2)
        for tag, over in (("default", {}), ("tvdoff", dict(tvd_off=1)), ("coadv", dict(co_mode=1)))},
+    # the same check in 3-D at D = 0.1 (Gamma = 4, gamma = 1.4, Pr = 0.7): default readings against co_mode = 1
+    **{f"lowmach3d-Ra{Ra:g}-{tag}": dict(ndim=3, Ra=Ra, D=0.1, Gamma=4.0, gamma=1.4, Pr=0.7, eps=0.1, nx=n, ny=n, nz=nz, over=over,
+                                         t_spin=120.0, t_avg=80.0, paper=(float("nan"), 0.0, float("nan"), 0.0),
+                                         ref=(float("nan"), float("nan")), cite="Boussinesq limit (no table)")
+       for Ra, n, nz in ((3e4, 128, 49), (1e5, 192, 65), (3e5, 256, 97))
+       for tag, over in (("default", {}), ("coadv", dict(co_mode=1)))},
     # and with every spacing halved (151 M nodes; about an hour on one B200)
     "table1-3-fine": dict(ndim=3, Ra=1e6, D=0.5, Gamma=4.0, gamma=1.4, Pr=0.7, eps=0.1, nx=768, ny=768, nz=257,
                           t_spin=70.0, t_avg=40.0, paper=(6.89, 0.05, 406.0, 3.0), ref=(6.93, 407.0), cite="Table 1 case 3"),
