@@ -17,6 +17,12 @@ import time
 from . import inputs
 
 # PAPER.md:331-345.  `paper` = (Nu, +-, Re, +-) of "our simulations"; `ref` = the earlier code's (Nu, Re).
+def _rho_mean(D: float, eps: float = 0.1, gamma: float = 1.4) -> float:
+    """Mean density of the hydrostatic conduction state rho = T^m, T = 1 - (eps + D) z (bottom density 1)."""
+    m = gamma * D / ((gamma - 1.0) * (eps + D)) - 1.0
+    return (1.0 - (1.0 - eps - D) ** (m + 1.0)) / ((eps + D) * (m + 1.0))
+
+
 CASES = {
     "table2-1": dict(ndim=2, Ra=1e4, D=0.49, Gamma=2.0, gamma=5.0 / 3.0, Pr=0.7, eps=0.1, nx=256, ny=1, nz=129,
                      t_spin=150.0, t_avg=50.0, paper=(2.175, 0.005, 26.98, 0.05), ref=(2.1, 26.3), cite="Table 2 case 1"),
@@ -86,6 +92,17 @@ CASES = {
                                          ref=(float("nan"), float("nan")), cite="Boussinesq limit (no table)")
        for Ra, n, nz in ((3e4, 128, 49), (1e5, 192, 65), (3e5, 256, 97))
        for tag, over in (("default", {}), ("coadv", dict(co_mode=1)))},
+    # A lead on the D trend of Table 1: mu and K multiplied by the MEAN density of the layer
+    # (= the conserved mass per area, from the polytropic conduction state), i.e. a Rayleigh number that refers to the
+    # mean instead of the bottom density.  Re of Eq. 26 must then be divided by the same factor.
+    **{f"table1-{i + 1}-coadv-rhomean": dict(ndim=3, Ra=1e6, D=D, Gamma=4.0, gamma=1.4, Pr=0.7, eps=0.1, nx=192, ny=192, nz=65,
+                                             over=dict(co_mode=1, mu_override=_rho_mean(D) * (0.7 / 1e6) ** 0.5,
+                                                       K_override=_rho_mean(D) / (0.1 * D * (1e6 * 0.7) ** 0.5)),
+                                             t_spin=80.0, t_avg=60.0, paper=(nu, dnu, re, dre), ref=ref, cite=f"Table 1 case {i + 1}")
+       for i, (D, nu, dnu, re, dre, ref) in enumerate(((0.1, 7.90, 0.06, 425.0, 3.0, (7.94, 424.0)),
+                                                       (0.34, 7.67, 0.08, 414.0, 4.0, (7.64, 414.0)),
+                                                       (0.5, 6.89, 0.05, 406.0, 3.0, (6.93, 407.0)),
+                                                       (0.6, 6.18, 0.09, 368.0, 5.0, (6.24, 370.0))))},
     # and with every spacing halved (151 M nodes; about an hour on one B200)
     "table1-3-fine": dict(ndim=3, Ra=1e6, D=0.5, Gamma=4.0, gamma=1.4, Pr=0.7, eps=0.1, nx=768, ny=768, nz=257,
                           t_spin=70.0, t_avg=40.0, paper=(6.89, 0.05, 406.0, 3.0), ref=(6.93, 407.0), cite="Table 1 case 3"),
