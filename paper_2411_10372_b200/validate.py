@@ -103,6 +103,10 @@ CASES = {
                                                        (0.34, 7.67, 0.08, 414.0, 4.0, (7.64, 414.0)),
                                                        (0.5, 6.89, 0.05, 406.0, 3.0, (6.93, 407.0)),
                                                        (0.6, 6.18, 0.09, 368.0, 5.0, (6.24, 370.0))))},
+    "table1-3-coadv-rhomean-384": dict(ndim=3, Ra=1e6, D=0.5, Gamma=4.0, gamma=1.4, Pr=0.7, eps=0.1, nx=384, ny=384, nz=129,
+                                       over=dict(co_mode=1, mu_override=_rho_mean(0.5) * (0.7 / 1e6) ** 0.5,
+                                                 K_override=_rho_mean(0.5) / (0.1 * 0.5 * (1e6 * 0.7) ** 0.5)),
+                                       t_spin=80.0, t_avg=50.0, paper=(6.89, 0.05, 406.0, 3.0), ref=(6.93, 407.0), cite="Table 1 case 3"),
     # and with every spacing halved (151 M nodes; about an hour on one B200)
     "table1-3-fine": dict(ndim=3, Ra=1e6, D=0.5, Gamma=4.0, gamma=1.4, Pr=0.7, eps=0.1, nx=768, ny=768, nz=257,
                           t_spin=70.0, t_avg=40.0, paper=(6.89, 0.05, 406.0, 3.0), ref=(6.93, 407.0), cite="Table 1 case 3"),
